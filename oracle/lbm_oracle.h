@@ -1,0 +1,83 @@
+/*
+ * CPU ORACLE -- TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, double-precision restatement of the coupled phase-field lattice Boltzmann step of
+ * Verdier, Kestener, Cartalade, "Performance portability of lattice Boltzmann methods for two-phase
+ * flows with phase change", following the paper's equations pass by pass (separate
+ * derive / collide / stream / moment loops, no fusion, no blocking).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may use
+ * anything under oracle/.  The product (paper_2003_06342_b200/) never includes, links or imports it,
+ * and this directory shares no header, table or helper with the CUDA path.
+ *
+ * Readings of garbled / silent passages of the paper are the ones listed in DESIGN.md ("Readings");
+ * tags G* / S* in comments refer to that list.
+ *
+ * Parity unpinned: discretisation of div(u phi) (S5), the OPEN pressure face (S12),
+ * the 3D coupling terms beyond symmetry checks (A34).  Everything else is pinned by tests/test_oracle_*.py.
+ */
+#ifndef LBM_ORACLE_H
+#define LBM_ORACLE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* lattice ids (D2Q5 is not in the paper, reading S1) */
+enum { ORA_D2Q5 = 0, ORA_D2Q9 = 1, ORA_D3Q7 = 2, ORA_D3Q19 = 3 };
+/* boundary kinds of the Navier-Stokes distribution f, per face */
+enum { ORA_F_PERIODIC = 0, ORA_F_WALL = 1 /* half bounce-back */,
+       ORA_F_OPEN = 2 /* pressure anti-bounce-back, reading S12 */ };
+/* boundary kinds of the scalar distributions g (phase field) and s (temperature), per face */
+enum { ORA_S_PERIODIC = 0, ORA_S_ZEROFLUX = 1 /* bounce-back */,
+       ORA_S_DIRICHLET = 2 /* anti-bounce-back */ };
+/* flags */
+enum { ORA_PHASE_CHANGE = 1u /* Eq.(18) production rate on */,
+       ORA_LATENT_HEAT = 2u /* Eq.(33c,d),(34) source of the heat equation on */ };
+/* conservative Allen-Cahn collision form */
+enum { ORA_CAC_MODIFIED_EQ = 0 /* Eq.(31a,b) */, ORA_CAC_SOURCE = 1 /* Eq.(29a,b),(30a,b) */ };
+/* stage selector of oracle_read_pops */
+enum { ORA_POPS_POSTCOLLISION = 0, ORA_POPS_STREAMED = 1 };
+
+typedef struct oracle_params {
+    int nx, ny, nz;               /* nz == 1 : two-dimensional                                   */
+    int lat_f, lat_g, lat_s;      /* lattice of f (NS), g (Allen-Cahn), s (heat)                 */
+    int bc_f[3][2];               /* [axis][lo,hi]                                               */
+    int bc_g[3][2];
+    int bc_s[3][2];
+    double bc_phi[3][2];          /* Dirichlet values of phi                                     */
+    double bc_T[3][2];            /* Dirichlet values of T                                       */
+    double bc_p[3][2];            /* pressure of OPEN faces                                      */
+    double dx, dt;
+    double rho_l, rho_g, nu_l, nu_g;
+    double sigma, W, M;           /* surface tension, interface width, mobility                  */
+    double grav[3];               /* gravity acceleration vector g (points "down")               */
+    double alpha_l, alpha_g;      /* thermal diffusivities                                       */
+    double L_latent, Cp, T_sat, theta_I;
+    double A;                     /* script-A of Eq.(18); 10/48 in the paper      */
+    double eps_n;                 /* regularisation of n = grad phi / |grad phi| (reading S7)    */
+    unsigned flags;
+} oracle_params;
+
+typedef struct oracle_ctx oracle_ctx;
+
+/* returns NULL on invalid parameters */
+oracle_ctx *oracle_create(const oracle_params *p);
+void oracle_destroy(oracle_ctx *c);
+/* arrays are x-fastest [z][y][x]; u is [comp][z][y][x] with 3 components; NULL => u=0, p=0, T=T_sat */
+int oracle_init(oracle_ctx *c, const double *phi, const double *T, const double *u, const double *p);
+int oracle_step(oracle_ctx *c, int n);
+int oracle_read_macro(oracle_ctx *c, double *phi, double *u, double *p, double *T);
+/* which: 0=f, 1=g, 2=s ; out is [Q][z][y][x] */
+int oracle_read_pops(oracle_ctx *c, int which, int stage, double *out);
+/* auxiliary fields for the pins: grad phi [3][N], laplacian [N], production rate Pdot [N], dphi/dt [N] */
+int oracle_read_aux(oracle_ctx *c, double *grad, double *lap, double *pdot, double *dtphi);
+void oracle_set_cac_form(oracle_ctx *c, int form);
+int oracle_num_threads(void);
+/* lattice table access for the pins: returns Q, fills e[Q][3], w[Q], *e2 */
+int oracle_lattice(int id, int *e, double *w, double *e2);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

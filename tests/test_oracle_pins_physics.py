@@ -1,0 +1,208 @@
+"""Pins of the CPU oracle against closed forms the paper fixes (north_star list):
+P2 equilibrium tanh profile, P4 Laplace jump, P6 Poiseuille, P8 diffusion decay (lattice e2), P9 Dirichlet
+anti-bounce-back, P10 discrete enthalpy invariant, P11 the paper's Stefan set-up with the printed xi,
+P12 config-2 one-phase Stefan, G6 buoyancy direction."""
+import math
+
+import numpy as np
+import pytest
+
+import analytic
+from paper_2003_06342_b200 import workloads as wl
+
+
+def _interface(row, rising):
+    x = np.arange(len(row)) + 0.5
+    if rising:
+        j = np.where((row[:-1] < 0.5) & (row[1:] >= 0.5))[0][0]
+    else:
+        j = np.where((row[:-1] >= 0.5) & (row[1:] < 0.5))[0][0]
+    return x[j] + (0.5 - row[j]) / (row[j + 1] - row[j])
+
+
+def test_flat_interface_keeps_tanh_profile(oracle_mod):
+    """P2: Eq.(7),(8): a plane interface initialised with the kernel function stays put."""
+    ny, W = 64, 4.0
+    P = wl.base_params(4, ny, 1, phase_change=False, latent_heat=False)
+    y = np.arange(ny) + 0.5
+    prof = 0.5 * (np.tanh(2 * (y - 16) / W) - np.tanh(2 * (y - 48) / W))
+    phi0 = np.tile(prof[None, :, None], (1, 1, 4))
+    o = oracle_mod.Oracle(P)
+    o.init(phi0)
+    o.step(2000)
+    phi, u, _, _ = o.read_macro()
+    assert np.abs(phi - phi0).max() < 1e-2          # O((dx/W)^2) relaxation of the discrete profile
+    assert abs(_interface(phi[0, :, 0], True) - 16.0) < 1e-3
+    assert np.abs(u).max() < 1e-7
+    grad, _, _, _ = o.read_aux()
+    gn = np.sqrt((grad ** 2).sum(0))
+    assert np.abs(gn - 4 * phi * (1 - phi) / W).max() < 0.1 / W   # Eq.(8) to discretisation error
+    o.close()
+
+
+def _laplace_ratio(oracle_mod, n, R, W, steps, avg):
+    P, I = wl.config1_droplet(n=n, radius=R, W=W, noise=0.0)
+    o = oracle_mod.Oracle(P)
+    o.init(I["phi"], I["T"])
+    o.step(steps - avg)
+    acc, cnt = 0.0, 0
+    for _ in range(avg // 50):
+        o.step(50)
+        p = o.read_macro()[2]
+        acc += p[0, n // 2, n // 2] - p[0, 0, 0]
+        cnt += 1
+    u = o.read_macro()[1]
+    o.close()
+    return acc / cnt / (P["sigma"] / R), np.abs(u).max()
+
+
+def test_laplace_pressure_jump(oracle_mod):
+    """P4: Eq.(39) p_in - p_out = sigma/R on config 1 (R=16, W=4); the deficit is the
+    O((dx/W)^2) discretisation error of the diffuse interface and shrinks like 1/W^2 (R=24, W=6)."""
+    r4, umax = _laplace_ratio(oracle_mod, 64, 16.0, 4.0, 6000, 1000)
+    assert 0.90 < r4 < 0.97, r4
+    assert umax < 5e-6                                # spurious currents
+    r6, _ = _laplace_ratio(oracle_mod, 96, 24.0, 6.0, 6000, 1000)
+    assert 0.95 < r6 < 1.0 and (1 - r6) < 0.6 * (1 - r4), (r4, r6)
+
+
+def test_poiseuille(oracle_mod):
+    """P6: single fluid (phi = 1) between half-way bounce-back walls, uniform body force G from the buoyancy
+    term: steady second difference of u_x equals -G/(rho nu) and the profile is the parabola."""
+    G, ny, nu = 1e-6, 32, 0.1
+    P = wl.base_params(4, ny, 1, rho_g=1.0, rho_l=2.0, grav=[-G, 0, 0], phase_change=False, latent_heat=False,
+                       nu_l=nu, nu_g=nu)
+    P["bc_f"][1] = ["wall", "wall"]; P["bc_g"][1] = ["zeroflux", "zeroflux"]; P["bc_s"][1] = ["zeroflux", "zeroflux"]
+    o = oracle_mod.Oracle(P)
+    o.init(np.ones((1, ny, 4)))
+    o.step(20000)
+    phi, u, _, _ = o.read_macro()
+    ux = u[0][0, :, 0]
+    y = np.arange(ny) + 0.5
+    exact = G / (2 * nu) * y * (ny - y)
+    assert np.abs(ux - exact).max() / exact.max() < 1e-3
+    d2 = ux[2:] - 2 * ux[1:-1] + ux[:-2]
+    assert np.abs(d2 + G / nu).max() < 1e-6 * G / nu
+    assert np.abs(u[1]).max() < 1e-12 and np.abs(phi - 1).max() < 1e-10
+    o.close()
+
+
+@pytest.mark.parametrize("lat,dims", [("D2Q5", (32, 4, 1)), ("D2Q9", (32, 4, 1)), ("D3Q7", (32, 4, 4))])
+def test_temperature_diffusion_decay(oracle_mod, lat, dims):
+    """P8: T = sin(kx) exp(-alpha k^2 t) in pure liquid at rest; pins tau_s <-> alpha with each lattice's e2
+     -- a wrong e2 (1/3 for D3Q7) changes the rate by 33%."""
+    P = wl.base_params(*dims, phase_change=False, latent_heat=False, lat_s=lat, alpha_l=0.03, alpha_g=0.07)
+    nz, ny, nx = dims[::-1]
+    x = np.arange(nx) + 0.5
+    k = 2 * np.pi / nx
+    T = np.tile(np.sin(k * x)[None, None, :], (nz, ny, 1))
+    o = oracle_mod.Oracle(P)
+    o.init(np.zeros((nz, ny, nx)), T)
+    o.step(200)
+    Tn = o.read_macro()[3]
+    amp = (Tn[0, 0, :] * np.sin(k * x)).sum() * 2 / nx
+    rate = -math.log(amp) / 200
+    assert abs(rate / (0.03 * k * k) - 1) < 0.03
+    o.close()
+
+
+def test_dirichlet_anti_bounce_back_linear_profile(oracle_mod):
+    """P9: steady T between two anti-bounce-back walls is linear, walls half a cell outside."""
+    P = wl.base_params(4, 16, 1, phase_change=False, latent_heat=False)
+    P["bc_f"][1] = ["wall", "wall"]; P["bc_g"][1] = ["zeroflux", "zeroflux"]
+    P["bc_s"][1] = ["dirichlet", "dirichlet"]; P["bc_T"][1] = [1.0, 0.25]
+    o = oracle_mod.Oracle(P)
+    o.init(np.zeros((1, 16, 4)), np.zeros((1, 16, 4)))
+    o.step(30000)
+    T = o.read_macro()[3][0, :, 0]
+    y = np.arange(16) + 0.5
+    assert np.abs(T - (1.0 + (0.25 - 1.0) * y / 16)).max() < 1e-9
+    o.close()
+
+
+def test_discrete_enthalpy_invariant(oracle_mod):
+    """P10: sum_x [T^n + (L/2Cp)(phi^n + phi^{n-1})] is conserved to round-off on a periodic box with phase
+    change on and the flow frozen (rho_l = rho_g, sigma = 0 => u = 0 exactly).  Pins the sign of Eq.(33d)
+    (reading G2), the lagging rule S3 and the backward difference S4: any other choice drifts."""
+    P, I = wl.config1_droplet(n=48, radius=12.0, rho_l=1.0, rho_g=1.0, sigma=0.0)
+    P["phase_change"] = True; P["latent_heat"] = True
+    rng = np.random.Generator(np.random.PCG64(7))
+    T = 0.2 * rng.uniform(-1, 1, (1, 48, 48)) + 0.1
+    o = oracle_mod.Oracle(P)
+    o.init(I["phi"], T)
+    LC = P["L_latent"] / P["Cp"]
+    prev = I["phi"].copy()
+    inv = []
+    for _ in range(200):
+        o.step(1)
+        ph, u, _, Tn = o.read_macro()
+        inv.append((Tn + 0.5 * LC * (ph + prev)).sum())
+        prev = ph
+    inv = np.array(inv)
+    assert np.abs(u).max() == 0.0
+    assert np.abs(ph - I["phi"]).max() > 1e-2         # the interface really moved
+    assert np.abs(inv - inv[0]).max() < 1e-10 * abs(inv[0])
+    o.close()
+
+
+def _paper_stefan(oracle_mod, alpha_l, alpha_g, theta_I, steps):
+    """The paper's condensation set-up: 512 x ny, D2Q9 for phi and T, u = 0, W = 3, M = 0.08,
+    theta_w = -0.3, theta_inf = 0.3, Dirichlet anti-bounce-back on both x faces, phi(x,0) = (1+tanh(2x/W))/2."""
+    nx, ny = 512, 2
+    P = wl.base_params(nx, ny, 1, lat_s="D2Q9", rho_l=1.0, rho_g=1.0, sigma=0.0, W=3.0, M=0.08, Cp=1.0,
+                       L_latent=1.0, alpha_l=alpha_l, alpha_g=alpha_g, theta_I=theta_I)
+    P["bc_f"][0] = ["wall", "wall"]; P["bc_g"][0] = ["dirichlet", "dirichlet"]; P["bc_s"][0] = ["dirichlet", "dirichlet"]
+    P["bc_phi"][0] = [0.0, 1.0]; P["bc_T"][0] = [-0.3, 0.3]
+    x = (np.arange(nx) + 0.5)[None, None, :]
+    phi = 0.5 * (1 + np.tanh(2 * x / 3.0)) + np.zeros((1, ny, 1))
+    o = oracle_mod.Oracle(P)
+    o.init(phi, np.full((1, ny, nx), 0.3))
+    o.step(steps)
+    ph, u, _, _ = o.read_macro()
+    o.close()
+    assert np.abs(u).max() == 0.0
+    return _interface(ph[0, 0, :], True)
+
+
+def test_stefan_paper_setup_equal_diffusivities(oracle_mod):
+    """P11: x_I = 2 xi sqrt(alpha_l t), Eq.(41a), with the xi the paper prints: pins Eq.(18),
+    script-A = 10/48, the sign G2 and the coupling order S3/S4."""
+    xi = 0.280680
+    steps = 10000
+    x_i = _paper_stefan(oracle_mod, 0.14, 0.14, 0.0, steps)
+    assert abs(x_i / (2 * xi * math.sqrt(0.14 * steps)) - 1) < 3e-3
+
+
+def test_stefan_paper_setup_diffusivity_ratio_10(oracle_mod):
+    """P11: alpha_l/alpha_g = 10, theta_I = 0.05, xi = 0.349635: pins alpha(phi) (reading S6) and theta_I."""
+    xi = 0.349635
+    steps = 10000
+    x_i = _paper_stefan(oracle_mod, 0.14, 0.014, 0.05, steps)
+    assert abs(x_i / (2 * xi * math.sqrt(0.14 * steps)) - 1) < 3e-2
+
+
+def test_config2_one_phase_stefan_flow_frozen(oracle_mod):
+    """P12: config 2 (evaporation, hot wall, vapour at the wall) with the flow frozen follows the one-phase
+    solution x_I = 2 xi sqrt(alpha_g (t + t0)), xi exp(xi^2) erf(xi) = St/sqrt(pi)."""
+    P, I = wl.config2_stefan(nx=512, ny=4, open_right=False, rho_l=1.0, rho_g=1.0, sigma=0.0)
+    o = oracle_mod.Oracle(P)
+    o.init(I["phi"], I["T"])
+    o.step(10000)
+    ph, u, _, _ = o.read_macro()
+    ana = 2 * I["xi"] * math.sqrt(P["alpha_g"] * (10000 + I["t0"]))
+    assert ana - 32.0 > 1.4                            # the interface has moved by ~1.5 cells
+    assert abs(_interface(ph[0, 0, :], False) - ana) < 0.02
+    assert np.abs(ph - ph[:, 0:1, :]).max() == 0.0     # y-invariance
+    o.close()
+
+
+def test_gas_bubble_rises(oracle_mod):
+    """G6: with g pointing down, a gas bubble in liquid must accelerate upward."""
+    P, I = wl.config1_droplet(n=48, radius=10.0, grav=[0, -1e-4, 0])
+    phi = 1 - I["phi"]
+    o = oracle_mod.Oracle(P)
+    o.init(phi, I["T"])
+    o.step(200)
+    ph, u, _, _ = o.read_macro()
+    assert (u[1] * ph).sum() / ph.sum() > 1e-3
+    o.close()
