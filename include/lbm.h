@@ -1,0 +1,163 @@
+/*
+ * lbm.h -- C ABI of the B200-native coupled phase-field lattice Boltzmann step.
+ *
+ * The library advances, per time step, the three coupled BGK lattice Boltzmann distributions of
+ * Verdier, Kestener, Cartalade (arXiv 2003.06342; citations are PAPER.md:<line>):
+ *   f  incompressible Navier-Stokes with surface tension, buoyancy and phase-change source
+ *      (Eq.26a,b 27a-d 28a,b),
+ *   g  conservative Allen-Cahn phase field, modified-equilibrium form (Eq.31a,b 32),
+ *   s  temperature with latent-heat source (Eq.33a-d 34),
+ * coupled through grad phi / lap phi (Eq.35,36), the chemical potential (Eq.14;
+ * PAPER.md:118) and the production rate (Eq.18).  Every step of that path runs in
+ * hand-written sm_100a CUDA kernels; there is no CPU fallback.  The readings taken where the paper is
+ * garbled or silent are listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Fields are x-fastest, [z][y][x]; vector fields [comp][z][y][x] with 3 components (u_z = 0 in 2D);
+ *     populations [Q][z][y][x] in the direction order documented in DESIGN.md ("Lattices").
+ *   - "h_" pointers are HOST memory (pageable or pinned), "d_" pointers are DEVICE memory.
+ *   - Element type of every field pointer is the context's precision: double (64) or float (32).
+ *   - All calls return 0 (LBM_OK) or a negative LBM_E_* code; nothing throws across this boundary.
+ *   - A context is bound to one device, one stream; calls on one context must not race.
+ */
+#ifndef LBM_H
+#define LBM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* lattices, PAPER.md:190 (D2Q5 is not in the paper: DESIGN.md reading S1) */
+enum { LBM_D2Q5 = 0, LBM_D2Q9 = 1, LBM_D3Q7 = 2, LBM_D3Q19 = 3 };
+
+/* boundary rule of f on a face */
+enum {
+    LBM_F_PERIODIC = 0,
+    LBM_F_WALL = 1, /* no-slip half bounce-back */
+    LBM_F_OPEN = 2  /* pressure anti-bounce-back f_i = -f*_ibar + 2 w_i p_face (reading S12) */
+};
+/* boundary rule of g (phase field) and s (temperature) on a face */
+enum {
+    LBM_S_PERIODIC = 0,
+    LBM_S_ZEROFLUX = 1, /* bounce-back */
+    LBM_S_DIRICHLET = 2 /* anti-bounce-back s_i = -s*_ibar + 2 w_i value */
+};
+
+/* flags */
+#define LBM_FLAG_PHASE_CHANGE 1u /* production rate Eq.(18) on (otherwise m''' = 0)        */
+#define LBM_FLAG_LATENT_HEAT 2u  /* source of the heat equation Eq.(33c,d),(34) on          */
+
+/* error codes */
+enum {
+    LBM_OK = 0,
+    LBM_E_INVALID = -1,   /* bad argument / parameter combination                         */
+    LBM_E_UNSUPPORTED = -2, /* lattice set or precision not built                          */
+    LBM_E_WORKSPACE = -3, /* workspace too small or misaligned                             */
+    LBM_E_CUDA = -4,      /* a CUDA runtime call failed (lbm_last_cuda_error for the code) */
+    LBM_E_STATE = -5,     /* call not valid in this state (e.g. step before init)          */
+    LBM_E_NODEVICE = -6   /* no sm_100 device / kernels not loadable                       */
+};
+
+/* which-population selectors and stages of lbm_read_pops */
+enum { LBM_POPS_F = 0, LBM_POPS_G = 1, LBM_POPS_S = 2 };
+enum {
+    LBM_STAGE_POSTCOLLISION = 0, /* what the library stores: collided at the current level, not streamed */
+    LBM_STAGE_STREAMED = 1       /* arrived at the node at the current level (post-pull, post-BC);        */
+                                 /* needs at least one step since init                                   */
+};
+
+/*
+ * Problem description; plain data, copied by lbm_create.
+ * nz == 1 selects 2D (lattices must be D2Q*), nz > 1 selects 3D (D3Q*).
+ * Supported lattice sets (f, g, s): (D2Q9, D2Q9, D2Q5), (D2Q9, D2Q9, D2Q9), (D3Q19, D3Q7, D3Q7).
+ * bc_*[axis][side]: axis 0,1,2 = x,y,z; side 0 = low face, 1 = high face.  A periodic face must be
+ * periodic on both sides and for all three distributions.  Walls sit half a cell outside the first/last
+ * node (node i is at (i + 1/2) dx).
+ */
+typedef struct lbm_params {
+    int nx, ny, nz;
+    int lat_f, lat_g, lat_s;
+    int precision;          /* 64 or 32: storage and arithmetic type                                */
+    int bc_f[3][2];         /* LBM_F_*                                                              */
+    int bc_g[3][2];         /* LBM_S_* for the phase field                                          */
+    int bc_s[3][2];         /* LBM_S_* for the temperature                                          */
+    double bc_phi[3][2];    /* Dirichlet value of phi per face                                      */
+    double bc_T[3][2];      /* Dirichlet value of T per face                                        */
+    double bc_p[3][2];      /* pressure of LBM_F_OPEN faces                                         */
+    double dx, dt;          /* space and time step; c = dx/dt                                       */
+    double rho_l, rho_g;    /* bulk densities, Eq.(1a)                                              */
+    double nu_l, nu_g;      /* kinematic viscosities, harmonic interpolation Eq.(1b)                */
+    double sigma, W, M;     /* surface tension, interface width, mobility (Eq.15b, 5)               */
+    double grav[3];         /* gravity acceleration g; F_v = (rho - rho_l) g (reading G6) */
+    double alpha_l, alpha_g;/* thermal diffusivities, linear in phi (reading S6)          */
+    double L_latent, Cp;    /* latent heat and specific heat; theta = Cp (T - T_sat)/L              */
+    double T_sat, theta_I;  /* saturation temperature; dimensionless interface temperature          */
+    double A;               /* script-A of Eq.(18): 10/48 in the paper               */
+    double eps_n;           /* n = grad phi / sqrt(|grad phi|^2 + eps_n^2) (reading S7)   */
+    unsigned flags;         /* LBM_FLAG_*                                                           */
+} lbm_params;
+
+typedef struct lbm_ctx lbm_ctx;
+
+/* Bytes of device memory a context for *p needs (0 if p is invalid).  The caller allocates it (e.g. with
+ * torch.empty(..., device="cuda")), 256-byte aligned, and lends it to the context until lbm_destroy. */
+size_t lbm_workspace_bytes(const lbm_params *p);
+
+/* Validate *p and build a context on the current CUDA device.  d_workspace: DEVICE pointer, >= bytes from
+ * lbm_workspace_bytes, borrowed (never freed by the library).  cuda_stream: a cudaStream_t (NULL = legacy
+ * default stream) on which every kernel and copy of this context is enqueued.  *out receives the context
+ * (owned by the library; release with lbm_destroy). */
+int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_stream, lbm_ctx **out);
+
+/* Set the state of time level 0 from HOST arrays (element type = precision).  h_phi is required; h_T, h_u,
+ * h_p may be NULL (T = T_sat, u = 0, p = 0).  Sets dphi/dt = 0, the production field from the initial macros
+ * (Eq.18) and the populations to bar-equilibrium theta_eq - dt/2 S (Eq.24; DESIGN.md reading
+ * S9), then collides once so that the stored state is post-collision at level 0.  Resets the step counter.
+ * Synchronises the stream before returning (the host arrays may be reused at once). */
+int lbm_init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, const void *h_p);
+
+/* Enqueue n full coupled steps (each: K_phi = pull g + Eq.32, then K_main = stencils, closures, moments,
+ * production refresh, collision of f, g, s) on the context's stream.  Asynchronous: returns after the
+ * launches; launch errors are returned, execution errors surface at the next synchronising call.
+ * The last of the n steps also stores u, p, T for lbm_read_macro. */
+int lbm_step(lbm_ctx *c, int n);
+
+/* Copy the macroscopic fields of the current time level to HOST arrays; any pointer may be NULL.
+ * h_u is [3][z][y][x].  Synchronises. */
+int lbm_read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T);
+
+/* Debug / parity access: copy populations [Q][z][y][x] of lattice `which` at `stage` to HOST.  Synchronises.
+ * Not on the hot path. */
+int lbm_read_pops(lbm_ctx *c, int which, int stage, void *h_pops);
+
+/* Block until everything enqueued on the context's stream has finished; returns LBM_E_CUDA on a fault. */
+int lbm_sync(lbm_ctx *c);
+
+/* Per-kernel device timing for measurement (off by default).  While enabled, lbm_step brackets K_phi and K_main of
+ * every step (at most 4096 steps between two lbm_kernel_times calls) with CUDA events on the context's stream.
+ * lbm_kernel_times synchronises, returns the summed durations in milliseconds and the number of timed steps,
+ * and clears the record.  Any output pointer may be NULL. */
+int lbm_set_timing(lbm_ctx *c, int enable);
+int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *steps);
+
+/* Counters: steps taken since init; kernels launched by this context since creation. */
+long long lbm_step_count(const lbm_ctx *c);
+long long lbm_launch_count(const lbm_ctx *c);
+
+/* Names of the kernel variant the context launches for K_main ("direct" or "tma"), for logs. */
+const char *lbm_variant(const lbm_ctx *c);
+
+/* Last CUDA runtime error code seen by this library (cudaError_t as int), 0 if none. */
+int lbm_last_cuda_error(void);
+
+const char *lbm_strerror(int code);
+
+/* Release the host context (NULL-safe).  Does not free the borrowed workspace. */
+void lbm_destroy(lbm_ctx *c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_H */

@@ -1,0 +1,237 @@
+"""Thin Python binding of the C ABI in ``include/lbm.h`` (argument marshalling only).
+
+Same names as the C calls: :func:`lbm_workspace_bytes`, :class:`LBM` with ``init / step / read_macro / read_pops /
+sync / destroy``.  PyTorch is used for the device allocation and the CUDA stream only; every step of the path runs
+in the library's kernels.  There is no CPU fallback: a missing library or a missing GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblbm_b200.so")
+
+LATTICES = {"D2Q5": 0, "D2Q9": 1, "D3Q7": 2, "D3Q19": 3}
+LATTICE_Q = {"D2Q5": 5, "D2Q9": 9, "D3Q7": 7, "D3Q19": 19}
+F_KINDS = {"periodic": 0, "wall": 1, "open": 2}
+S_KINDS = {"periodic": 0, "zeroflux": 1, "dirichlet": 2}
+FLAG_PHASE_CHANGE = 1
+FLAG_LATENT_HEAT = 2
+POPS_F, POPS_G, POPS_S = 0, 1, 2
+STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
+
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_read_macro", "lbm_read_pops",
+           "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
+           "lbm_destroy"]
+
+
+class lbm_params(C.Structure):
+    """Mirror of ``struct lbm_params`` (include/lbm.h)."""
+    _fields_ = [
+        ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+        ("lat_f", C.c_int), ("lat_g", C.c_int), ("lat_s", C.c_int),
+        ("precision", C.c_int),
+        ("bc_f", (C.c_int * 2) * 3), ("bc_g", (C.c_int * 2) * 3), ("bc_s", (C.c_int * 2) * 3),
+        ("bc_phi", (C.c_double * 2) * 3), ("bc_T", (C.c_double * 2) * 3), ("bc_p", (C.c_double * 2) * 3),
+        ("dx", C.c_double), ("dt", C.c_double),
+        ("rho_l", C.c_double), ("rho_g", C.c_double), ("nu_l", C.c_double), ("nu_g", C.c_double),
+        ("sigma", C.c_double), ("W", C.c_double), ("M", C.c_double),
+        ("grav", C.c_double * 3),
+        ("alpha_l", C.c_double), ("alpha_g", C.c_double),
+        ("L_latent", C.c_double), ("Cp", C.c_double), ("T_sat", C.c_double), ("theta_I", C.c_double),
+        ("A", C.c_double), ("eps_n", C.c_double),
+        ("flags", C.c_uint),
+    ]
+
+
+class LBMError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree C-ABI library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise LBMError("%s is missing: run `python -m paper_2003_06342_b200.build` (there is no CPU fallback)" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        L.lbm_workspace_bytes.restype = C.c_size_t
+        L.lbm_workspace_bytes.argtypes = [C.POINTER(lbm_params)]
+        L.lbm_create.argtypes = [C.POINTER(lbm_params), C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]
+        L.lbm_init.argtypes = [C.c_void_p] + [C.c_void_p] * 4
+        L.lbm_step.argtypes = [C.c_void_p, C.c_int]
+        L.lbm_read_macro.argtypes = [C.c_void_p] + [C.c_void_p] * 4
+        L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.lbm_sync.argtypes = [C.c_void_p]
+        L.lbm_set_timing.argtypes = [C.c_void_p, C.c_int]
+        L.lbm_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.lbm_step_count.restype = C.c_longlong
+        L.lbm_step_count.argtypes = [C.c_void_p]
+        L.lbm_launch_count.restype = C.c_longlong
+        L.lbm_launch_count.argtypes = [C.c_void_p]
+        L.lbm_variant.restype = C.c_char_p
+        L.lbm_variant.argtypes = [C.c_void_p]
+        L.lbm_last_cuda_error.restype = C.c_int
+        L.lbm_strerror.restype = C.c_char_p
+        L.lbm_strerror.argtypes = [C.c_int]
+        L.lbm_destroy.argtypes = [C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def make_params(P: dict, precision: int = 64) -> lbm_params:
+    s = lbm_params()
+    s.nx, s.ny, s.nz = int(P["nx"]), int(P["ny"]), int(P.get("nz", 1))
+    s.lat_f, s.lat_g, s.lat_s = (LATTICES[P[k]] for k in ("lat_f", "lat_g", "lat_s"))
+    s.precision = int(precision)
+    for a in range(3):
+        for side in range(2):
+            s.bc_f[a][side] = F_KINDS[P["bc_f"][a][side]]
+            s.bc_g[a][side] = S_KINDS[P["bc_g"][a][side]]
+            s.bc_s[a][side] = S_KINDS[P["bc_s"][a][side]]
+            s.bc_phi[a][side] = float(P["bc_phi"][a][side])
+            s.bc_T[a][side] = float(P["bc_T"][a][side])
+            s.bc_p[a][side] = float(P["bc_p"][a][side])
+        s.grav[a] = float(P["grav"][a])
+    for k in ("dx", "dt", "rho_l", "rho_g", "nu_l", "nu_g", "sigma", "W", "M", "alpha_l", "alpha_g",
+              "L_latent", "Cp", "T_sat", "theta_I", "A", "eps_n"):
+        setattr(s, k, float(P[k]))
+    s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0)
+    return s
+
+
+def lbm_strerror(code: int) -> str:
+    return load_library().lbm_strerror(int(code)).decode()
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        L = load_library()
+        raise LBMError("%s failed: %s (code %d, cuda error %d)" % (what, lbm_strerror(rc), rc, L.lbm_last_cuda_error()))
+
+
+def lbm_workspace_bytes(P: dict, precision: int = 64) -> int:
+    s = make_params(P, precision)
+    return int(load_library().lbm_workspace_bytes(C.byref(s)))
+
+
+def _host_ptr(a, dtype, shape, name):
+    """Pointer to a host array: numpy array or CPU torch tensor (pinned or not), contiguous, right dtype/shape."""
+    if a is None:
+        return None, None
+    if isinstance(a, np.ndarray):
+        b = np.ascontiguousarray(a, dtype=dtype)
+        if tuple(b.shape) != tuple(shape):
+            raise ValueError("%s: shape %s, expected %s" % (name, b.shape, shape))
+        return b.ctypes.data, b
+    import torch
+    if isinstance(a, torch.Tensor):
+        if a.device.type != "cpu" or not a.is_contiguous() or tuple(a.shape) != tuple(shape):
+            raise ValueError("%s: need a contiguous CPU tensor of shape %s" % (name, shape))
+        want = torch.float64 if dtype == np.float64 else torch.float32
+        if a.dtype != want:
+            raise ValueError("%s: dtype %s, expected %s" % (name, a.dtype, want))
+        return a.data_ptr(), a
+    raise TypeError("%s: numpy array or CPU torch tensor expected" % name)
+
+
+class LBM:
+    """One simulation context on the current CUDA device and stream."""
+
+    def __init__(self, P: dict, precision: int = 64, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise LBMError("no CUDA device: the library has no CPU path")
+        self._L = load_library()
+        self.P = dict(P)
+        self.precision = int(precision)
+        self.dtype = np.float64 if precision == 64 else np.float32
+        self.shape = (int(P.get("nz", 1)), int(P["ny"]), int(P["nx"]))
+        self.N = self.shape[0] * self.shape[1] * self.shape[2]
+        self.Q = tuple(LATTICE_Q[P[k]] for k in ("lat_f", "lat_g", "lat_s"))
+        self._params = make_params(P, precision)
+        nbytes = int(self._L.lbm_workspace_bytes(C.byref(self._params)))
+        if nbytes == 0:
+            raise LBMError("lbm_workspace_bytes rejected the parameters")
+        self.workspace_bytes = nbytes
+        # device memory is allocated by torch and lent to the library (torch allocations are 512-byte aligned)
+        self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        self._stream = stream if stream is not None else torch.cuda.current_stream()
+        h = C.c_void_p()
+        _check(self._L.lbm_create(C.byref(self._params), C.c_void_p(self._ws.data_ptr()), nbytes,
+                                  C.c_void_p(self._stream.cuda_stream), C.byref(h)), "lbm_create")
+        self._h = h
+
+    # -- the calls of include/lbm.h --------------------------------------------------------------------------
+    def init(self, phi, T=None, u=None, p=None):
+        keep = []
+        ptrs = []
+        for a, shape, name in ((phi, self.shape, "phi"), (T, self.shape, "T"), (u, (3,) + self.shape, "u"),
+                               (p, self.shape, "p")):
+            ptr, k = _host_ptr(a, self.dtype, shape, name)
+            ptrs.append(C.c_void_p(ptr) if ptr is not None else None)
+            keep.append(k)
+        _check(self._L.lbm_init(self._h, *ptrs), "lbm_init")
+
+    def step(self, n: int = 1):
+        _check(self._L.lbm_step(self._h, int(n)), "lbm_step")
+
+    def read_macro(self, out=None):
+        """Returns (phi, u, p, T) as numpy arrays; ``out`` may give preallocated host arrays/tensors (pinned)."""
+        if out is None:
+            out = (np.empty(self.shape, self.dtype), np.empty((3,) + self.shape, self.dtype),
+                   np.empty(self.shape, self.dtype), np.empty(self.shape, self.dtype))
+        shapes = (self.shape, (3,) + self.shape, self.shape, self.shape)
+        ptrs = []
+        for a, shape, name in zip(out, shapes, ("phi", "u", "p", "T")):
+            ptr, _ = _host_ptr(a, self.dtype, shape, name)
+            ptrs.append(C.c_void_p(ptr) if ptr is not None else None)
+        _check(self._L.lbm_read_macro(self._h, *ptrs), "lbm_read_macro")
+        return out
+
+    def read_pops(self, which: int, stage: int = STAGE_STREAMED):
+        out = np.empty((self.Q[which],) + self.shape, self.dtype)
+        _check(self._L.lbm_read_pops(self._h, int(which), int(stage), C.c_void_p(out.ctypes.data)), "lbm_read_pops")
+        return out
+
+    def sync(self):
+        _check(self._L.lbm_sync(self._h), "lbm_sync")
+
+    def set_timing(self, enable: bool):
+        _check(self._L.lbm_set_timing(self._h, 1 if enable else 0), "lbm_set_timing")
+
+    def kernel_times(self):
+        """(ms in K_phi, ms in K_main, timed steps) since the last call; synchronises."""
+        a, b, n = C.c_double(), C.c_double(), C.c_longlong()
+        _check(self._L.lbm_kernel_times(self._h, C.byref(a), C.byref(b), C.byref(n)), "lbm_kernel_times")
+        return a.value, b.value, int(n.value)
+
+    @property
+    def step_count(self) -> int:
+        return int(self._L.lbm_step_count(self._h))
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._L.lbm_launch_count(self._h))
+
+    @property
+    def variant(self) -> str:
+        return self._L.lbm_variant(self._h).decode()
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._L.lbm_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -1,0 +1,116 @@
+// K_phi (step H1): phi^{n+1} = sum_i g_i + dt/2 sum_i P_i^g  (Eq.32) from the pulled, boundary-treated
+// g populations, written into the padded phi array together with its ghost images so that K_main's stencils
+// (and its TMA halo boxes) never leave the array.
+#pragma once
+
+#include "kernels.cuh"
+
+namespace lbm {
+
+// Store phi of node g into the padded array and into every ghost image of that node (reading S8-iv):
+// periodic axis -> image one period away; zero-flux face -> mirror phi(-1) = phi(0); Dirichlet face with value v ->
+// phi(-1) = 2 v - phi(0).  Transforms compose in axis order x, y, z (what an axis-by-axis ghost fill would give).
+template <class real>
+__device__ __forceinline__ void store_phi_with_images(real *__restrict__ phi_pad, const DevParams<real> &P,
+                                                      const NodeGeom &g, real v) {
+    const long long pc = ((long long)(g.z + P.pz) * P.ppy + (g.y + 1)) * P.ppx + (g.x + 1);
+    phi_pad[pc] = v;
+    const bool edge = g.lo[0] | g.hi[0] | g.lo[1] | g.hi[1] | (P.pz && (g.lo[2] | g.hi[2]));
+    if (!edge) return;
+    int cnt[3];
+    long long off[3][3];
+    int kind[3][3];
+    real bval[3][3];
+    const long long stride[3] = {1, P.ppx, P.pplane};
+    const int len[3] = {P.nx, P.ny, P.nz};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        cnt[a] = 1; off[a][0] = 0; kind[a][0] = BC_PERIODIC; bval[a][0] = real(0);
+        if (a == 2 && !P.pz) continue;
+        if (g.lo[a]) {
+            const int k = cnt[a]++;
+            if (P.bc_g[a][0] == BC_PERIODIC) { off[a][k] = (long long)len[a] * stride[a]; kind[a][k] = BC_PERIODIC; bval[a][k] = real(0); }
+            else { off[a][k] = -stride[a]; kind[a][k] = P.bc_g[a][0]; bval[a][k] = P.bc_phi[a][0]; }
+        }
+        if (g.hi[a]) {
+            const int k = cnt[a]++;
+            if (P.bc_g[a][1] == BC_PERIODIC) { off[a][k] = -(long long)len[a] * stride[a]; kind[a][k] = BC_PERIODIC; bval[a][k] = real(0); }
+            else { off[a][k] = stride[a]; kind[a][k] = P.bc_g[a][1]; bval[a][k] = P.bc_phi[a][1]; }
+        }
+    }
+    for (int i2 = 0; i2 < cnt[2]; ++i2)
+        for (int i1 = 0; i1 < cnt[1]; ++i1)
+            for (int i0 = 0; i0 < cnt[0]; ++i0) {
+                if ((i0 | i1 | i2) == 0) continue;
+                real w = v;
+                if (kind[0][i0] == BC_ANTI) w = real(2) * bval[0][i0] - w;
+                if (kind[1][i1] == BC_ANTI) w = real(2) * bval[1][i1] - w;
+                if (kind[2][i2] == BC_ANTI) w = real(2) * bval[2][i2] - w;
+                phi_pad[pc + off[0][i0] + off[1][i1] + off[2][i2]] = w;
+            }
+}
+
+template <class LG, class real, int BX, int BY, int BZ>
+__global__ void __launch_bounds__(BX *BY *BZ)
+k_phi(const DevParams<real> P, const real *__restrict__ g_in, const real *__restrict__ pdot, real *__restrict__ phi_new) {
+    const int t = threadIdx.x;
+    const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY, z0 = blockIdx.z * BZ;
+    const int x = x0 + t % BX, y = y0 + (t / BX) % BY, z = z0 + t / (BX * BY);
+    if (x >= P.nx || y >= P.ny || z >= P.nz) return;
+    const NodeGeom g = make_geom(P, x, y, z);
+    real gi[LG::Q];
+    if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) pull<LG, real, true>(g_in, P.N, g, P.bc_g, P.bc_phi, gi);
+    else pull<LG, real, false>(g_in, P.N, g, P.bc_g, P.bc_phi, gi);
+    real sum = gi[0];
+#pragma unroll
+    for (int i = 1; i < LG::Q; ++i) sum += gi[i];
+    const real phi = sum + P.hdt * __ldg(pdot + g.n);   // sum_i w_i = 1
+    store_phi_with_images(phi_new, P, g, phi);
+}
+
+// Initialisation helper: copy a plain [z][y][x] phi into both padded buffers with ghost images.
+template <class real, int BX, int BY, int BZ>
+__global__ void __launch_bounds__(BX *BY *BZ)
+k_phi_fill(const DevParams<real> P, const real *__restrict__ phi_plain, real *__restrict__ pad_a, real *__restrict__ pad_b) {
+    const int t = threadIdx.x;
+    const int x = blockIdx.x * BX + t % BX, y = blockIdx.y * BY + (t / BX) % BY, z = blockIdx.z * BZ + t / (BX * BY);
+    if (x >= P.nx || y >= P.ny || z >= P.nz) return;
+    const NodeGeom g = make_geom(P, x, y, z);
+    const real v = phi_plain[g.n];
+    store_phi_with_images(pad_a, P, g, v);
+    store_phi_with_images(pad_b, P, g, v);
+}
+
+// Debug / parity: streamed (post-pull, post-BC) populations of one lattice, all directions, to a [Q][N] scratch.
+template <class L, class real, int BX, int BY, int BZ>
+__global__ void __launch_bounds__(BX *BY *BZ)
+k_stream_only(const DevParams<real> P, const real *__restrict__ src, real *__restrict__ dst, int which) {
+    const int t = threadIdx.x;
+    const int x = blockIdx.x * BX + t % BX, y = blockIdx.y * BY + (t / BX) % BY, z = blockIdx.z * BZ + t / (BX * BY);
+    if (x >= P.nx || y >= P.ny || z >= P.nz) return;
+    const NodeGeom g = make_geom(P, x, y, z);
+    real v[L::Q];
+    if (which == 0) pull<L, real, true>(src, P.N, g, P.bc_f, P.bc_p, v);
+    else if (which == 1) pull<L, real, true>(src, P.N, g, P.bc_g, P.bc_phi, v);
+    else pull<L, real, true>(src, P.N, g, P.bc_s, P.bc_T, v);
+#pragma unroll
+    for (int i = 0; i < L::Q; ++i) dst[(size_t)i * P.N + g.n] = v[i];
+}
+
+template <class real> __global__ void k_fill(real *__restrict__ dst, long long n, real v) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = v;
+}
+
+// unpadded copy of phi (for lbm_read_macro)
+template <class real, int BX, int BY, int BZ>
+__global__ void __launch_bounds__(BX *BY *BZ)
+k_phi_unpad(const DevParams<real> P, const real *__restrict__ pad, real *__restrict__ plain) {
+    const int t = threadIdx.x;
+    const int x = blockIdx.x * BX + t % BX, y = blockIdx.y * BY + (t / BX) % BY, z = blockIdx.z * BZ + t / (BX * BY);
+    if (x >= P.nx || y >= P.ny || z >= P.nz) return;
+    plain[(long long)z * P.nx * P.ny + (long long)y * P.nx + x] =
+        pad[((long long)(z + P.pz) * P.ppy + (y + 1)) * P.ppx + (x + 1)];
+}
+
+}  // namespace lbm

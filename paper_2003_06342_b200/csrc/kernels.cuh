@@ -1,0 +1,152 @@
+// Device code of the coupled phase-field LBM step (sm_100a).  Shares nothing with oracle/.
+//
+// Data layout in HBM:
+//   populations  SoA [Q][z][y][x], two buffers per lattice (pull scheme, read A / write B, swap);
+//   phi          padded [nz+2][ny+2][ppx] (2D: [ny+2][ppx]) with materialised ghost layers (periodic image,
+//                zero-flux mirror, Dirichlet 2v - mirror), two buffers (level n and n+1);
+//   Pdot, u, p, T  [z][y][x].
+// Kernels:
+//   k_phi   H1: pull g (+BC), phi^{n+1} = sum g + dt/2 Pdot (Eq.32), ghost images.
+//   k_main  H2..H7: stencils (Eq.35,36), closures, pull f,s,g (+BC), moments (Eq.28a,b, 34), production
+//           refresh (Eq.18), BGK collision of the three lattices (Eq.25), store post-collision populations.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <type_traits>
+#include <utility>
+
+#include "lattices.cuh"
+
+namespace lbm {
+
+enum { BC_PERIODIC = 0, BC_BOUNCE = 1 /* wall / zero-flux */, BC_ANTI = 2 /* open / Dirichlet */ };
+enum { MODE_STEP = 0, MODE_STEP_MACRO = 1, MODE_INIT = 2 };
+
+// ---- compile-time loop over directions ---------------------------------------------------------------
+template <class F, int... I>
+__device__ __forceinline__ void static_for_impl(F &&f, std::integer_sequence<int, I...>) {
+    (f(std::integral_constant<int, I>{}), ...);
+}
+template <int N, class F> __device__ __forceinline__ void static_for(F &&f) {
+    static_for_impl(f, std::make_integer_sequence<int, N>{});
+}
+
+// e_i . v with e_i in {-1,0,1}^3 folded at compile time (no multiplications, no 0*x terms)
+template <class L, int I, class real> __device__ __forceinline__ real dot_e(real v0, real v1, real v2) {
+    real r = real(0);
+    bool first = true;
+    if constexpr (L::ex(I) != 0) { r = (L::ex(I) > 0) ? v0 : -v0; first = false; }
+    if constexpr (L::ey(I) != 0) { r = first ? ((L::ey(I) > 0) ? v1 : -v1) : ((L::ey(I) > 0) ? r + v1 : r - v1); first = false; }
+    if constexpr (L::ez(I) != 0) { r = first ? ((L::ez(I) > 0) ? v2 : -v2) : ((L::ez(I) > 0) ? r + v2 : r - v2); first = false; }
+    (void)first;
+    return r;
+}
+
+// ---- kernel parameters (passed by value) ------------------------------------------------------------------
+template <class real> struct DevParams {
+    int nx, ny, nz;
+    long long N;           // nx*ny*nz
+    int ppx, ppy, pz;      // padded phi: row pitch, ny+2, z offset (1 in 3D, 0 in 2D)
+    long long pplane;      // ppx*ppy
+    int bc_f[3][2], bc_g[3][2], bc_s[3][2];   // BC_* per face (f: wall->BOUNCE, open->ANTI)
+    real bc_phi[3][2], bc_T[3][2], bc_p[3][2];
+    int nonper[3];         // axis has non-periodic faces
+    real dt, hdt, c, inv_dx, inv_dx2;
+    real cs2f, cs2g, cs2s;           // e2 * c^2 per lattice
+    real rho_l, rho_g, rho_diff, drho;   // rho_g - rho_l ; 1/rho_g - 1/rho_l
+    real nu_l, nu_g, nu_prod;            // nu_l * nu_g
+    real fourH, K;                       // Eq.(14),(15b)
+    real grav[3];
+    real alpha_l, alpha_diff;            // alpha_g - alpha_l
+    real M, om_g, cac;                   // mobility, 1/(M/(cs2g dt)+1/2), M*(4/W)/cs2g * c
+    real LCp, CpL, T_sat, theta_I, pc_coef;   // L/Cp, Cp/L, 4/(A W^2)
+    real eps_n2;
+    int phase_change, latent_heat;
+};
+
+template <class real> struct DevFields {
+    const real *f_in, *g_in, *s_in;   // post-collision populations of the previous level
+    real *f_out, *g_out, *s_out;      // post-collision populations of this level
+    const real *phi_new;              // padded, level n+1 (written by k_phi)
+    const real *phi_old;              // padded, level n
+    real *pdot;                       // production field: read (stored, level n), then overwritten (level n+1)
+    real *u, *p, *T;                  // macro arrays: outputs (MODE_STEP_MACRO) or inputs (MODE_INIT)
+};
+
+// ---- per-node geometry ------------------------------------------------------------------------------------
+struct NodeGeom {
+    int x, y, z;
+    long long n;          // own linear index
+    int sx[3];            // source x for e_x = -1, 0, +1  (x - e_x, wrapped)
+    long long sy[3];      // source row offset (y - e_y wrapped) * nx
+    long long sz[3];      // source plane offset (z - e_z wrapped) * nx*ny
+    bool lo[3], hi[3];    // node sits on the first / last layer of the axis
+};
+
+template <class real>
+__device__ __forceinline__ NodeGeom make_geom(const DevParams<real> &P, int x, int y, int z) {
+    NodeGeom g;
+    g.x = x; g.y = y; g.z = z;
+    const long long row = P.nx, plane = (long long)P.nx * P.ny;
+    g.n = (long long)z * plane + (long long)y * row + x;
+    g.lo[0] = x == 0; g.hi[0] = x == P.nx - 1;
+    g.lo[1] = y == 0; g.hi[1] = y == P.ny - 1;
+    g.lo[2] = z == 0; g.hi[2] = z == P.nz - 1;
+    g.sx[0] = g.hi[0] ? 0 : x + 1;  g.sx[1] = x;  g.sx[2] = g.lo[0] ? P.nx - 1 : x - 1;
+    g.sy[0] = (long long)(g.hi[1] ? 0 : y + 1) * row;  g.sy[1] = (long long)y * row;
+    g.sy[2] = (long long)(g.lo[1] ? P.ny - 1 : y - 1) * row;
+    g.sz[0] = (long long)(g.hi[2] ? 0 : z + 1) * plane;  g.sz[1] = (long long)z * plane;
+    g.sz[2] = (long long)(g.lo[2] ? P.nz - 1 : z - 1) * plane;
+    return g;
+}
+
+// Pull-stream all Q directions of one lattice into registers (theta* = theta(x + c_i dt, t + dt)).
+// BC = false: every axis the node touches is periodic -> pure wrapped gather.
+// BC = true : a link that leaves through a non-periodic face takes the post-collision opposite population of the
+//             same node: bounce-back or anti-bounce-back -v + 2 w_i value;
+//             tangential wrap first, lowest axis decides (reading S8).
+template <class L, class real, bool BC>
+__device__ __forceinline__ void pull(const real *__restrict__ src, long long N, const NodeGeom &g,
+                                     const int (&bc)[3][2], const real (&val)[3][2], real (&out)[L::Q]) {
+    static_for<L::Q>([&](auto ic) {
+        constexpr int I = decltype(ic)::value;
+        constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I);
+        const long long ns = g.sz[ez + 1] + g.sy[ey + 1] + g.sx[ex + 1];
+        if constexpr (!BC || I == 0) {
+            out[I] = __ldg(src + (size_t)I * N + ns);
+        } else {
+            int kind = BC_PERIODIC;
+            real v = real(0);
+            if constexpr (ex != 0) {
+                constexpr int side = ex > 0 ? 0 : 1;
+                if ((side == 0 ? g.lo[0] : g.hi[0]) && bc[0][side] != BC_PERIODIC) { kind = bc[0][side]; v = val[0][side]; }
+            }
+            if constexpr (ey != 0) {
+                constexpr int side = ey > 0 ? 0 : 1;
+                if (kind == BC_PERIODIC && (side == 0 ? g.lo[1] : g.hi[1]) && bc[1][side] != BC_PERIODIC) { kind = bc[1][side]; v = val[1][side]; }
+            }
+            if constexpr (ez != 0) {
+                constexpr int side = ez > 0 ? 0 : 1;
+                if (kind == BC_PERIODIC && (side == 0 ? g.lo[2] : g.hi[2]) && bc[2][side] != BC_PERIODIC) { kind = bc[2][side]; v = val[2][side]; }
+            }
+            if (kind == BC_PERIODIC) {
+                out[I] = __ldg(src + (size_t)I * N + ns);
+            } else {
+                const real back = __ldg(src + (size_t)L::opp(I) * N + g.n);
+                out[I] = kind == BC_BOUNCE ? back : real(2.0 * L::w(I)) * v - back;
+            }
+        }
+    });
+}
+
+// does the tile [x0,x0+bx) x [y0,y0+by) x [z0,z0+bz) touch a non-periodic face?  (block-uniform)
+template <class real>
+__device__ __forceinline__ bool tile_touches_bc(const DevParams<real> &P, int x0, int y0, int z0, int bx, int by, int bz) {
+    bool t = false;
+    if (P.nonper[0]) t |= (x0 == 0) || (x0 + bx >= P.nx);
+    if (P.nonper[1]) t |= (y0 == 0) || (y0 + by >= P.ny);
+    if (P.nonper[2]) t |= (z0 == 0) || (z0 + bz >= P.nz);
+    return t;
+}
+
+}  // namespace lbm

@@ -1,0 +1,443 @@
+// Host side of the C ABI declared in include/lbm.h: parameter validation, workspace carving, launch loop.
+// No torch types, no CPU fallback: every step of the path runs in the kernels of k_phi.cuh / k_main.cuh.
+#include "../../include/lbm.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "k_main.cuh"
+#include "k_phi.cuh"
+
+namespace {
+
+using namespace lbm;
+
+int g_last_cuda_error = 0;
+
+#define CK(call)                                                     \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) { g_last_cuda_error = (int)e_; return LBM_E_CUDA; } \
+    } while (0)
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+int lattice_q(int id) {
+    switch (id) { case LBM_D2Q5: return 5; case LBM_D2Q9: return 9; case LBM_D3Q7: return 7; case LBM_D3Q19: return 19; }
+    return 0;
+}
+bool lattice_3d(int id) { return id == LBM_D3Q7 || id == LBM_D3Q19; }
+
+enum LatSet { SET_NONE = 0, SET_2D_995, SET_2D_999, SET_3D_1977 };
+
+LatSet lattice_set(const lbm_params *p) {
+    if (p->lat_f == LBM_D2Q9 && p->lat_g == LBM_D2Q9 && p->lat_s == LBM_D2Q5) return SET_2D_995;
+    if (p->lat_f == LBM_D2Q9 && p->lat_g == LBM_D2Q9 && p->lat_s == LBM_D2Q9) return SET_2D_999;
+    if (p->lat_f == LBM_D3Q19 && p->lat_g == LBM_D3Q7 && p->lat_s == LBM_D3Q7) return SET_3D_1977;
+    return SET_NONE;
+}
+
+// tile of nodes per thread block (one node per thread)
+template <int D> struct Tile;
+template <> struct Tile<2> { static constexpr int BX = 32, BY = 8, BZ = 1; };
+template <> struct Tile<3> { static constexpr int BX = 32, BY = 4, BZ = 2; };
+
+struct Layout {
+    long long N;
+    int ppx, ppy, ppz, pz;
+    size_t phi_pad_elems;
+    size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot, off_u, off_p, off_T, off_scratch, total;
+};
+
+int validate(const lbm_params *p) {
+    if (!p) return LBM_E_INVALID;
+    if (p->nx < 2 || p->ny < 2 || p->nz < 1) return LBM_E_INVALID;
+    if (p->precision != 64 && p->precision != 32) return LBM_E_INVALID;
+    if (!lattice_q(p->lat_f) || !lattice_q(p->lat_g) || !lattice_q(p->lat_s)) return LBM_E_INVALID;
+    const bool three_d = p->nz > 1;
+    if (lattice_3d(p->lat_f) != three_d || lattice_3d(p->lat_g) != three_d || lattice_3d(p->lat_s) != three_d)
+        return LBM_E_INVALID;
+    if (lattice_set(p) == SET_NONE) return LBM_E_UNSUPPORTED;
+    if ((double)p->nx * p->ny * p->nz > 2147483647.0) return LBM_E_INVALID;
+    if (!(p->dx > 0) || !(p->dt > 0) || !(p->W > 0) || !(p->rho_l > 0) || !(p->rho_g > 0)) return LBM_E_INVALID;
+    if (!(p->nu_l > 0) || !(p->nu_g > 0) || !(p->M > 0) || !(p->alpha_l > 0) || !(p->alpha_g > 0)) return LBM_E_INVALID;
+    if (!(p->Cp > 0) || p->L_latent == 0.0 || !(p->A > 0) || !(p->eps_n >= 0) || !(p->sigma >= 0)) return LBM_E_INVALID;
+    for (int a = 0; a < 3; ++a) {
+        for (int s = 0; s < 2; ++s) {
+            if (p->bc_f[a][s] < 0 || p->bc_f[a][s] > 2 || p->bc_g[a][s] < 0 || p->bc_g[a][s] > 2 ||
+                p->bc_s[a][s] < 0 || p->bc_s[a][s] > 2) return LBM_E_INVALID;
+        }
+        const bool per = p->bc_f[a][0] == LBM_F_PERIODIC;
+        if ((p->bc_f[a][1] == LBM_F_PERIODIC) != per || (p->bc_g[a][0] == LBM_S_PERIODIC) != per ||
+            (p->bc_g[a][1] == LBM_S_PERIODIC) != per || (p->bc_s[a][0] == LBM_S_PERIODIC) != per ||
+            (p->bc_s[a][1] == LBM_S_PERIODIC) != per) return LBM_E_INVALID;
+    }
+    return LBM_OK;
+}
+
+Layout make_layout(const lbm_params *p) {
+    Layout L{};
+    const size_t es = p->precision == 64 ? 8 : 4;
+    L.N = (long long)p->nx * p->ny * p->nz;
+    const int mult = (int)(16 / es);                          // TMA: row pitch must be a multiple of 16 bytes
+    L.ppx = (p->nx + 2 + mult - 1) / mult * mult;
+    L.ppy = p->ny + 2;
+    L.pz = p->nz > 1 ? 1 : 0;
+    L.ppz = p->nz + 2 * L.pz;
+    L.phi_pad_elems = (size_t)L.ppx * L.ppy * L.ppz;
+    const size_t N = (size_t)L.N;
+    size_t o = 0;
+    auto take = [&](size_t elems) { size_t r = o; o = align_up(o + elems * es); return r; };
+    for (int b = 0; b < 2; ++b) L.off_f[b] = take(N * lattice_q(p->lat_f));
+    for (int b = 0; b < 2; ++b) L.off_g[b] = take(N * lattice_q(p->lat_g));
+    for (int b = 0; b < 2; ++b) L.off_s[b] = take(N * lattice_q(p->lat_s));
+    for (int b = 0; b < 2; ++b) L.off_phi[b] = take(L.phi_pad_elems);
+    L.off_pdot = take(N);
+    L.off_u = take(3 * N);
+    L.off_p = take(N);
+    L.off_T = take(N);
+    L.off_scratch = take(N);
+    L.total = o;
+    return L;
+}
+
+template <class real> DevParams<real> make_dev_params(const lbm_params *p, const Layout &L) {
+    DevParams<real> d{};
+    d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.N = L.N;
+    d.ppx = L.ppx; d.ppy = L.ppy; d.pz = L.pz; d.pplane = (long long)L.ppx * L.ppy;
+    for (int a = 0; a < 3; ++a) {
+        for (int s = 0; s < 2; ++s) {
+            d.bc_f[a][s] = p->bc_f[a][s];   // PERIODIC 0, WALL -> BOUNCE 1, OPEN -> ANTI 2 (same numbering)
+            d.bc_g[a][s] = p->bc_g[a][s];
+            d.bc_s[a][s] = p->bc_s[a][s];
+            d.bc_phi[a][s] = (real)p->bc_phi[a][s];
+            d.bc_T[a][s] = (real)p->bc_T[a][s];
+            d.bc_p[a][s] = (real)p->bc_p[a][s];
+        }
+        d.nonper[a] = p->bc_f[a][0] != LBM_F_PERIODIC;
+        d.grav[a] = (real)p->grav[a];
+    }
+    if (p->nz == 1) d.nonper[2] = 0;
+    const double c = p->dx / p->dt;
+    auto e2 = [](int id) { return id == LBM_D3Q7 ? 0.25 : 1.0 / 3.0; };
+    const double cs2f = e2(p->lat_f) * c * c, cs2g = e2(p->lat_g) * c * c, cs2s = e2(p->lat_s) * c * c;
+    d.dt = (real)p->dt; d.hdt = (real)(0.5 * p->dt); d.c = (real)c;
+    d.inv_dx = (real)(1.0 / p->dx); d.inv_dx2 = (real)(1.0 / (p->dx * p->dx));
+    d.cs2f = (real)cs2f; d.cs2g = (real)cs2g; d.cs2s = (real)cs2s;
+    d.rho_l = (real)p->rho_l; d.rho_g = (real)p->rho_g; d.rho_diff = (real)(p->rho_g - p->rho_l);
+    d.drho = (real)(1.0 / p->rho_g - 1.0 / p->rho_l);
+    d.nu_l = (real)p->nu_l; d.nu_g = (real)p->nu_g; d.nu_prod = (real)(p->nu_l * p->nu_g);
+    d.fourH = (real)(4.0 * 12.0 * p->sigma / p->W);            // H = 12 sigma / W, Eq.(15b)
+    d.K = (real)(1.5 * p->W * p->sigma);                       // K = 3/2 W sigma, Eq.(15b)
+    d.alpha_l = (real)p->alpha_l; d.alpha_diff = (real)(p->alpha_g - p->alpha_l);
+    d.M = (real)p->M;
+    d.om_g = (real)(1.0 / (p->M / (cs2g * p->dt) + 0.5));      // PAPER.md:236, Eq.(25)
+    d.cac = (real)(p->M * (4.0 / p->W) * c / cs2g);            // Eq.(31b) counter term factor
+    d.LCp = (real)(p->L_latent / p->Cp); d.CpL = (real)(p->Cp / p->L_latent);
+    d.T_sat = (real)p->T_sat; d.theta_I = (real)p->theta_I;
+    d.pc_coef = (real)(4.0 / (p->A * p->W * p->W));            // Eq.(18)
+    d.eps_n2 = (real)(p->eps_n * p->eps_n);
+    d.phase_change = (p->flags & LBM_FLAG_PHASE_CHANGE) ? 1 : 0;
+    d.latent_heat = (p->flags & LBM_FLAG_LATENT_HEAT) ? 1 : 0;
+    return d;
+}
+
+}  // namespace
+
+struct lbm_ctx {
+    lbm_params P;
+    Layout L;
+    LatSet set;
+    char *ws;
+    cudaStream_t stream;
+    int cur;       // buffer holding the post-collision populations of the current level
+    int curphi;    // padded phi buffer of the current level
+    bool inited;
+    long long nsteps, launches;
+    DevParams<double> pd;
+    DevParams<float> pf;
+    // optional per-kernel timing (lbm_set_timing): 3 events per step: before k_phi, between, after k_main
+    bool timing;
+    std::vector<cudaEvent_t> ev;
+};
+
+namespace {
+
+template <class real> const DevParams<real> &dev_params(const lbm_ctx *c);
+template <> const DevParams<double> &dev_params<double>(const lbm_ctx *c) { return c->pd; }
+template <> const DevParams<float> &dev_params<float>(const lbm_ctx *c) { return c->pf; }
+
+template <class real> real *wsp(const lbm_ctx *c, size_t off) { return reinterpret_cast<real *>(c->ws + off); }
+
+template <int D> dim3 grid_for(const lbm_params &P) {
+    using T = Tile<D>;
+    return dim3((P.nx + T::BX - 1) / T::BX, (P.ny + T::BY - 1) / T::BY, (P.nz + T::BZ - 1) / T::BZ);
+}
+
+template <class LF, class LG, class LS, class real> struct Impl {
+    static constexpr int D = LF::D;
+    using T = Tile<D>;
+    static constexpr int NT = T::BX * T::BY * T::BZ;
+
+    static DevFields<real> fields(const lbm_ctx *c, int in, int out, int phi_new, int phi_old) {
+        DevFields<real> F{};
+        F.f_in = wsp<real>(c, c->L.off_f[in]);  F.f_out = wsp<real>(c, c->L.off_f[out]);
+        F.g_in = wsp<real>(c, c->L.off_g[in]);  F.g_out = wsp<real>(c, c->L.off_g[out]);
+        F.s_in = wsp<real>(c, c->L.off_s[in]);  F.s_out = wsp<real>(c, c->L.off_s[out]);
+        F.phi_new = wsp<real>(c, c->L.off_phi[phi_new]);
+        F.phi_old = wsp<real>(c, c->L.off_phi[phi_old]);
+        F.pdot = wsp<real>(c, c->L.off_pdot);
+        F.u = wsp<real>(c, c->L.off_u); F.p = wsp<real>(c, c->L.off_p); F.T = wsp<real>(c, c->L.off_T);
+        return F;
+    }
+
+    template <int MODE> static int launch_main(lbm_ctx *c, const DevFields<real> &F) {
+        k_main_direct<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, 1>
+            <<<grid_for<D>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F);
+        c->launches++;
+        CK(cudaGetLastError());
+        return LBM_OK;
+    }
+
+    static int init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, const void *h_p) {
+        const size_t N = (size_t)c->L.N, es = sizeof(real);
+        const DevParams<real> &P = dev_params<real>(c);
+        real *scratch = wsp<real>(c, c->L.off_scratch);
+        CK(cudaMemcpyAsync(scratch, h_phi, N * es, cudaMemcpyHostToDevice, c->stream));
+        real *dT = wsp<real>(c, c->L.off_T), *du = wsp<real>(c, c->L.off_u), *dp = wsp<real>(c, c->L.off_p);
+        if (h_T) CK(cudaMemcpyAsync(dT, h_T, N * es, cudaMemcpyHostToDevice, c->stream));
+        else {
+            k_fill<real><<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(dT, (long long)N, (real)c->P.T_sat);
+            c->launches++;
+            CK(cudaGetLastError());
+        }
+        if (h_u) CK(cudaMemcpyAsync(du, h_u, 3 * N * es, cudaMemcpyHostToDevice, c->stream));
+        else CK(cudaMemsetAsync(du, 0, 3 * N * es, c->stream));
+        if (h_p) CK(cudaMemcpyAsync(dp, h_p, N * es, cudaMemcpyHostToDevice, c->stream));
+        else CK(cudaMemsetAsync(dp, 0, N * es, c->stream));
+        for (int b = 0; b < 2; ++b)
+            CK(cudaMemsetAsync(wsp<real>(c, c->L.off_phi[b]), 0, c->L.phi_pad_elems * es, c->stream));
+        k_phi_fill<real, T::BX, T::BY, T::BZ><<<grid_for<D>(c->P), NT, 0, c->stream>>>(
+            P, scratch, wsp<real>(c, c->L.off_phi[0]), wsp<real>(c, c->L.off_phi[1]));
+        c->launches++;
+        CK(cudaGetLastError());
+        c->cur = 0; c->curphi = 0;
+        DevFields<real> F = fields(c, 1, 0, 0, 0);   // INIT reads no populations; writes buffer 0
+        int rc = launch_main<MODE_INIT>(c, F);
+        if (rc) return rc;
+        CK(cudaStreamSynchronize(c->stream));
+        c->nsteps = 0;
+        c->inited = true;
+        return LBM_OK;
+    }
+
+    static int step(lbm_ctx *c, int n) {
+        const DevParams<real> &P = dev_params<real>(c);
+        for (int k = 0; k < n; ++k) {
+            const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
+            const bool timed = c->timing && c->ev.size() < 3 * 4096;
+            cudaEvent_t e3[3] = {nullptr, nullptr, nullptr};
+            if (timed) {
+                for (auto &e : e3) CK(cudaEventCreate(&e));
+                CK(cudaEventRecord(e3[0], c->stream));
+            }
+            k_phi<LG, real, T::BX, T::BY, T::BZ><<<grid_for<D>(c->P), NT, 0, c->stream>>>(
+                P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot), wsp<real>(c, c->L.off_phi[pnew]));
+            c->launches++;
+            CK(cudaGetLastError());
+            if (timed) CK(cudaEventRecord(e3[1], c->stream));
+            DevFields<real> F = fields(c, in, out, pnew, pold);
+            int rc = (k == n - 1) ? launch_main<MODE_STEP_MACRO>(c, F) : launch_main<MODE_STEP>(c, F);
+            if (rc) return rc;
+            if (timed) {
+                CK(cudaEventRecord(e3[2], c->stream));
+                for (auto e : e3) c->ev.push_back(e);
+            }
+            c->cur = out; c->curphi = pnew; c->nsteps++;
+        }
+        return LBM_OK;
+    }
+
+    static int read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T) {
+        const size_t N = (size_t)c->L.N, es = sizeof(real);
+        if (h_phi) {
+            real *scratch = wsp<real>(c, c->L.off_scratch);
+            k_phi_unpad<real, T::BX, T::BY, T::BZ><<<grid_for<D>(c->P), NT, 0, c->stream>>>(
+                dev_params<real>(c), wsp<real>(c, c->L.off_phi[c->curphi]), scratch);
+            c->launches++;
+            CK(cudaGetLastError());
+            CK(cudaMemcpyAsync(h_phi, scratch, N * es, cudaMemcpyDeviceToHost, c->stream));
+        }
+        if (h_u) CK(cudaMemcpyAsync(h_u, wsp<real>(c, c->L.off_u), 3 * N * es, cudaMemcpyDeviceToHost, c->stream));
+        if (h_p) CK(cudaMemcpyAsync(h_p, wsp<real>(c, c->L.off_p), N * es, cudaMemcpyDeviceToHost, c->stream));
+        if (h_T) CK(cudaMemcpyAsync(h_T, wsp<real>(c, c->L.off_T), N * es, cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        return LBM_OK;
+    }
+
+    template <class L> static int read_pops_one(lbm_ctx *c, int which, int stage, const size_t (&off)[2], void *h) {
+        const size_t N = (size_t)c->L.N, bytes = (size_t)L::Q * N * sizeof(real);
+        if (stage == LBM_STAGE_POSTCOLLISION) {
+            CK(cudaMemcpyAsync(h, wsp<real>(c, off[c->cur]), bytes, cudaMemcpyDeviceToHost, c->stream));
+            CK(cudaStreamSynchronize(c->stream));
+            return LBM_OK;
+        }
+        if (c->nsteps < 1) return LBM_E_STATE;
+        real *tmp = nullptr;
+        CK(cudaMalloc(&tmp, bytes));   // debug path: own temporary, not the borrowed workspace
+        k_stream_only<L, real, T::BX, T::BY, T::BZ><<<grid_for<D>(c->P), NT, 0, c->stream>>>(
+            dev_params<real>(c), wsp<real>(c, off[1 - c->cur]), tmp, which);
+        c->launches++;
+        cudaError_t e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        cudaFree(tmp);
+        CK(e);
+        return LBM_OK;
+    }
+
+    static int read_pops(lbm_ctx *c, int which, int stage, void *h) {
+        if (which == LBM_POPS_F) return read_pops_one<LF>(c, which, stage, c->L.off_f, h);
+        if (which == LBM_POPS_G) return read_pops_one<LG>(c, which, stage, c->L.off_g, h);
+        if (which == LBM_POPS_S) return read_pops_one<LS>(c, which, stage, c->L.off_s, h);
+        return LBM_E_INVALID;
+    }
+};
+
+// dispatch on (lattice set, precision)
+template <class Fn> int dispatch(const lbm_ctx *c, Fn &&fn) {
+    const bool d = c->P.precision == 64;
+    switch (c->set) {
+    case SET_2D_995: return d ? fn(Impl<D2Q9, D2Q9, D2Q5, double>{}) : fn(Impl<D2Q9, D2Q9, D2Q5, float>{});
+    case SET_2D_999: return d ? fn(Impl<D2Q9, D2Q9, D2Q9, double>{}) : fn(Impl<D2Q9, D2Q9, D2Q9, float>{});
+    case SET_3D_1977: return d ? fn(Impl<D3Q19, D3Q7, D3Q7, double>{}) : fn(Impl<D3Q19, D3Q7, D3Q7, float>{});
+    default: return LBM_E_UNSUPPORTED;
+    }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+size_t lbm_workspace_bytes(const lbm_params *p) {
+    if (validate(p) != LBM_OK) return 0;
+    return make_layout(p).total;
+}
+
+int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_stream, lbm_ctx **out) {
+    if (!out) return LBM_E_INVALID;
+    *out = nullptr;
+    int rc = validate(p);
+    if (rc) return rc;
+    Layout L = make_layout(p);
+    if (!d_workspace || bytes < L.total || (reinterpret_cast<size_t>(d_workspace) % ALIGN) != 0) return LBM_E_WORKSPACE;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        g_last_cuda_error = (int)cudaGetLastError();
+        return LBM_E_NODEVICE;
+    }
+    if (prop.major != 10) return LBM_E_NODEVICE;   // kernels are built for sm_100a only
+    cudaPointerAttributes attr;
+    CK(cudaPointerGetAttributes(&attr, d_workspace));
+    if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged) return LBM_E_WORKSPACE;
+    lbm_ctx *c = new (std::nothrow) lbm_ctx();
+    if (!c) return LBM_E_INVALID;
+    c->P = *p; c->L = L; c->set = lattice_set(p);
+    c->ws = static_cast<char *>(d_workspace);
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->cur = 0; c->curphi = 0; c->inited = false; c->nsteps = 0; c->launches = 0; c->timing = false;
+    c->pd = make_dev_params<double>(p, L);
+    c->pf = make_dev_params<float>(p, L);
+    *out = c;
+    return LBM_OK;
+}
+
+int lbm_init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, const void *h_p) {
+    if (!c || !h_phi) return LBM_E_INVALID;
+    return dispatch(c, [&](auto impl) { return decltype(impl)::init(c, h_phi, h_T, h_u, h_p); });
+}
+
+int lbm_step(lbm_ctx *c, int n) {
+    if (!c || n < 0) return LBM_E_INVALID;
+    if (!c->inited) return LBM_E_STATE;
+    return dispatch(c, [&](auto impl) { return decltype(impl)::step(c, n); });
+}
+
+int lbm_read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T) {
+    if (!c) return LBM_E_INVALID;
+    if (!c->inited) return LBM_E_STATE;
+    return dispatch(c, [&](auto impl) { return decltype(impl)::read_macro(c, h_phi, h_u, h_p, h_T); });
+}
+
+int lbm_read_pops(lbm_ctx *c, int which, int stage, void *h_pops) {
+    if (!c || !h_pops || which < 0 || which > 2 || (stage != LBM_STAGE_POSTCOLLISION && stage != LBM_STAGE_STREAMED))
+        return LBM_E_INVALID;
+    if (!c->inited) return LBM_E_STATE;
+    return dispatch(c, [&](auto impl) { return decltype(impl)::read_pops(c, which, stage, h_pops); });
+}
+
+int lbm_sync(lbm_ctx *c) {
+    if (!c) return LBM_E_INVALID;
+    CK(cudaStreamSynchronize(c->stream));
+    return LBM_OK;
+}
+
+int lbm_set_timing(lbm_ctx *c, int enable) {
+    if (!c) return LBM_E_INVALID;
+    c->timing = enable != 0;
+    return LBM_OK;
+}
+
+int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *steps) {
+    if (!c) return LBM_E_INVALID;
+    CK(cudaStreamSynchronize(c->stream));
+    double a = 0.0, b = 0.0;
+    const size_t n = c->ev.size() / 3;
+    for (size_t k = 0; k < n; ++k) {
+        float t0 = 0.f, t1 = 0.f;
+        CK(cudaEventElapsedTime(&t0, c->ev[3 * k], c->ev[3 * k + 1]));
+        CK(cudaEventElapsedTime(&t1, c->ev[3 * k + 1], c->ev[3 * k + 2]));
+        a += t0; b += t1;
+    }
+    for (auto e : c->ev) cudaEventDestroy(e);
+    c->ev.clear();
+    if (ms_phi) *ms_phi = a;
+    if (ms_main) *ms_main = b;
+    if (steps) *steps = (long long)n;
+    return LBM_OK;
+}
+
+long long lbm_step_count(const lbm_ctx *c) { return c ? c->nsteps : -1; }
+long long lbm_launch_count(const lbm_ctx *c) { return c ? c->launches : -1; }
+const char *lbm_variant(const lbm_ctx *c) { return c ? "direct" : ""; }
+int lbm_last_cuda_error(void) { return g_last_cuda_error; }
+
+const char *lbm_strerror(int code) {
+    switch (code) {
+    case LBM_OK: return "ok";
+    case LBM_E_INVALID: return "invalid argument or parameter combination";
+    case LBM_E_UNSUPPORTED: return "lattice set or precision not built";
+    case LBM_E_WORKSPACE: return "workspace too small, misaligned or not device memory";
+    case LBM_E_CUDA: return "CUDA runtime error (see lbm_last_cuda_error)";
+    case LBM_E_STATE: return "call not valid in this state";
+    case LBM_E_NODEVICE: return "no sm_100 CUDA device";
+    default: return "unknown error";
+    }
+}
+
+void lbm_destroy(lbm_ctx *c) {
+    if (!c) return;
+    for (auto e : c->ev) cudaEventDestroy(e);
+    delete c;
+}
+
+}  // extern "C"

@@ -1,0 +1,35 @@
+"""Evidence for the parity horizons: how fast the model itself amplifies a 1-ulp
+perturbation of the input, measured oracle against oracle.  Two correct implementations differ by at least this much."""
+import numpy as np
+
+from paper_2003_06342_b200 import workloads as wl
+
+
+def _ulp_perturbed(a, rng):
+    return a * (1 + 1e-16 * rng.integers(-2, 3, a.shape))
+
+
+def test_config2_amplifies_roundoff_beyond_1e10_by_step_1000(oracle_mod):
+    P, I = wl.config2_stefan()
+    rng = np.random.Generator(np.random.PCG64(1))
+    a = oracle_mod.Oracle(P); a.init(I["phi"], I["T"])
+    b = oracle_mod.Oracle(P); b.init(_ulp_perturbed(I["phi"], rng), _ulp_perturbed(I["T"], rng))
+    a.step(200); b.step(200)
+    d200 = max(float(np.abs(x - y).max()) for x, y in zip(a.read_macro(), b.read_macro()))
+    a.step(800); b.step(800)
+    d1000 = max(float(np.abs(x - y).max()) for x, y in zip(a.read_macro(), b.read_macro()))
+    assert d1000 > 1e-7, d1000           # 1e-10 at N = 1000 is not attainable by any second implementation
+    assert d1000 < 5e-3                  # ... and the difference saturates at a small amplitude
+    assert d200 < 1e-4
+    a.close(); b.close()
+
+
+def test_config1_is_well_conditioned_to_1000_steps(oracle_mod):
+    P, I = wl.config1_droplet()
+    rng = np.random.Generator(np.random.PCG64(2))
+    a = oracle_mod.Oracle(P); a.init(I["phi"], I["T"])
+    b = oracle_mod.Oracle(P); b.init(_ulp_perturbed(I["phi"], rng), I["T"])
+    a.step(1000); b.step(1000)
+    d = max(float(np.abs(x - y).max()) for x, y in zip(a.read_macro(), b.read_macro()))
+    assert d < 1e-11, d
+    a.close(); b.close()
