@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SRC_DIR = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblbm_b200.so")
 SOURCES = ["lbm.cu"]
-DEPS = ["lbm.cu", "kernels.cuh", "k_phi.cuh", "k_main.cuh", "lattices.cuh", os.path.join("..", "..", "include", "lbm.h")]
+DEPS = ["lbm.cu", "kernels.cuh", "k_phi.cuh", "k_main.cuh", "k_main_tma.cuh", "lattices.cuh", os.path.join("..", "..", "include", "lbm.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xptxas", "-v",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 

@@ -1,5 +1,7 @@
-// K_main (steps H2..H7): one thread per lattice node, everything between the pull and the post-collision store in
-// registers.  Citations are PAPER.md:<line>; readings (G*/S*) are listed in DESIGN.md.
+// K_main (steps H2..H7): one thread per lattice node.  Citations are PAPER.md:<line>; readings (G*/S*) are listed in
+// DESIGN.md.  Populations are NOT held in registers across the step: the moments are accumulated while the pulled
+// values stream in, and every population is read again (L1 hit, or shared memory in the TMA variant) at the point
+// where it is collided.  That keeps the live state at ~50 doubles and lets two 256-thread CTAs share an SM.
 #pragma once
 
 #include "kernels.cuh"
@@ -9,35 +11,49 @@ namespace lbm {
 __device__ __forceinline__ double rsqrt_(double a) { return rsqrt(a); }
 __device__ __forceinline__ float rsqrt_(float a) { return rsqrtf(a); }
 
-// phi^{n+1} neighbourhood straight from the padded global array (L1/L2 serve the 18 re-reads)
-template <class real> struct PhiGlobal {
-    const real *__restrict__ c;   // pointer to the node's own padded element
-    long long sy, sz;             // row pitch, plane pitch
-    __device__ __forceinline__ real operator()(int dx, int dy, int dz) const { return __ldg(c + dx + dy * sy + dz * sz); }
+// Source of one node's inputs, direct variant: gathers straight from global memory (pull with wrap / boundary
+// rules); the phi^{n+1} neighbourhood comes from the padded array through L1/L2.
+template <class LF, class LG, class LS, class real, bool BC> struct SrcGlobal {
+    const DevParams<real> &P;
+    const DevFields<real> &Fd;
+    const NodeGeom &g;
+    const real *__restrict__ pc;   // the node's own element of the padded phi^{n+1}
+    unsigned pcoff;
+    __device__ __forceinline__ SrcGlobal(const DevParams<real> &P_, const DevFields<real> &Fd_, const NodeGeom &g_)
+        : P(P_), Fd(Fd_), g(g_) {
+        pcoff = ((unsigned)(g.z + P.pz) * (unsigned)P.ppy + (unsigned)(g.y + 1)) * (unsigned)P.ppx + (unsigned)(g.x + P.xpad);
+        pc = Fd.phi_new + pcoff;
+    }
+    __device__ __forceinline__ real phi(int dx, int dy, int dz) const { return __ldg(pc + (dx + dy * P.ppx + dz * (int)P.pplane)); }
+    __device__ __forceinline__ real phi_old() const { return __ldg(Fd.phi_old + pcoff); }
+    __device__ __forceinline__ real pdot_old() const { return Fd.pdot[g.n]; }
+    // AGAIN = true: second read of a value already read for the moments (see ld_again)
+    template <int I, bool AGAIN = false> __device__ __forceinline__ real f() const { return pull_one<LF, I, real, BC, AGAIN>(Fd.f_in, (unsigned)P.N, g, P.bc_f, P.bc_p); }
+    template <int I, bool AGAIN = false> __device__ __forceinline__ real s() const { return pull_one<LS, I, real, BC, AGAIN>(Fd.s_in, (unsigned)P.N, g, P.bc_s, P.bc_T); }
+    template <int I, bool AGAIN = false> __device__ __forceinline__ real gg() const { return pull_one<LG, I, real, BC, AGAIN>(Fd.g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi); }
 };
 
-// phi^{n+1} neighbourhood from a shared-memory halo tile (filled by TMA)
-template <class real> struct PhiShared {
-    const real *c;                // pointer to the node's own element in the tile
-    int sy, sz;
-    __device__ __forceinline__ real operator()(int dx, int dy, int dz) const { return c[dx + dy * sy + dz * sz]; }
-};
-
-template <class LF, class LG, class LS, class real, int MODE, bool BC, class PhiAcc>
+template <class LF, class LG, class LS, class real, int MODE, class Src>
 __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevFields<real> &Fd, const NodeGeom &g,
-                                            const PhiAcc &ph) {
-    const long long n = g.n;
-    const long long N = P.N;
+                                            const Src &src) {
+    const unsigned n = g.n;
+    const unsigned N = (unsigned)P.N;
+
+    // ---- H5 (first half): zeroth moment of s.  Loaded first so that these loads are in flight during the stencil.
+    real sum_s = real(0);
+    if constexpr (MODE != MODE_INIT) {
+        static_for<LS::Q>([&](auto ic) { sum_s += src.template s<decltype(ic)::value>(); });
+    }
 
     // ---- H2: grad phi, lap phi by directional derivatives on the NS lattice (Eq.35a,b 36a,b; PAPER.md:291-315;
     //      the printed factor 3 is 1/e2, reading S2).  Opposite directions are paired: one difference, one sum.
-    const real phi = ph(0, 0, 0);
+    const real phi = src.phi(0, 0, 0);
     real gx = real(0), gy = real(0), gz = real(0), lsum = real(0);
     static_for<LF::Q>([&](auto ic) {
         constexpr int I = decltype(ic)::value;
         if constexpr (I > 0 && I < LF::opp(I)) {
             constexpr int ex = LF::ex(I), ey = LF::ey(I), ez = LF::ez(I);
-            const real pp = ph(ex, ey, ez), pm = ph(-ex, -ey, -ez);
+            const real pp = src.phi(ex, ey, ez), pm = src.phi(-ex, -ey, -ez);
             const real d = pp - pm;
             constexpr real w = real(LF::w(I));
             if constexpr (ex != 0) gx += (ex > 0 ? w : -w) * d;
@@ -61,42 +77,42 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
     const real Fz = mu * gz + bu * P.grav[2];
     const real grx = P.rho_diff * gx, gry = P.rho_diff * gy, grz = P.rho_diff * gz;   // grad rho
     const real alpha = P.alpha_l + phi * P.alpha_diff;                         // reading S6
+    // relaxation rates: tau_bar = nu/(cs2 dt) with harmonic nu (Eq.1b); alpha/(cs2 dt);
+    // om = 1/(tau_bar + 1/2) (Eq.25).  om_f = den/(nu_l nu_g/(cs2 dt) + den/2), den = phi nu_l + (1-phi) nu_g.
+    // The three per-node divisions (1/rho, om_f, om_s) share ONE reciprocal: 1/(rho * df * ds).
+    const real den = phi * P.nu_l + (real(1) - phi) * P.nu_g;
+    const real df = P.tauf_num + real(0.5) * den;
+    const real ds = alpha * P.taus_den + real(0.5);
+    const real rds = rho * ds;
+    const real rall = real(1) / (rds * df);
+    const real inv_rho = rall * ds * df;
+    const real om_f = den * (rall * rds);
+    const real om_s = rall * (rho * df);
 
     real ux, uy, uz, p, T, dtphi;
-    real f[LF::Q], s[LS::Q];
     if constexpr (MODE == MODE_INIT) {
-#pragma unroll
-        for (int i = 0; i < LF::Q; ++i) f[i] = real(0);   // unused in this mode (bar = eq - dt/2 S)
-#pragma unroll
-        for (int i = 0; i < LS::Q; ++i) s[i] = real(0);
         ux = Fd.u[n]; uy = Fd.u[N + n]; uz = (LF::D == 3) ? Fd.u[2 * N + n] : real(0);
         p = Fd.p[n]; T = Fd.T[n]; dtphi = real(0);
     } else {
-        // ---- H4: NS moments (Eq.28a)
-        pull<LF, real, BC>(Fd.f_in, N, g, P.bc_f, P.bc_p, f);
+        // ---- H4: NS moments (Eq.28a), accumulated as the pulled values arrive
         real m0 = real(0), mx = real(0), my = real(0), mz = real(0);
         static_for<LF::Q>([&](auto ic) {
             constexpr int I = decltype(ic)::value;
-            m0 += f[I];
-            if constexpr (LF::ex(I) != 0) mx += LF::ex(I) > 0 ? f[I] : -f[I];
-            if constexpr (LF::ey(I) != 0) my += LF::ey(I) > 0 ? f[I] : -f[I];
-            if constexpr (LF::ez(I) != 0) mz += LF::ez(I) > 0 ? f[I] : -f[I];
+            const real fi = src.template f<I>();
+            m0 += fi;
+            if constexpr (LF::ex(I) != 0) mx += LF::ex(I) > 0 ? fi : -fi;
+            if constexpr (LF::ey(I) != 0) my += LF::ey(I) > 0 ? fi : -fi;
+            if constexpr (LF::ez(I) != 0) mz += LF::ez(I) > 0 ? fi : -fi;
         });
-        const real inv_rho = real(1) / rho;
-        const real cm = P.c / P.cs2f;
+        const real cm = P.c_cs2f;
         ux = (cm * mx + P.hdt * Fx) * inv_rho;
         uy = (cm * my + P.hdt * Fy) * inv_rho;
         uz = (cm * mz + P.hdt * Fz) * inv_rho;
         // ---- H1 (time derivative), H5: heat moment with the STORED production rate (reading S3; Eq.34)
-        const long long pc = ((long long)(g.z + P.pz) * P.ppy + (g.y + 1)) * P.ppx + (g.x + 1);
-        const real phi_old = __ldg(Fd.phi_old + pc);
-        dtphi = (phi - phi_old) / P.dt;                                        // reading S4
-        const real mdot_old = P.rho_g * Fd.pdot[n];
+        dtphi = (phi - src.phi_old()) * P.inv_dt;                              // reading S4
+        const real mdot_old = P.rho_g * src.pdot_old();
         const real D_old = ux * gx + uy * gy + uz * gz + phi * mdot_old * P.drho;   // reading S5
-        pull<LS, real, BC>(Fd.s_in, N, g, P.bc_s, P.bc_T, s);
-        T = s[0];
-#pragma unroll
-        for (int i = 1; i < LS::Q; ++i) T += s[i];
+        T = sum_s;
         if (P.latent_heat) T -= P.hdt * P.LCp * (dtphi + D_old);
         // pressure (Eq.28b)
         p = m0 + P.hdt * (P.cs2f * (ux * grx + uy * gry + uz * grz) + rho * P.cs2f * mdot_old * P.drho);
@@ -114,121 +130,125 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
         Fd.p[n] = p; Fd.T[n] = T;
     }
 
-    // ---- H7: sources, equilibria, BGK (Eq.25): out = (1-om) bar + om eq + dt (1 - om/2) S
+    // ---- H7: sources, equilibria, BGK (Eq.25)
     const real mdot = P.rho_g * pdot;
     const real ug = ux * gx + uy * gy + uz * gz;
     const real D = ug + phi * mdot * P.drho;
     const real uu = ux * ux + uy * uy + uz * uz;
 
-    // relaxation rates: tau_bar = nu/(cs2 dt) with harmonic nu (Eq.1b); alpha/(cs2 dt)
-    const real den = phi * P.nu_l + (real(1) - phi) * P.nu_g;
-    const real om_f = den / (P.nu_prod / (P.cs2f * P.dt) + real(0.5) * den);
-    const real om_s = real(1) / (alpha / (P.cs2s * P.dt) + real(0.5));
-    const real om_g = P.om_g;
-
-    auto relax = [&](real bar, real eq, real S, real om) -> real {
-        if constexpr (MODE == MODE_INIT) return eq + P.hdt * S;   // bar = eq - dt/2 S (Eq.24), reading S9
-        else return (real(1) - om) * bar + om * eq + P.dt * (real(1) - real(0.5) * om) * S;
-    };
-
-    // -- Navier-Stokes (Eq.26b, 27a-d PAPER.md:198-220)
+    // BGK with the source shift folded in: out_i = a bar_i + om eq_i + b S_i, with (a, om, b) = (1-om, om, dt(1-om/2)),
+    // or (0, 1, dt/2) at initialisation where bar = eq - dt/2 S (Eq.24, reading S9).
+    //
+    // -- Navier-Stokes (Eq.26b, 27a-d PAPER.md:198-220).  With Gamma_i - w_i = w_i (q +- t), t = c_i.u/cs2,
+    //    q = t^2/2 - u.u/(2 cs2), A = cs2 grad rho, H = A + F_tot, mdot = mass production rate:
+    //      eq_i = w_i p + rho cs2 (Gamma_i - w_i)
+    //      S_i  = (Gamma_i - w_i)(c_i.H - u.H) + w_i (c_i.F - u.F + rho cs2 mdot Drho)
+    //    so out_i = a bar_i + (Gamma_i - w_i)(K1 + b c_i.H) + w_i (K2 + b c_i.F),
+    //    K1 = om rho cs2 - b u.H,  K2 = om p + b (rho cs2 mdot Drho - u.F).
     {
-        const real ic = P.c / P.cs2f;
+        const real om = MODE == MODE_INIT ? real(1) : om_f;
+        const real a = MODE == MODE_INIT ? real(0) : real(1) - om_f;
+        const real b = MODE == MODE_INIT ? P.hdt : P.dt * (real(1) - real(0.5) * om_f);
+        const real ic = P.c_cs2f;
         const real tx = ux * ic, ty = uy * ic, tz = uz * ic;          // c u / cs2
-        const real uu_cs = uu / P.cs2f;
-        const real Ax = P.cs2f * grx, Ay = P.cs2f * gry, Az = P.cs2f * grz;   // cs2 grad rho
-        const real uA = ux * Ax + uy * Ay + uz * Az;
-        const real uF = ux * Fx + uy * Fy + uz * Fz;
-        const real cAx = P.c * Ax, cAy = P.c * Ay, cAz = P.c * Az;
-        const real cFx = P.c * Fx, cFy = P.c * Fy, cFz = P.c * Fz;
+        const real U = real(-0.5) * uu * P.inv_cs2f;
         const real rcs = rho * P.cs2f;
-        const real Pf = rcs * mdot * P.drho;                           // Eq.(27c) without w_i
-        {   // rest direction
+        const real Hx = P.cs2f * grx + Fx, Hy = P.cs2f * gry + Fy, Hz = P.cs2f * grz + Fz;
+        const real K1 = om * rcs - b * (ux * Hx + uy * Hy + uz * Hz);
+        const real K2 = om * p + b * (rcs * mdot * P.drho - (ux * Fx + uy * Fy + uz * Fz));
+        const real bc = b * P.c;
+        const real Hbx = bc * Hx, Hby = bc * Hy, Hbz = bc * Hz;
+        const real Fbx = bc * Fx, Fby = bc * Fy, Fbz = bc * Fz;
+        {   // rest direction: t = 0
             constexpr real w = real(LF::w(0));
-            const real As = -real(0.5) * w * uu_cs;
-            const real S = As * (-uA) + (w + As) * (-uF) + w * Pf;
-            const real eq = w * p + rcs * As;
-            Fd.f_out[n] = relax(MODE == MODE_INIT ? real(0) : f[0], eq, S, om_f);
+            real bar = real(0);
+            if constexpr (MODE != MODE_INIT) bar = src.template f<0, true>();
+            Fd.f_out[n] = a * bar + w * (U * K1 + K2);
         }
         static_for<LF::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
             if constexpr (I > 0 && I < LF::opp(I)) {
                 constexpr int J = LF::opp(I);
                 constexpr real w = real(LF::w(I));
+                real bi = real(0), bj = real(0);
+                if constexpr (MODE != MODE_INIT) { bi = src.template f<I, true>(); bj = src.template f<J, true>(); }
                 const real t = dot_e<LF, I, real>(tx, ty, tz);
-                const real As = real(0.5) * w * (t * t - uu_cs);
-                const real Aa = w * t;
-                const real cA = dot_e<LF, I, real>(cAx, cAy, cAz);
-                const real cF = dot_e<LF, I, real>(cFx, cFy, cFz);
-                const real Gi = As + Aa, Gj = As - Aa;                 // Gamma - w
-                const real Si = Gi * (cA - uA) + (w + Gi) * (cF - uF) + w * Pf;
-                const real Sj = Gj * (-cA - uA) + (w + Gj) * (-cF - uF) + w * Pf;
-                const real eqi = w * p + rcs * Gi, eqj = w * p + rcs * Gj;
-                Fd.f_out[(size_t)I * N + n] = relax(MODE == MODE_INIT ? real(0) : f[I], eqi, Si, om_f);
-                Fd.f_out[(size_t)J * N + n] = relax(MODE == MODE_INIT ? real(0) : f[J], eqj, Sj, om_f);
+                const real q = real(0.5) * t * t + U;
+                const real h = dot_e<LF, I, real>(Hbx, Hby, Hbz);
+                const real fb = dot_e<LF, I, real>(Fbx, Fby, Fbz);
+                Fd.f_out[(unsigned)I * N + n] = a * bi + w * ((q + t) * (K1 + h) + (K2 + fb));
+                Fd.f_out[(unsigned)J * N + n] = a * bj + w * ((q - t) * (K1 - h) + (K2 - fb));
             }
         });
     }
-    // -- temperature (Eq.33a-d, sign of reading G2)
+    // -- temperature (Eq.33a-d, sign of reading G2): eq_i = T Gamma_i, S_i = -w_i (L/Cp)(dphi/dt + D)
     {
-        const real ic = P.c / P.cs2s;
+        const real om = MODE == MODE_INIT ? real(1) : om_s;
+        const real a = MODE == MODE_INIT ? real(0) : real(1) - om_s;
+        const real b = MODE == MODE_INIT ? P.hdt : P.dt * (real(1) - real(0.5) * om_s);
+        const real ic = P.c_cs2s;
         const real tx = ux * ic, ty = uy * ic, tz = uz * ic;
-        const real uu_cs = uu / P.cs2s;
-        const real Qs = P.latent_heat ? -P.LCp * (dtphi + D) : real(0);
+        const real U1 = real(1) - real(0.5) * uu * P.inv_cs2s;
+        const real TO = om * T;
+        const real bQ = P.latent_heat ? -b * P.LCp * (dtphi + D) : real(0);
         {
             constexpr real w = real(LS::w(0));
-            const real G0 = w - real(0.5) * w * uu_cs;
-            Fd.s_out[n] = relax(MODE == MODE_INIT ? real(0) : s[0], T * G0, w * Qs, om_s);
+            real bar = real(0);
+            if constexpr (MODE != MODE_INIT) bar = src.template s<0, true>();
+            Fd.s_out[n] = a * bar + w * (TO * U1 + bQ);
         }
         static_for<LS::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
             if constexpr (I > 0 && I < LS::opp(I)) {
                 constexpr int J = LS::opp(I);
                 constexpr real w = real(LS::w(I));
+                real bi = real(0), bj = real(0);
+                if constexpr (MODE != MODE_INIT) { bi = src.template s<I, true>(); bj = src.template s<J, true>(); }
                 const real t = dot_e<LS, I, real>(tx, ty, tz);
-                const real Gs = w + real(0.5) * w * (t * t - uu_cs);
-                const real Aa = w * t;
-                Fd.s_out[(size_t)I * N + n] = relax(MODE == MODE_INIT ? real(0) : s[I], T * (Gs + Aa), w * Qs, om_s);
-                Fd.s_out[(size_t)J * N + n] = relax(MODE == MODE_INIT ? real(0) : s[J], T * (Gs - Aa), w * Qs, om_s);
+                const real q = real(0.5) * t * t + U1;
+                Fd.s_out[(unsigned)I * N + n] = a * bi + w * (TO * (q + t) + bQ);
+                Fd.s_out[(unsigned)J * N + n] = a * bj + w * (TO * (q - t) + bQ);
             }
         });
     }
-    // -- conservative Allen-Cahn, modified-equilibrium form (Eq.31a,b PAPER.md:246-251; P_i^g Eq.30b)
+    // -- conservative Allen-Cahn, modified-equilibrium form (Eq.31a,b PAPER.md:246-251; P_i^g Eq.30b):
+    //    eq_i = phi Gamma_i + M (4/W) phi (1-phi) w_i c_i.n / cs2,  S_i = w_i Pdot
     {
-        real gi[LG::Q];
-        if constexpr (MODE != MODE_INIT) pull<LG, real, BC>(Fd.g_in, N, g, P.bc_g, P.bc_phi, gi);
-        else {
-#pragma unroll
-            for (int i = 0; i < LG::Q; ++i) gi[i] = real(0);
-        }
-        const real ic = P.c / P.cs2g;
+        const real om = MODE == MODE_INIT ? real(1) : P.om_g;
+        const real a = MODE == MODE_INIT ? real(0) : real(1) - P.om_g;
+        const real b = MODE == MODE_INIT ? P.hdt : P.dt * (real(1) - real(0.5) * P.om_g);
+        const real ic = P.c_cs2g;
         const real tx = ux * ic, ty = uy * ic, tz = uz * ic;
-        const real uu_cs = uu / P.cs2g;
+        const real U1 = real(1) - real(0.5) * uu * P.inv_cs2g;
         const real inv_norm = rsqrt_(gx * gx + gy * gy + gz * gz + P.eps_n2);     // Eq.(6), reading S7
-        const real B = P.cac * phi * (real(1) - phi) * inv_norm;                  // M (4/W) phi(1-phi) c / cs2 / |grad phi|
+        const real B = om * P.cac * phi * (real(1) - phi) * inv_norm;             // om M (4/W) phi(1-phi) c / cs2 / |grad phi|
         const real bx = B * gx, by = B * gy, bz = B * gz;
+        const real PO = om * phi;
+        const real bP = b * pdot;
         {
             constexpr real w = real(LG::w(0));
-            const real G0 = w - real(0.5) * w * uu_cs;
-            Fd.g_out[n] = relax(MODE == MODE_INIT ? real(0) : gi[0], phi * G0, w * pdot, om_g);
+            real bar = real(0);
+            if constexpr (MODE != MODE_INIT) bar = src.template gg<0>();
+            Fd.g_out[n] = a * bar + w * (PO * U1 + bP);
         }
         static_for<LG::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
             if constexpr (I > 0 && I < LG::opp(I)) {
                 constexpr int J = LG::opp(I);
                 constexpr real w = real(LG::w(I));
+                real bi = real(0), bj = real(0);
+                if constexpr (MODE != MODE_INIT) { bi = src.template gg<I>(); bj = src.template gg<J>(); }
                 const real t = dot_e<LG, I, real>(tx, ty, tz);
-                const real Gs = w + real(0.5) * w * (t * t - uu_cs);
-                const real Aa = w * t;
-                const real cn = w * dot_e<LG, I, real>(bx, by, bz);
-                Fd.g_out[(size_t)I * N + n] = relax(MODE == MODE_INIT ? real(0) : gi[I], phi * (Gs + Aa) + cn, w * pdot, om_g);
-                Fd.g_out[(size_t)J * N + n] = relax(MODE == MODE_INIT ? real(0) : gi[J], phi * (Gs - Aa) - cn, w * pdot, om_g);
+                const real q = real(0.5) * t * t + U1;
+                const real cn = dot_e<LG, I, real>(bx, by, bz);
+                Fd.g_out[(unsigned)I * N + n] = a * bi + w * (PO * (q + t) + (bP + cn));
+                Fd.g_out[(unsigned)J * N + n] = a * bj + w * (PO * (q - t) + (bP - cn));
             }
         });
     }
 }
 
-// Direct variant: phi neighbourhood read from global memory through L1.
+// Direct variant: everything gathered from global memory.
 template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB>
 __global__ void __launch_bounds__(BX *BY *BZ, MINB)
 k_main_direct(const DevParams<real> P, const DevFields<real> Fd) {
@@ -237,9 +257,13 @@ k_main_direct(const DevParams<real> P, const DevFields<real> Fd) {
     const int x = x0 + t % BX, y = y0 + (t / BX) % BY, z = z0 + t / (BX * BY);
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
     const NodeGeom g = make_geom(P, x, y, z);
-    PhiGlobal<real> ph{Fd.phi_new + ((long long)(z + P.pz) * P.ppy + (y + 1)) * P.ppx + (x + 1), (long long)P.ppx, P.pplane};
-    if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) node_update<LF, LG, LS, real, MODE, true>(P, Fd, g, ph);
-    else node_update<LF, LG, LS, real, MODE, false>(P, Fd, g, ph);
+    if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) {
+        const SrcGlobal<LF, LG, LS, real, true> src(P, Fd, g);
+        node_update<LF, LG, LS, real, MODE>(P, Fd, g, src);
+    } else {
+        const SrcGlobal<LF, LG, LS, real, false> src(P, Fd, g);
+        node_update<LF, LG, LS, real, MODE>(P, Fd, g, src);
+    }
 }
 
 }  // namespace lbm

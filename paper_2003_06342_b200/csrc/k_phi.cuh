@@ -13,7 +13,7 @@ namespace lbm {
 template <class real>
 __device__ __forceinline__ void store_phi_with_images(real *__restrict__ phi_pad, const DevParams<real> &P,
                                                       const NodeGeom &g, real v) {
-    const long long pc = ((long long)(g.z + P.pz) * P.ppy + (g.y + 1)) * P.ppx + (g.x + 1);
+    const long long pc = ((long long)(g.z + P.pz) * P.ppy + (g.y + 1)) * P.ppx + (g.x + P.xpad);
     phi_pad[pc] = v;
     const bool edge = g.lo[0] | g.hi[0] | g.lo[1] | g.hi[1] | (P.pz && (g.lo[2] | g.hi[2]));
     if (!edge) return;
@@ -59,8 +59,8 @@ k_phi(const DevParams<real> P, const real *__restrict__ g_in, const real *__rest
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
     const NodeGeom g = make_geom(P, x, y, z);
     real gi[LG::Q];
-    if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) pull<LG, real, true>(g_in, P.N, g, P.bc_g, P.bc_phi, gi);
-    else pull<LG, real, false>(g_in, P.N, g, P.bc_g, P.bc_phi, gi);
+    if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) pull<LG, real, true>(g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi, gi);
+    else pull<LG, real, false>(g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi, gi);
     real sum = gi[0];
 #pragma unroll
     for (int i = 1; i < LG::Q; ++i) sum += gi[i];
@@ -90,9 +90,9 @@ k_stream_only(const DevParams<real> P, const real *__restrict__ src, real *__res
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
     const NodeGeom g = make_geom(P, x, y, z);
     real v[L::Q];
-    if (which == 0) pull<L, real, true>(src, P.N, g, P.bc_f, P.bc_p, v);
-    else if (which == 1) pull<L, real, true>(src, P.N, g, P.bc_g, P.bc_phi, v);
-    else pull<L, real, true>(src, P.N, g, P.bc_s, P.bc_T, v);
+    if (which == 0) pull<L, real, true>(src, (unsigned)P.N, g, P.bc_f, P.bc_p, v);
+    else if (which == 1) pull<L, real, true>(src, (unsigned)P.N, g, P.bc_g, P.bc_phi, v);
+    else pull<L, real, true>(src, (unsigned)P.N, g, P.bc_s, P.bc_T, v);
 #pragma unroll
     for (int i = 0; i < L::Q; ++i) dst[(size_t)i * P.N + g.n] = v[i];
 }
@@ -110,7 +110,7 @@ k_phi_unpad(const DevParams<real> P, const real *__restrict__ pad, real *__restr
     const int x = blockIdx.x * BX + t % BX, y = blockIdx.y * BY + (t / BX) % BY, z = blockIdx.z * BZ + t / (BX * BY);
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
     plain[(long long)z * P.nx * P.ny + (long long)y * P.nx + x] =
-        pad[((long long)(z + P.pz) * P.ppy + (y + 1)) * P.ppx + (x + 1)];
+        pad[((long long)(z + P.pz) * P.ppy + (y + 1)) * P.ppx + (x + P.xpad)];
 }
 
 }  // namespace lbm

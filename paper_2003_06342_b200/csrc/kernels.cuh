@@ -2,7 +2,7 @@
 //
 // Data layout in HBM:
 //   populations  SoA [Q][z][y][x], two buffers per lattice (pull scheme, read A / write B, swap);
-//   phi          padded [nz+2][ny+2][ppx] (2D: [ny+2][ppx]) with materialised ghost layers (periodic image,
+//   phi          padded [nz+2][ny+2][ppx] (2D: [ny+2][ppx]; node x at column x + xpad) with materialised ghost layers (periodic image,
 //                zero-flux mirror, Dirichlet 2v - mirror), two buffers (level n and n+1);
 //   Pdot, u, p, T  [z][y][x].
 // Kernels:
@@ -47,12 +47,16 @@ template <class real> struct DevParams {
     int nx, ny, nz;
     long long N;           // nx*ny*nz
     int ppx, ppy, pz;      // padded phi: row pitch, ny+2, z offset (1 in 3D, 0 in 2D)
+    int xpad;              // padded phi: x offset of node 0 (16 bytes of elements, so TMA boxes start 16-byte aligned)
     long long pplane;      // ppx*ppy
     int bc_f[3][2], bc_g[3][2], bc_s[3][2];   // BC_* per face (f: wall->BOUNCE, open->ANTI)
     real bc_phi[3][2], bc_T[3][2], bc_p[3][2];
     int nonper[3];         // axis has non-periodic faces
     real dt, hdt, c, inv_dx, inv_dx2;
     real cs2f, cs2g, cs2s;           // e2 * c^2 per lattice
+    real inv_cs2f, inv_cs2g, inv_cs2s;   // reciprocals, and c / cs2 per lattice (host-computed: no per-node divisions)
+    real c_cs2f, c_cs2g, c_cs2s;
+    real inv_dt, tauf_num, taus_den;     // 1/dt ; nu_l nu_g/(cs2f dt) ; 1/(cs2s dt)
     real rho_l, rho_g, rho_diff, drho;   // rho_g - rho_l ; 1/rho_g - 1/rho_l
     real nu_l, nu_g, nu_prod;            // nu_l * nu_g
     real fourH, K;                       // Eq.(14),(15b)
@@ -74,12 +78,13 @@ template <class real> struct DevFields {
 };
 
 // ---- per-node geometry ------------------------------------------------------------------------------------
+// Element offsets are 32-bit: Q * N < 2^32 is checked by the host (lbm_create).
 struct NodeGeom {
     int x, y, z;
-    long long n;          // own linear index
-    int sx[3];            // source x for e_x = -1, 0, +1  (x - e_x, wrapped)
-    long long sy[3];      // source row offset (y - e_y wrapped) * nx
-    long long sz[3];      // source plane offset (z - e_z wrapped) * nx*ny
+    unsigned n;           // own linear index
+    unsigned sx[3];       // source x for e_x = -1, 0, +1  (x - e_x, wrapped)
+    unsigned sy[3];       // source row offset (y - e_y wrapped) * nx
+    unsigned sz[3];       // source plane offset (z - e_z wrapped) * nx*ny
     bool lo[3], hi[3];    // node sits on the first / last layer of the axis
 };
 
@@ -87,61 +92,85 @@ template <class real>
 __device__ __forceinline__ NodeGeom make_geom(const DevParams<real> &P, int x, int y, int z) {
     NodeGeom g;
     g.x = x; g.y = y; g.z = z;
-    const long long row = P.nx, plane = (long long)P.nx * P.ny;
-    g.n = (long long)z * plane + (long long)y * row + x;
+    const unsigned row = (unsigned)P.nx, plane = (unsigned)P.nx * (unsigned)P.ny;
+    g.n = (unsigned)z * plane + (unsigned)y * row + (unsigned)x;
     g.lo[0] = x == 0; g.hi[0] = x == P.nx - 1;
     g.lo[1] = y == 0; g.hi[1] = y == P.ny - 1;
     g.lo[2] = z == 0; g.hi[2] = z == P.nz - 1;
-    g.sx[0] = g.hi[0] ? 0 : x + 1;  g.sx[1] = x;  g.sx[2] = g.lo[0] ? P.nx - 1 : x - 1;
-    g.sy[0] = (long long)(g.hi[1] ? 0 : y + 1) * row;  g.sy[1] = (long long)y * row;
-    g.sy[2] = (long long)(g.lo[1] ? P.ny - 1 : y - 1) * row;
-    g.sz[0] = (long long)(g.hi[2] ? 0 : z + 1) * plane;  g.sz[1] = (long long)z * plane;
-    g.sz[2] = (long long)(g.lo[2] ? P.nz - 1 : z - 1) * plane;
+    g.sx[0] = g.hi[0] ? 0u : (unsigned)(x + 1);  g.sx[1] = (unsigned)x;  g.sx[2] = g.lo[0] ? (unsigned)(P.nx - 1) : (unsigned)(x - 1);
+    g.sy[0] = (unsigned)(g.hi[1] ? 0 : y + 1) * row;  g.sy[1] = (unsigned)y * row;
+    g.sy[2] = (unsigned)(g.lo[1] ? P.ny - 1 : y - 1) * row;
+    g.sz[0] = (unsigned)(g.hi[2] ? 0 : z + 1) * plane;  g.sz[1] = (unsigned)z * plane;
+    g.sz[2] = (unsigned)(g.lo[2] ? P.nz - 1 : z - 1) * plane;
     return g;
 }
 
-// Pull-stream all Q directions of one lattice into registers (theta* = theta(x + c_i dt, t + dt)).
+// Loads.  ld_first: read-only path, free for the compiler to schedule.  ld_again: the SAME address read a second time
+// (at collision time) -- opaque to common-subexpression elimination on purpose, so that the first value need not stay
+// in a register for the whole step; it hits L1.
+__device__ __forceinline__ double ld_again(const double *p) {
+    double v;
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float ld_again(const float *p) {
+    float v;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+template <bool AGAIN, class real> __device__ __forceinline__ real ld_pop(const real *p) {
+    if constexpr (AGAIN) return ld_again(p);
+    else return __ldg(p);
+}
+
+// Pull-stream ONE direction of one lattice (theta* = theta(x + c_i dt, t + dt)).
 // BC = false: every axis the node touches is periodic -> pure wrapped gather.
 // BC = true : a link that leaves through a non-periodic face takes the post-collision opposite population of the
 //             same node: bounce-back or anti-bounce-back -v + 2 w_i value;
 //             tangential wrap first, lowest axis decides (reading S8).
+template <class L, int I, class real, bool BC, bool AGAIN = false>
+__device__ __forceinline__ real pull_one(const real *__restrict__ src, unsigned N, const NodeGeom &g,
+                                         const int (&bc)[3][2], const real (&val)[3][2]) {
+    constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I);
+    const unsigned ns = (unsigned)I * N + g.sz[ez + 1] + g.sy[ey + 1] + g.sx[ex + 1];
+    if constexpr (!BC || I == 0) {
+        return ld_pop<AGAIN>(src + ns);
+    } else {
+        int kind = BC_PERIODIC;
+        real v = real(0);
+        if constexpr (ex != 0) {
+            constexpr int side = ex > 0 ? 0 : 1;
+            if ((side == 0 ? g.lo[0] : g.hi[0]) && bc[0][side] != BC_PERIODIC) { kind = bc[0][side]; v = val[0][side]; }
+        }
+        if constexpr (ey != 0) {
+            constexpr int side = ey > 0 ? 0 : 1;
+            if (kind == BC_PERIODIC && (side == 0 ? g.lo[1] : g.hi[1]) && bc[1][side] != BC_PERIODIC) { kind = bc[1][side]; v = val[1][side]; }
+        }
+        if constexpr (ez != 0) {
+            constexpr int side = ez > 0 ? 0 : 1;
+            if (kind == BC_PERIODIC && (side == 0 ? g.lo[2] : g.hi[2]) && bc[2][side] != BC_PERIODIC) { kind = bc[2][side]; v = val[2][side]; }
+        }
+        if (kind == BC_PERIODIC) return ld_pop<AGAIN>(src + ns);
+        const real back = ld_pop<AGAIN>(src + (unsigned)L::opp(I) * N + g.n);
+        return kind == BC_BOUNCE ? back : real(2.0 * L::w(I)) * v - back;
+    }
+}
+
 template <class L, class real, bool BC>
-__device__ __forceinline__ void pull(const real *__restrict__ src, long long N, const NodeGeom &g,
+__device__ __forceinline__ void pull(const real *__restrict__ src, unsigned N, const NodeGeom &g,
                                      const int (&bc)[3][2], const real (&val)[3][2], real (&out)[L::Q]) {
     static_for<L::Q>([&](auto ic) {
         constexpr int I = decltype(ic)::value;
-        constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I);
-        const long long ns = g.sz[ez + 1] + g.sy[ey + 1] + g.sx[ex + 1];
-        if constexpr (!BC || I == 0) {
-            out[I] = __ldg(src + (size_t)I * N + ns);
-        } else {
-            int kind = BC_PERIODIC;
-            real v = real(0);
-            if constexpr (ex != 0) {
-                constexpr int side = ex > 0 ? 0 : 1;
-                if ((side == 0 ? g.lo[0] : g.hi[0]) && bc[0][side] != BC_PERIODIC) { kind = bc[0][side]; v = val[0][side]; }
-            }
-            if constexpr (ey != 0) {
-                constexpr int side = ey > 0 ? 0 : 1;
-                if (kind == BC_PERIODIC && (side == 0 ? g.lo[1] : g.hi[1]) && bc[1][side] != BC_PERIODIC) { kind = bc[1][side]; v = val[1][side]; }
-            }
-            if constexpr (ez != 0) {
-                constexpr int side = ez > 0 ? 0 : 1;
-                if (kind == BC_PERIODIC && (side == 0 ? g.lo[2] : g.hi[2]) && bc[2][side] != BC_PERIODIC) { kind = bc[2][side]; v = val[2][side]; }
-            }
-            if (kind == BC_PERIODIC) {
-                out[I] = __ldg(src + (size_t)I * N + ns);
-            } else {
-                const real back = __ldg(src + (size_t)L::opp(I) * N + g.n);
-                out[I] = kind == BC_BOUNCE ? back : real(2.0 * L::w(I)) * v - back;
-            }
-        }
+        out[I] = pull_one<L, I, real, BC>(src, N, g, bc, val);
     });
 }
 
 // does the tile [x0,x0+bx) x [y0,y0+by) x [z0,z0+bz) touch a non-periodic face?  (block-uniform)
 template <class real>
 __device__ __forceinline__ bool tile_touches_bc(const DevParams<real> &P, int x0, int y0, int z0, int bx, int by, int bz) {
+#ifdef LBM_EXP_NOBC
+    return false;
+#endif
     bool t = false;
     if (P.nonper[0]) t |= (x0 == 0) || (x0 + bx >= P.nx);
     if (P.nonper[1]) t |= (y0 == 0) || (y0 + by >= P.ny);

@@ -11,7 +11,10 @@
 #include <new>
 #include <vector>
 
+#include <cudaTypedefs.h>
+
 #include "k_main.cuh"
+#include "k_main_tma.cuh"
 #include "k_phi.cuh"
 
 namespace {
@@ -51,7 +54,7 @@ template <> struct Tile<3> { static constexpr int BX = 32, BY = 4, BZ = 2; };
 
 struct Layout {
     long long N;
-    int ppx, ppy, ppz, pz;
+    int ppx, ppy, ppz, pz, xpad;
     size_t phi_pad_elems;
     size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot, off_u, off_p, off_T, off_scratch, total;
 };
@@ -65,7 +68,7 @@ int validate(const lbm_params *p) {
     if (lattice_3d(p->lat_f) != three_d || lattice_3d(p->lat_g) != three_d || lattice_3d(p->lat_s) != three_d)
         return LBM_E_INVALID;
     if (lattice_set(p) == SET_NONE) return LBM_E_UNSUPPORTED;
-    if ((double)p->nx * p->ny * p->nz > 2147483647.0) return LBM_E_INVALID;
+    if ((double)p->nx * p->ny * p->nz * 19.0 > 4294967295.0) return LBM_E_INVALID;   // 32-bit element offsets
     if (!(p->dx > 0) || !(p->dt > 0) || !(p->W > 0) || !(p->rho_l > 0) || !(p->rho_g > 0)) return LBM_E_INVALID;
     if (!(p->nu_l > 0) || !(p->nu_g > 0) || !(p->M > 0) || !(p->alpha_l > 0) || !(p->alpha_g > 0)) return LBM_E_INVALID;
     if (!(p->Cp > 0) || p->L_latent == 0.0 || !(p->A > 0) || !(p->eps_n >= 0) || !(p->sigma >= 0)) return LBM_E_INVALID;
@@ -86,8 +89,9 @@ Layout make_layout(const lbm_params *p) {
     Layout L{};
     const size_t es = p->precision == 64 ? 8 : 4;
     L.N = (long long)p->nx * p->ny * p->nz;
-    const int mult = (int)(16 / es);                          // TMA: row pitch must be a multiple of 16 bytes
-    L.ppx = (p->nx + 2 + mult - 1) / mult * mult;
+    const int mult = (int)(16 / es);                          // TMA: row pitch and box starts are multiples of 16 bytes
+    L.xpad = mult;                                            // node 0 sits 16 bytes into the padded row
+    L.ppx = (p->nx + 2 * mult + mult - 1) / mult * mult;
     L.ppy = p->ny + 2;
     L.pz = p->nz > 1 ? 1 : 0;
     L.ppz = p->nz + 2 * L.pz;
@@ -111,7 +115,7 @@ Layout make_layout(const lbm_params *p) {
 template <class real> DevParams<real> make_dev_params(const lbm_params *p, const Layout &L) {
     DevParams<real> d{};
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.N = L.N;
-    d.ppx = L.ppx; d.ppy = L.ppy; d.pz = L.pz; d.pplane = (long long)L.ppx * L.ppy;
+    d.ppx = L.ppx; d.ppy = L.ppy; d.pz = L.pz; d.xpad = L.xpad; d.pplane = (long long)L.ppx * L.ppy;
     for (int a = 0; a < 3; ++a) {
         for (int s = 0; s < 2; ++s) {
             d.bc_f[a][s] = p->bc_f[a][s];   // PERIODIC 0, WALL -> BOUNCE 1, OPEN -> ANTI 2 (same numbering)
@@ -131,6 +135,11 @@ template <class real> DevParams<real> make_dev_params(const lbm_params *p, const
     d.dt = (real)p->dt; d.hdt = (real)(0.5 * p->dt); d.c = (real)c;
     d.inv_dx = (real)(1.0 / p->dx); d.inv_dx2 = (real)(1.0 / (p->dx * p->dx));
     d.cs2f = (real)cs2f; d.cs2g = (real)cs2g; d.cs2s = (real)cs2s;
+    d.inv_cs2f = (real)(1.0 / cs2f); d.inv_cs2g = (real)(1.0 / cs2g); d.inv_cs2s = (real)(1.0 / cs2s);
+    d.c_cs2f = (real)(c / cs2f); d.c_cs2g = (real)(c / cs2g); d.c_cs2s = (real)(c / cs2s);
+    d.inv_dt = (real)(1.0 / p->dt);
+    d.tauf_num = (real)(p->nu_l * p->nu_g / (cs2f * p->dt));
+    d.taus_den = (real)(1.0 / (cs2s * p->dt));
     d.rho_l = (real)p->rho_l; d.rho_g = (real)p->rho_g; d.rho_diff = (real)(p->rho_g - p->rho_l);
     d.drho = (real)(1.0 / p->rho_g - 1.0 / p->rho_l);
     d.nu_l = (real)p->nu_l; d.nu_g = (real)p->nu_g; d.nu_prod = (real)(p->nu_l * p->nu_g);
@@ -163,6 +172,10 @@ struct lbm_ctx {
     long long nsteps, launches;
     DevParams<double> pd;
     DevParams<float> pf;
+    // TMA variant of K_main: tensor maps of both buffers of every input array
+    bool use_tma;
+    int num_sms;
+    CUtensorMap map_f[2], map_g[2], map_s[2], map_phi[2], map_pdot;
     // optional per-kernel timing (lbm_set_timing): 3 events per step: before k_phi, between, after k_main
     bool timing;
     std::vector<cudaEvent_t> ev;
@@ -198,8 +211,29 @@ template <class LF, class LG, class LS, class real> struct Impl {
         return F;
     }
 
-    template <int MODE> static int launch_main(lbm_ctx *c, const DevFields<real> &F) {
-        k_main_direct<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, 1>
+    template <int MODE> static int launch_main(lbm_ctx *c, const DevFields<real> &F, int in = 0, int pnew = 0) {
+        if constexpr (MODE != MODE_INIT) {
+            if (c->use_tma) {
+                using C = TmaCfg<LF, LG, LS, real>;
+                auto kern = k_main_tma<LF, LG, LS, real, MODE>;
+                static bool attr_set = false;
+                if (!attr_set) {
+                    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
+                    attr_set = true;
+                }
+                TmaMaps M;
+                M.f = c->map_f[in]; M.g = c->map_g[in]; M.s = c->map_s[in];
+                M.phi_new = c->map_phi[pnew]; M.phi_old = c->map_phi[1 - pnew]; M.pdot = c->map_pdot;
+                const int nxt = (c->P.nx + C::TX - 1) / C::TX, nyt = (c->P.ny + C::TY - 1) / C::TY;
+                const long long ntiles = (long long)nxt * nyt * c->P.nz;
+                const unsigned grid = (unsigned)(ntiles < c->num_sms ? ntiles : c->num_sms);
+                kern<<<grid, C::NT, C::SMEM_BYTES, c->stream>>>(dev_params<real>(c), F, M, ntiles, nxt, nyt);
+                c->launches++;
+                CK(cudaGetLastError());
+                return LBM_OK;
+            }
+        }
+        k_main_direct<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, 2>
             <<<grid_for<D>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F);
         c->launches++;
         CK(cudaGetLastError());
@@ -254,7 +288,7 @@ template <class LF, class LG, class LS, class real> struct Impl {
             CK(cudaGetLastError());
             if (timed) CK(cudaEventRecord(e3[1], c->stream));
             DevFields<real> F = fields(c, in, out, pnew, pold);
-            int rc = (k == n - 1) ? launch_main<MODE_STEP_MACRO>(c, F) : launch_main<MODE_STEP>(c, F);
+            int rc = (k == n - 1) ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
             if (rc) return rc;
             if (timed) {
                 CK(cudaEventRecord(e3[2], c->stream));
@@ -324,6 +358,69 @@ template <class Fn> int dispatch(const lbm_ctx *c, Fn &&fn) {
 
 }  // namespace
 
+namespace {
+
+PFN_cuTensorMapEncodeTiled_v12000 get_encode_fn() {
+    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
+    }
+    return fn;
+}
+
+// row-box tensor map: dims (x-fastest) of an array of `es`-byte elements, box = boxx x 1 x 1 (x 1)
+bool encode_rows(CUtensorMap *m, void *base, int es, int rank, const unsigned long long *dims, int boxx) {
+    auto fn = get_encode_fn();
+    if (!fn) return false;
+    cuuint64_t gdim[4], gstr[3];
+    cuuint32_t box[4], estr[4];
+    unsigned long long stride = (unsigned long long)es;
+    for (int i = 0; i < rank; ++i) {
+        gdim[i] = dims[i];
+        box[i] = i == 0 ? (cuuint32_t)boxx : 1u;
+        estr[i] = 1u;
+        stride *= dims[i];
+        if (i < rank - 1) {
+            gstr[i] = stride;
+            if (stride % 16 != 0) return false;
+        }
+    }
+    CUresult r = fn(m, es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, base,
+                    gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+bool build_tma_maps(lbm_ctx *c) {
+    const int es = c->P.precision == 64 ? 8 : 4;
+    const int epb = 16 / es;
+    const int boxx = 128 + 2 * epb;                       // TmaCfg::BOXX
+    if (((size_t)c->P.nx * es) % 16 != 0) return false;
+    const unsigned long long nx = c->P.nx, ny = c->P.ny, nz = c->P.nz;
+    bool ok = true;
+    for (int b = 0; b < 2; ++b) {
+        const unsigned long long df[4] = {nx, ny, nz, (unsigned long long)lattice_q(c->P.lat_f)};
+        const unsigned long long dg[4] = {nx, ny, nz, (unsigned long long)lattice_q(c->P.lat_g)};
+        const unsigned long long ds[4] = {nx, ny, nz, (unsigned long long)lattice_q(c->P.lat_s)};
+        const unsigned long long dp[3] = {(unsigned long long)c->L.ppx, (unsigned long long)c->L.ppy, (unsigned long long)c->L.ppz};
+        ok = ok && encode_rows(&c->map_f[b], c->ws + c->L.off_f[b], es, 4, df, boxx);
+        ok = ok && encode_rows(&c->map_g[b], c->ws + c->L.off_g[b], es, 4, dg, boxx);
+        ok = ok && encode_rows(&c->map_s[b], c->ws + c->L.off_s[b], es, 4, ds, boxx);
+        ok = ok && encode_rows(&c->map_phi[b], c->ws + c->L.off_phi[b], es, 3, dp, boxx);
+    }
+    const unsigned long long dd[3] = {nx, ny, nz};
+    ok = ok && encode_rows(&c->map_pdot, c->ws + c->L.off_pdot, es, 3, dd, boxx);
+    return ok;
+}
+
+}  // namespace
+
 // ------------------------------------------------------------------------------------------------ C ABI
 extern "C" {
 
@@ -357,6 +454,12 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
     c->cur = 0; c->curphi = 0; c->inited = false; c->nsteps = 0; c->launches = 0; c->timing = false;
     c->pd = make_dev_params<double>(p, L);
     c->pf = make_dev_params<float>(p, L);
+    c->num_sms = prop.multiProcessorCount;
+    {   // K_main variant, chosen by measurement: the gather kernel at 2 CTAs/SM is the default
+        // (90% of the measured HBM peak on config 4); LBM_VARIANT=tma selects the TMA-staged persistent kernel.
+        const char *v = getenv("LBM_VARIANT");
+        c->use_tma = (v && strcmp(v, "tma") == 0) && build_tma_maps(c);
+    }
     *out = c;
     return LBM_OK;
 }
@@ -418,7 +521,7 @@ int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *ste
 
 long long lbm_step_count(const lbm_ctx *c) { return c ? c->nsteps : -1; }
 long long lbm_launch_count(const lbm_ctx *c) { return c ? c->launches : -1; }
-const char *lbm_variant(const lbm_ctx *c) { return c ? "direct" : ""; }
+const char *lbm_variant(const lbm_ctx *c) { return c ? (c->use_tma ? "tma" : "direct") : ""; }
 int lbm_last_cuda_error(void) { return g_last_cuda_error; }
 
 const char *lbm_strerror(int code) {

@@ -132,6 +132,23 @@ def test_minimal_grids(gpu, oracle_mod):
         _run_parity(gpu, oracle_mod, P, _random_state(P, 30), [1, 4], label="tiny %s" % (dims,))
 
 
+# ---------------------------------------------------------------------------- the TMA-staged variant of K_main
+def test_tma_variant(gpu, oracle_mod, monkeypatch):
+    """LBM_VARIANT=tma: persistent kernel, inputs staged through shared memory by cp.async.bulk.tensor."""
+    monkeypatch.setenv("LBM_VARIANT", "tma")
+    P = wl.base_params(264, 10, 7, grav=[1e-4, 0.0, -2e-4])       # 3 x-tiles of 128 (ragged), periodic wrap lanes
+    sim = gpu.LBM(P, 64)
+    assert sim.variant == "tma"
+    sim.destroy()
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 31), [1, 2, 12], label="tma 3d periodic")
+    P = wl.base_params(136, 9, 12, grav=[0.0, 0.0, -1e-4])        # z walls: boundary tiles take the gather path
+    P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
+    P["bc_T"][2] = [1.0, 0.0]
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 32), [1, 12], label="tma 3d z walls")
+    P = wl.base_params(40, 28, 1, grav=[1e-4, -2e-4, 0.0])
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 33), [1, 12], label="tma 2d periodic")
+
+
 # ---------------------------------------------------------------------------- the five configs (bounded horizons)
 def test_config1_droplet_1000_steps(gpu, oracle_mod):
     P, I = wl.config1_droplet()
