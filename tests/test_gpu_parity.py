@@ -191,6 +191,34 @@ def test_config5_droplets_reduced_220_steps(gpu, oracle_mod):
     _run_parity(gpu, oracle_mod, P, (I["phi"], I["T"]), [20, 220], pops=False, label="config5 40^3")
 
 
+# ---------------------------------------------------------------------------- full size, bench.py's launch configuration
+def test_config4_full_size_periodic_replica(gpu, oracle_mod):
+    """BASELINE.json configs[3] at FULL size (256x256x512, the grid bench.py times, same kernels and launch shapes).
+    The oracle cannot step 33.5 M nodes in seconds, so the input is a 64x64 (x, y) film-boiling pattern replicated
+    4x4 times: x and y are periodic, hence the exact solution is the same replication of the 64x64x512 solution,
+    which the oracle computes.  Every one of the 33.5 M outputs is compared."""
+    Ps, Is = wl.config4_film3d(nx=64, ny=64, nz=512)
+    P, _ = wl.config4_film3d(nx=8, ny=8, nz=8)
+    P.update(nx=256, ny=256, nz=512)
+    phi = np.tile(Is["phi"], (1, 4, 4))
+    T = np.tile(Is["T"], (1, 4, 4))
+    steps = 10
+    sim = gpu.LBM(P, 64)
+    sim.init(phi, T)
+    sim.step(steps)
+    got = sim.read_macro()
+    sim.destroy()
+    o = oracle_mod.Oracle(Ps)
+    o.init(Is["phi"], Is["T"])
+    o.step(steps)
+    ref = o.read_macro()
+    o.close()
+    for a, r, name in zip(got, ref, ("phi", "u", "p", "T")):
+        reps = (1, 1, 4, 4) if a.ndim == 4 else (1, 4, 4)
+        err = float(np.abs(a - np.tile(r, reps)).max())
+        assert err <= TOL64, (name, err)
+
+
 # ---------------------------------------------------------------------------- fp32 variant
 def test_fp32_variant_config5_reduced(gpu, oracle_mod):
     P, I = wl.config5_droplets(n=40, nspheres=6, rmin=4.0, rmax=8.0)
