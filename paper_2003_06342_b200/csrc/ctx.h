@@ -1,0 +1,71 @@
+// Host-side declarations shared by the C-ABI translation unit (lbm.cu) and the per-lattice-set instantiation units
+// (inst_*.cu).  Not part of the public boundary (that is include/lbm.h).
+#pragma once
+
+#include "../../include/lbm.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <vector>
+
+#include "kernels.cuh"
+
+namespace lbm {
+
+extern int g_last_cuda_error;
+
+#define CK(call)                                                     \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) { lbm::g_last_cuda_error = (int)e_; return LBM_E_CUDA; } \
+    } while (0)
+
+enum LatSet { SET_NONE = 0, SET_2D_995, SET_2D_999, SET_3D_1977 };
+
+struct Layout {
+    long long N;
+    int ppx, ppy, ppz, pz, xpad;
+    size_t phi_pad_elems;
+    size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot, off_u, off_p, off_T, off_scratch, total;
+};
+
+// One implementation = one (lattice set, precision, tile shape); chosen once in lbm_create.
+struct ImplOps {
+    int (*init)(lbm_ctx *, const void *, const void *, const void *, const void *);
+    int (*step)(lbm_ctx *, int);
+    int (*read_macro)(lbm_ctx *, void *, void *, void *, void *);
+    int (*read_pops)(lbm_ctx *, int, int, void *);
+};
+
+// defined in inst_*.cu (compiled in parallel); nx selects the tile shape
+const ImplOps *ops_2d995_f64(int nx);
+const ImplOps *ops_2d995_f32(int nx);
+const ImplOps *ops_2d999_f64(int nx);
+const ImplOps *ops_2d999_f32(int nx);
+const ImplOps *ops_3d_f64(int nx);
+const ImplOps *ops_3d_f32(int nx);
+
+}  // namespace lbm
+
+struct lbm_ctx {
+    lbm_params P;
+    lbm::Layout L;
+    lbm::LatSet set;
+    const lbm::ImplOps *ops;
+    char *ws;
+    cudaStream_t stream;
+    int cur;       // buffer holding the post-collision populations of the current level
+    int curphi;    // padded phi buffer of the current level
+    bool inited;
+    long long nsteps, launches;
+    lbm::DevParams<double> pd;
+    lbm::DevParams<float> pf;
+    // TMA variant of K_main: tensor maps of both buffers of every input array
+    bool use_tma;
+    int num_sms;
+    CUtensorMap map_f[2], map_g[2], map_s[2], map_phi[2], map_pdot;
+    // optional per-kernel timing (lbm_set_timing): 3 events per step: before k_phi, between, after k_main
+    bool timing;
+    std::vector<cudaEvent_t> ev;
+};

@@ -13,21 +13,15 @@
 
 #include <cudaTypedefs.h>
 
-#include "k_main.cuh"
-#include "k_main_tma.cuh"
-#include "k_phi.cuh"
+#include "ctx.h"
+
+namespace lbm {
+int g_last_cuda_error = 0;
+}
 
 namespace {
 
 using namespace lbm;
-
-int g_last_cuda_error = 0;
-
-#define CK(call)                                                     \
-    do {                                                             \
-        cudaError_t e_ = (call);                                     \
-        if (e_ != cudaSuccess) { g_last_cuda_error = (int)e_; return LBM_E_CUDA; } \
-    } while (0)
 
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
@@ -38,26 +32,12 @@ int lattice_q(int id) {
 }
 bool lattice_3d(int id) { return id == LBM_D3Q7 || id == LBM_D3Q19; }
 
-enum LatSet { SET_NONE = 0, SET_2D_995, SET_2D_999, SET_3D_1977 };
-
 LatSet lattice_set(const lbm_params *p) {
     if (p->lat_f == LBM_D2Q9 && p->lat_g == LBM_D2Q9 && p->lat_s == LBM_D2Q5) return SET_2D_995;
     if (p->lat_f == LBM_D2Q9 && p->lat_g == LBM_D2Q9 && p->lat_s == LBM_D2Q9) return SET_2D_999;
     if (p->lat_f == LBM_D3Q19 && p->lat_g == LBM_D3Q7 && p->lat_s == LBM_D3Q7) return SET_3D_1977;
     return SET_NONE;
 }
-
-// tile of nodes per thread block (one node per thread)
-template <int D> struct Tile;
-template <> struct Tile<2> { static constexpr int BX = 32, BY = 8, BZ = 1; };
-template <> struct Tile<3> { static constexpr int BX = 32, BY = 4, BZ = 2; };
-
-struct Layout {
-    long long N;
-    int ppx, ppy, ppz, pz, xpad;
-    size_t phi_pad_elems;
-    size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot, off_u, off_p, off_T, off_scratch, total;
-};
 
 int validate(const lbm_params *p) {
     if (!p) return LBM_E_INVALID;
@@ -160,204 +140,6 @@ template <class real> DevParams<real> make_dev_params(const lbm_params *p, const
 
 }  // namespace
 
-struct lbm_ctx {
-    lbm_params P;
-    Layout L;
-    LatSet set;
-    char *ws;
-    cudaStream_t stream;
-    int cur;       // buffer holding the post-collision populations of the current level
-    int curphi;    // padded phi buffer of the current level
-    bool inited;
-    long long nsteps, launches;
-    DevParams<double> pd;
-    DevParams<float> pf;
-    // TMA variant of K_main: tensor maps of both buffers of every input array
-    bool use_tma;
-    int num_sms;
-    CUtensorMap map_f[2], map_g[2], map_s[2], map_phi[2], map_pdot;
-    // optional per-kernel timing (lbm_set_timing): 3 events per step: before k_phi, between, after k_main
-    bool timing;
-    std::vector<cudaEvent_t> ev;
-};
-
-namespace {
-
-template <class real> const DevParams<real> &dev_params(const lbm_ctx *c);
-template <> const DevParams<double> &dev_params<double>(const lbm_ctx *c) { return c->pd; }
-template <> const DevParams<float> &dev_params<float>(const lbm_ctx *c) { return c->pf; }
-
-template <class real> real *wsp(const lbm_ctx *c, size_t off) { return reinterpret_cast<real *>(c->ws + off); }
-
-template <int D> dim3 grid_for(const lbm_params &P) {
-    using T = Tile<D>;
-    return dim3((P.nx + T::BX - 1) / T::BX, (P.ny + T::BY - 1) / T::BY, (P.nz + T::BZ - 1) / T::BZ);
-}
-
-template <class LF, class LG, class LS, class real> struct Impl {
-    static constexpr int D = LF::D;
-    using T = Tile<D>;
-    static constexpr int NT = T::BX * T::BY * T::BZ;
-
-    static DevFields<real> fields(const lbm_ctx *c, int in, int out, int phi_new, int phi_old) {
-        DevFields<real> F{};
-        F.f_in = wsp<real>(c, c->L.off_f[in]);  F.f_out = wsp<real>(c, c->L.off_f[out]);
-        F.g_in = wsp<real>(c, c->L.off_g[in]);  F.g_out = wsp<real>(c, c->L.off_g[out]);
-        F.s_in = wsp<real>(c, c->L.off_s[in]);  F.s_out = wsp<real>(c, c->L.off_s[out]);
-        F.phi_new = wsp<real>(c, c->L.off_phi[phi_new]);
-        F.phi_old = wsp<real>(c, c->L.off_phi[phi_old]);
-        F.pdot = wsp<real>(c, c->L.off_pdot);
-        F.u = wsp<real>(c, c->L.off_u); F.p = wsp<real>(c, c->L.off_p); F.T = wsp<real>(c, c->L.off_T);
-        return F;
-    }
-
-    template <int MODE> static int launch_main(lbm_ctx *c, const DevFields<real> &F, int in = 0, int pnew = 0) {
-        if constexpr (MODE != MODE_INIT) {
-            if (c->use_tma) {
-                using C = TmaCfg<LF, LG, LS, real>;
-                auto kern = k_main_tma<LF, LG, LS, real, MODE>;
-                static bool attr_set = false;
-                if (!attr_set) {
-                    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-                    attr_set = true;
-                }
-                TmaMaps M;
-                M.f = c->map_f[in]; M.g = c->map_g[in]; M.s = c->map_s[in];
-                M.phi_new = c->map_phi[pnew]; M.phi_old = c->map_phi[1 - pnew]; M.pdot = c->map_pdot;
-                const int nxt = (c->P.nx + C::TX - 1) / C::TX, nyt = (c->P.ny + C::TY - 1) / C::TY;
-                const long long ntiles = (long long)nxt * nyt * c->P.nz;
-                const unsigned grid = (unsigned)(ntiles < c->num_sms ? ntiles : c->num_sms);
-                kern<<<grid, C::NT, C::SMEM_BYTES, c->stream>>>(dev_params<real>(c), F, M, ntiles, nxt, nyt);
-                c->launches++;
-                CK(cudaGetLastError());
-                return LBM_OK;
-            }
-        }
-        k_main_direct<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, 2>
-            <<<grid_for<D>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F);
-        c->launches++;
-        CK(cudaGetLastError());
-        return LBM_OK;
-    }
-
-    static int init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, const void *h_p) {
-        const size_t N = (size_t)c->L.N, es = sizeof(real);
-        const DevParams<real> &P = dev_params<real>(c);
-        real *scratch = wsp<real>(c, c->L.off_scratch);
-        CK(cudaMemcpyAsync(scratch, h_phi, N * es, cudaMemcpyHostToDevice, c->stream));
-        real *dT = wsp<real>(c, c->L.off_T), *du = wsp<real>(c, c->L.off_u), *dp = wsp<real>(c, c->L.off_p);
-        if (h_T) CK(cudaMemcpyAsync(dT, h_T, N * es, cudaMemcpyHostToDevice, c->stream));
-        else {
-            k_fill<real><<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(dT, (long long)N, (real)c->P.T_sat);
-            c->launches++;
-            CK(cudaGetLastError());
-        }
-        if (h_u) CK(cudaMemcpyAsync(du, h_u, 3 * N * es, cudaMemcpyHostToDevice, c->stream));
-        else CK(cudaMemsetAsync(du, 0, 3 * N * es, c->stream));
-        if (h_p) CK(cudaMemcpyAsync(dp, h_p, N * es, cudaMemcpyHostToDevice, c->stream));
-        else CK(cudaMemsetAsync(dp, 0, N * es, c->stream));
-        for (int b = 0; b < 2; ++b)
-            CK(cudaMemsetAsync(wsp<real>(c, c->L.off_phi[b]), 0, c->L.phi_pad_elems * es, c->stream));
-        k_phi_fill<real, T::BX, T::BY, T::BZ><<<grid_for<D>(c->P), NT, 0, c->stream>>>(
-            P, scratch, wsp<real>(c, c->L.off_phi[0]), wsp<real>(c, c->L.off_phi[1]));
-        c->launches++;
-        CK(cudaGetLastError());
-        c->cur = 0; c->curphi = 0;
-        DevFields<real> F = fields(c, 1, 0, 0, 0);   // INIT reads no populations; writes buffer 0
-        int rc = launch_main<MODE_INIT>(c, F);
-        if (rc) return rc;
-        CK(cudaStreamSynchronize(c->stream));
-        c->nsteps = 0;
-        c->inited = true;
-        return LBM_OK;
-    }
-
-    static int step(lbm_ctx *c, int n) {
-        const DevParams<real> &P = dev_params<real>(c);
-        for (int k = 0; k < n; ++k) {
-            const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
-            const bool timed = c->timing && c->ev.size() < 3 * 4096;
-            cudaEvent_t e3[3] = {nullptr, nullptr, nullptr};
-            if (timed) {
-                for (auto &e : e3) CK(cudaEventCreate(&e));
-                CK(cudaEventRecord(e3[0], c->stream));
-            }
-            k_phi<LG, real, T::BX, T::BY, T::BZ><<<grid_for<D>(c->P), NT, 0, c->stream>>>(
-                P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot), wsp<real>(c, c->L.off_phi[pnew]));
-            c->launches++;
-            CK(cudaGetLastError());
-            if (timed) CK(cudaEventRecord(e3[1], c->stream));
-            DevFields<real> F = fields(c, in, out, pnew, pold);
-            int rc = (k == n - 1) ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
-            if (rc) return rc;
-            if (timed) {
-                CK(cudaEventRecord(e3[2], c->stream));
-                for (auto e : e3) c->ev.push_back(e);
-            }
-            c->cur = out; c->curphi = pnew; c->nsteps++;
-        }
-        return LBM_OK;
-    }
-
-    static int read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T) {
-        const size_t N = (size_t)c->L.N, es = sizeof(real);
-        if (h_phi) {
-            real *scratch = wsp<real>(c, c->L.off_scratch);
-            k_phi_unpad<real, T::BX, T::BY, T::BZ><<<grid_for<D>(c->P), NT, 0, c->stream>>>(
-                dev_params<real>(c), wsp<real>(c, c->L.off_phi[c->curphi]), scratch);
-            c->launches++;
-            CK(cudaGetLastError());
-            CK(cudaMemcpyAsync(h_phi, scratch, N * es, cudaMemcpyDeviceToHost, c->stream));
-        }
-        if (h_u) CK(cudaMemcpyAsync(h_u, wsp<real>(c, c->L.off_u), 3 * N * es, cudaMemcpyDeviceToHost, c->stream));
-        if (h_p) CK(cudaMemcpyAsync(h_p, wsp<real>(c, c->L.off_p), N * es, cudaMemcpyDeviceToHost, c->stream));
-        if (h_T) CK(cudaMemcpyAsync(h_T, wsp<real>(c, c->L.off_T), N * es, cudaMemcpyDeviceToHost, c->stream));
-        CK(cudaStreamSynchronize(c->stream));
-        return LBM_OK;
-    }
-
-    template <class L> static int read_pops_one(lbm_ctx *c, int which, int stage, const size_t (&off)[2], void *h) {
-        const size_t N = (size_t)c->L.N, bytes = (size_t)L::Q * N * sizeof(real);
-        if (stage == LBM_STAGE_POSTCOLLISION) {
-            CK(cudaMemcpyAsync(h, wsp<real>(c, off[c->cur]), bytes, cudaMemcpyDeviceToHost, c->stream));
-            CK(cudaStreamSynchronize(c->stream));
-            return LBM_OK;
-        }
-        if (c->nsteps < 1) return LBM_E_STATE;
-        real *tmp = nullptr;
-        CK(cudaMalloc(&tmp, bytes));   // debug path: own temporary, not the borrowed workspace
-        k_stream_only<L, real, T::BX, T::BY, T::BZ><<<grid_for<D>(c->P), NT, 0, c->stream>>>(
-            dev_params<real>(c), wsp<real>(c, off[1 - c->cur]), tmp, which);
-        c->launches++;
-        cudaError_t e = cudaGetLastError();
-        if (e == cudaSuccess) e = cudaMemcpyAsync(h, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-        cudaFree(tmp);
-        CK(e);
-        return LBM_OK;
-    }
-
-    static int read_pops(lbm_ctx *c, int which, int stage, void *h) {
-        if (which == LBM_POPS_F) return read_pops_one<LF>(c, which, stage, c->L.off_f, h);
-        if (which == LBM_POPS_G) return read_pops_one<LG>(c, which, stage, c->L.off_g, h);
-        if (which == LBM_POPS_S) return read_pops_one<LS>(c, which, stage, c->L.off_s, h);
-        return LBM_E_INVALID;
-    }
-};
-
-// dispatch on (lattice set, precision)
-template <class Fn> int dispatch(const lbm_ctx *c, Fn &&fn) {
-    const bool d = c->P.precision == 64;
-    switch (c->set) {
-    case SET_2D_995: return d ? fn(Impl<D2Q9, D2Q9, D2Q5, double>{}) : fn(Impl<D2Q9, D2Q9, D2Q5, float>{});
-    case SET_2D_999: return d ? fn(Impl<D2Q9, D2Q9, D2Q9, double>{}) : fn(Impl<D2Q9, D2Q9, D2Q9, float>{});
-    case SET_3D_1977: return d ? fn(Impl<D3Q19, D3Q7, D3Q7, double>{}) : fn(Impl<D3Q19, D3Q7, D3Q7, float>{});
-    default: return LBM_E_UNSUPPORTED;
-    }
-}
-
-}  // namespace
-
 namespace {
 
 PFN_cuTensorMapEncodeTiled_v12000 get_encode_fn() {
@@ -449,6 +231,15 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
     lbm_ctx *c = new (std::nothrow) lbm_ctx();
     if (!c) return LBM_E_INVALID;
     c->P = *p; c->L = L; c->set = lattice_set(p);
+    {
+        const bool d = p->precision == 64;
+        switch (c->set) {
+        case SET_2D_995: c->ops = d ? ops_2d995_f64(p->nx) : ops_2d995_f32(p->nx); break;
+        case SET_2D_999: c->ops = d ? ops_2d999_f64(p->nx) : ops_2d999_f32(p->nx); break;
+        case SET_3D_1977: c->ops = d ? ops_3d_f64(p->nx) : ops_3d_f32(p->nx); break;
+        default: delete c; return LBM_E_UNSUPPORTED;
+        }
+    }
     c->ws = static_cast<char *>(d_workspace);
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     c->cur = 0; c->curphi = 0; c->inited = false; c->nsteps = 0; c->launches = 0; c->timing = false;
@@ -466,26 +257,26 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
 
 int lbm_init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, const void *h_p) {
     if (!c || !h_phi) return LBM_E_INVALID;
-    return dispatch(c, [&](auto impl) { return decltype(impl)::init(c, h_phi, h_T, h_u, h_p); });
+    return c->ops->init(c, h_phi, h_T, h_u, h_p);
 }
 
 int lbm_step(lbm_ctx *c, int n) {
     if (!c || n < 0) return LBM_E_INVALID;
     if (!c->inited) return LBM_E_STATE;
-    return dispatch(c, [&](auto impl) { return decltype(impl)::step(c, n); });
+    return c->ops->step(c, n);
 }
 
 int lbm_read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T) {
     if (!c) return LBM_E_INVALID;
     if (!c->inited) return LBM_E_STATE;
-    return dispatch(c, [&](auto impl) { return decltype(impl)::read_macro(c, h_phi, h_u, h_p, h_T); });
+    return c->ops->read_macro(c, h_phi, h_u, h_p, h_T);
 }
 
 int lbm_read_pops(lbm_ctx *c, int which, int stage, void *h_pops) {
     if (!c || !h_pops || which < 0 || which > 2 || (stage != LBM_STAGE_POSTCOLLISION && stage != LBM_STAGE_STREAMED))
         return LBM_E_INVALID;
     if (!c->inited) return LBM_E_STATE;
-    return dispatch(c, [&](auto impl) { return decltype(impl)::read_pops(c, which, stage, h_pops); });
+    return c->ops->read_pops(c, which, stage, h_pops);
 }
 
 int lbm_sync(lbm_ctx *c) {
