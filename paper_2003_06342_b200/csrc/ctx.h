@@ -36,6 +36,7 @@ struct ImplOps {
     int (*step)(lbm_ctx *, int);
     int (*read_macro)(lbm_ctx *, void *, void *, void *, void *);
     int (*read_pops)(lbm_ctx *, int, int, void *);
+    int bx, by, bz;   // tile of nodes per CTA
 };
 
 // defined in inst_*.cu (compiled in parallel); nx selects the tile shape
@@ -65,6 +66,9 @@ struct lbm_ctx {
     bool use_tma;
     int num_sms;
     CUtensorMap map_f[2], map_g[2], map_s[2], map_phi[2], map_pdot;
+    // gather kernel with the phi halo tile staged by TMA: one box per CTA
+    bool phi_tma;
+    CUtensorMap map_phi_tile[2];
     // optional per-kernel timing (lbm_set_timing): 3 events per step: before k_phi, between, after k_main
     bool timing;
     std::vector<cudaEvent_t> ev;

@@ -3,6 +3,7 @@
 
 #include "ctx.h"
 #include "k_main.cuh"
+#include "k_main_phitma.cuh"
 #include "k_main_tma.cuh"
 #include "k_phi.cuh"
 
@@ -62,6 +63,15 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
                 const long long ntiles = (long long)nxt * nyt * c->P.nz;
                 const unsigned grid = (unsigned)(ntiles < c->num_sms ? ntiles : c->num_sms);
                 kern<<<grid, C::NT, C::SMEM_BYTES, c->stream>>>(dev_params<real>(c), F, M, ntiles, nxt, nyt);
+                c->launches++;
+                CK(cudaGetLastError());
+                return LBM_OK;
+            }
+        }
+        if constexpr (MODE != MODE_INIT) {
+            if (c->phi_tma) {
+                k_main_phitma<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB>
+                    <<<grid_for<T>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F, c->map_phi_tile[pnew]);
                 c->launches++;
                 CK(cudaGetLastError());
                 return LBM_OK;
@@ -179,7 +189,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     }
 
     static const ImplOps *ops() {
-        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::read_macro, &Impl::read_pops};
+        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::read_macro, &Impl::read_pops, T::BX, T::BY, T::BZ};
         return &o;
     }
 };

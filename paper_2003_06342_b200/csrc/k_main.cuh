@@ -24,6 +24,7 @@ template <class LF, class LG, class LS, class real, bool BC> struct SrcGlobal {
         pcoff = ((unsigned)(g.z + P.pz) * (unsigned)P.ppy + (unsigned)(g.y + 1)) * (unsigned)P.ppx + (unsigned)(g.x + P.xpad);
         pc = Fd.phi_new + pcoff;
     }
+    __device__ __forceinline__ void phi_ready() const {}
     __device__ __forceinline__ real phi(int dx, int dy, int dz) const { return __ldg(pc + (dx + dy * P.ppx + dz * (int)P.pplane)); }
     __device__ __forceinline__ real phi_old() const { return __ldg(Fd.phi_old + pcoff); }
     __device__ __forceinline__ real pdot_old() const { return Fd.pdot[g.n]; }
@@ -47,6 +48,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
 
     // ---- H2: grad phi, lap phi by directional derivatives on the NS lattice (Eq.35a,b 36a,b; PAPER.md:291-315;
     //      the printed factor 3 is 1/e2, reading S2).  Opposite directions are paired: one difference, one sum.
+    src.phi_ready();   // TMA-staged phi tile: wait here, after the s loads have been issued
     const real phi = src.phi(0, 0, 0);
     real gx = real(0), gy = real(0), gz = real(0), lsum = real(0);
     static_for<LF::Q>([&](auto ic) {

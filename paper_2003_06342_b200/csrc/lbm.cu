@@ -179,6 +179,28 @@ bool encode_rows(CUtensorMap *m, void *base, int es, int rank, const unsigned lo
     return r == CUDA_SUCCESS;
 }
 
+// box tensor map of the padded phi buffers for the gather kernel's halo tile (k_main_phitma.cuh)
+bool build_phi_tile_maps(lbm_ctx *c) {
+    auto fn = get_encode_fn();
+    if (!fn) return false;
+    const int es = c->P.precision == 64 ? 8 : 4;
+    const int epb = 16 / es;
+    const bool three_d = c->P.nz > 1;
+    for (int b = 0; b < 2; ++b) {
+        cuuint64_t gdim[3] = {(cuuint64_t)c->L.ppx, (cuuint64_t)c->L.ppy, (cuuint64_t)c->L.ppz};
+        cuuint64_t gstr[2] = {(cuuint64_t)c->L.ppx * es, (cuuint64_t)c->L.ppx * c->L.ppy * es};
+        cuuint32_t box[3] = {(cuuint32_t)(c->ops->bx + 2 * epb), (cuuint32_t)(c->ops->by + 2),
+                             (cuuint32_t)(three_d ? c->ops->bz + 2 : 1)};
+        cuuint32_t estr[3] = {1, 1, 1};
+        if (box[0] > 256 || gstr[0] % 16 != 0) return false;
+        CUresult r = fn(&c->map_phi_tile[b], es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3,
+                        c->ws + c->L.off_phi[b], gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return false;
+    }
+    return true;
+}
+
 bool build_tma_maps(lbm_ctx *c) {
     const int es = c->P.precision == 64 ? 8 : 4;
     const int epb = 16 / es;
@@ -250,6 +272,8 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         // (90% of the measured HBM peak on config 4); LBM_VARIANT=tma selects the TMA-staged persistent kernel.
         const char *v = getenv("LBM_VARIANT");
         c->use_tma = (v && strcmp(v, "tma") == 0) && build_tma_maps(c);
+        const char *ph = getenv("LBM_PHI");   // phi halo tile of the gather kernel: "tma" (shared memory) or "ldg"
+        c->phi_tma = !c->use_tma && !(ph && strcmp(ph, "ldg") == 0) && build_phi_tile_maps(c);   // default: TMA
     }
     *out = c;
     return LBM_OK;
@@ -312,7 +336,7 @@ int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *ste
 
 long long lbm_step_count(const lbm_ctx *c) { return c ? c->nsteps : -1; }
 long long lbm_launch_count(const lbm_ctx *c) { return c ? c->launches : -1; }
-const char *lbm_variant(const lbm_ctx *c) { return c ? (c->use_tma ? "tma" : "direct") : ""; }
+const char *lbm_variant(const lbm_ctx *c) { return c ? (c->use_tma ? "tma" : (c->phi_tma ? "gather+phi-tma" : "direct")) : ""; }
 int lbm_last_cuda_error(void) { return g_last_cuda_error; }
 
 const char *lbm_strerror(int code) {

@@ -132,6 +132,25 @@ def test_minimal_grids(gpu, oracle_mod):
         _run_parity(gpu, oracle_mod, P, _random_state(P, 30), [1, 4], label="tiny %s" % (dims,))
 
 
+# ---------------------------------------------------------------------------- K_main variants
+def test_default_variant_stages_phi_by_tma_and_ldg_variant_agrees(gpu, oracle_mod, monkeypatch):
+    """Default K_main: gather kernel whose phi halo tile arrives by one TMA box per CTA; LBM_PHI=ldg reads phi through
+    L1 instead.  Both must match the oracle (the other tests in this file run the default)."""
+    P = wl.base_params(40, 10, 7, grav=[1e-4, 0.0, -2e-4])
+    sim = gpu.LBM(P, 64)
+    assert sim.variant == "gather+phi-tma"
+    sim.destroy()
+    monkeypatch.setenv("LBM_PHI", "ldg")
+    sim = gpu.LBM(P, 64)
+    assert sim.variant == "direct"
+    sim.destroy()
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 34), [1, 12], label="ldg 3d periodic")
+    P = wl.base_params(40, 20, 1, grav=[0.0, -1e-4, 0.0])
+    P["bc_f"][1] = ["wall", "wall"]; P["bc_g"][1] = ["zeroflux", "dirichlet"]; P["bc_s"][1] = ["dirichlet", "zeroflux"]
+    P["bc_phi"][1] = [0.0, 1.0]; P["bc_T"][1] = [0.7, 0.0]
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 35), [1, 12], label="ldg 2d walls")
+
+
 # ---------------------------------------------------------------------------- the TMA-staged variant of K_main
 def test_tma_variant(gpu, oracle_mod, monkeypatch):
     """LBM_VARIANT=tma: persistent kernel, inputs staged through shared memory by cp.async.bulk.tensor."""
