@@ -33,6 +33,10 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     // resident CTAs per SM the register allocation is bounded for (measured on config 4): fp64 2 x 256 threads at 128
     // registers; fp32 4 x 256 at 64 registers (+25% over 2 CTAs although a few values spill)
     static constexpr int MINB = sizeof(real) == 8 ? 2 : 4;
+#ifndef LBM_PHI_NPT
+#define LBM_PHI_NPT 2
+#endif
+    static constexpr int PHI_NPT = LBM_PHI_NPT;   // nodes per thread in K_phi
 
     static DevFields<real> fields(const lbm_ctx *c, int in, int out, int phi_new, int phi_old) {
         DevFields<real> F{};
@@ -126,7 +130,9 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
                 for (auto &e : e3) CK(cudaEventCreate(&e));
                 CK(cudaEventRecord(e3[0], c->stream));
             }
-            k_phi<LG, real, T::BX, T::BY, T::BZ><<<grid_for<T>(c->P), NT, 0, c->stream>>>(
+            dim3 gphi = grid_for<T>(c->P);
+            if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
+            k_phi<LG, real, T::BX, T::BY, T::BZ, PHI_NPT><<<gphi, NT, 0, c->stream>>>(
                 P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot), wsp<real>(c, c->L.off_phi[pnew]));
             c->launches++;
             CK(cudaGetLastError());

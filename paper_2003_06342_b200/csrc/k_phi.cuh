@@ -50,22 +50,43 @@ __device__ __forceinline__ void store_phi_with_images(real *__restrict__ phi_pad
             }
 }
 
-template <class LG, class real, int BX, int BY, int BZ>
+// Each thread handles NPT nodes, NPT tiles apart along the slowest tiled axis (z in 3D, y in 2D); all 8 NPT loads are
+// issued before the first sum, which is what a latency-bound streaming kernel needs (measured: DESIGN.md "Kernels").
+template <class LG, class real, int BX, int BY, int BZ, int NPT>
 __global__ void __launch_bounds__(BX *BY *BZ)
 k_phi(const DevParams<real> P, const real *__restrict__ g_in, const real *__restrict__ pdot, real *__restrict__ phi_new) {
+    constexpr bool ALONG_Z = LG::D == 3;
     const int t = threadIdx.x;
-    const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY, z0 = blockIdx.z * BZ;
-    const int x = x0 + t % BX, y = y0 + (t / BX) % BY, z = z0 + t / (BX * BY);
-    if (x >= P.nx || y >= P.ny || z >= P.nz) return;
-    const NodeGeom g = make_geom(P, x, y, z);
-    real gi[LG::Q];
-    if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) pull<LG, real, true>(g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi, gi);
-    else pull<LG, real, false>(g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi, gi);
-    real sum = gi[0];
+    const int x0 = blockIdx.x * BX;
+    const int y0 = blockIdx.y * BY * (ALONG_Z ? 1 : NPT);
+    const int z0 = blockIdx.z * BZ * (ALONG_Z ? NPT : 1);
+    const int x = x0 + t % BX, yb = y0 + (t / BX) % BY, zb = z0 + t / (BX * BY);
+    if (x >= P.nx) return;
+    const bool bc = tile_touches_bc(P, x0, y0, z0, BX, BY * (ALONG_Z ? 1 : NPT), BZ * (ALONG_Z ? NPT : 1));
+    real gi[NPT][LG::Q];
+    real pd[NPT];
+    NodeGeom g[NPT];
+    bool ok[NPT];
 #pragma unroll
-    for (int i = 1; i < LG::Q; ++i) sum += gi[i];
-    const real phi = sum + P.hdt * __ldg(pdot + g.n);   // sum_i w_i = 1
-    store_phi_with_images(phi_new, P, g, phi);
+    for (int j = 0; j < NPT; ++j) {
+        const int y = yb + (ALONG_Z ? 0 : j * BY), z = zb + (ALONG_Z ? j * BZ : 0);
+        ok[j] = y < P.ny && z < P.nz;
+        if (ok[j]) {
+            g[j] = make_geom(P, x, y, z);
+            if (bc) pull<LG, real, true>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
+            else pull<LG, real, false>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
+            pd[j] = __ldg(pdot + g[j].n);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < NPT; ++j) {
+        if (ok[j]) {
+            real sum = gi[j][0];
+#pragma unroll
+            for (int i = 1; i < LG::Q; ++i) sum += gi[j][i];
+            store_phi_with_images(phi_new, P, g[j], sum + P.hdt * pd[j]);   // sum_i w_i = 1
+        }
+    }
 }
 
 // Initialisation helper: copy a plain [z][y][x] phi into both padded buffers with ghost images.
