@@ -91,6 +91,7 @@ typedef struct lbm_params {
     double nu_l, nu_g;      /* kinematic viscosities, harmonic interpolation Eq.(1b)                */
     double sigma, W, M;     /* surface tension, interface width, mobility (Eq.15b, 5)               */
     double grav[3];         /* gravity acceleration g; F_v = (rho - rho_l) g (reading G6) */
+    double force[3];        /* uniform body force density added to F_tot             */
     double alpha_l, alpha_g;/* thermal diffusivities, linear in phi (reading S6)          */
     double L_latent, Cp;    /* latent heat and specific heat; theta = Cp (T - T_sat)/L              */
     double T_sat, theta_I;  /* saturation temperature; dimensionless interface temperature          */

@@ -40,7 +40,7 @@ class _Params(C.Structure):
         ("dx", C.c_double), ("dt", C.c_double),
         ("rho_l", C.c_double), ("rho_g", C.c_double), ("nu_l", C.c_double), ("nu_g", C.c_double),
         ("sigma", C.c_double), ("W", C.c_double), ("M", C.c_double),
-        ("grav", C.c_double * 3),
+        ("grav", C.c_double * 3), ("force", C.c_double * 3),
         ("alpha_l", C.c_double), ("alpha_g", C.c_double),
         ("L_latent", C.c_double), ("Cp", C.c_double), ("T_sat", C.c_double), ("theta_I", C.c_double),
         ("A", C.c_double), ("eps_n", C.c_double),
@@ -102,6 +102,7 @@ def fill_params(P: dict) -> _Params:
         setattr(s, k, float(P[k]))
     for a in range(3):
         s.grav[a] = float(P["grav"][a])
+        s.force[a] = float(P.get("force", (0.0, 0.0, 0.0))[a])
     s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0)
     return s
 

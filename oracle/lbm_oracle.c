@@ -284,13 +284,15 @@ static double production_rate(const oracle_ctx *c, double phi, double T)
 /* Total force of Eq.(12) at one node from phi, grad phi, lap phi.
  * F_s = mu_phi grad phi, Eq.(13),(14) PAPER.md:114-118.
  * F_v = (rho - rho_l) g : buoyancy relative to the liquid, zero in pure liquid, pushes gas against g
- * (reading G6 of the printed F_v = (rho_l - rho) g). */
+ * (reading G6 of the printed F_v = (rho_l - rho) g).
+ * A uniform body force (the paper replaces the pressure gradient of the Poiseuille tests by F = (G,0,0),
+ * PAPER.md:418) is added to F_tot. */
 static void total_force(const oracle_ctx *c, double phi, const double grad[3], double lap, double rho,
                         double F[3])
 {
     const oracle_params *P = &c->P;
     double mu = 4.0 * c->H * phi * (phi - 1.0) * (phi - 0.5) - c->K * lap;
-    for (int a = 0; a < 3; ++a) F[a] = mu * grad[a] + (rho - P->rho_l) * P->grav[a];
+    for (int a = 0; a < 3; ++a) F[a] = mu * grad[a] + (rho - P->rho_l) * P->grav[a] + P->force[a];
 }
 
 /* P2 -- equilibria and sources of the three lattices at one node, from the level-n macros.

@@ -52,6 +52,7 @@ typedef struct oracle_params {
     double rho_l, rho_g, nu_l, nu_g;
     double sigma, W, M;           /* surface tension, interface width, mobility                  */
     double grav[3];               /* gravity acceleration vector g (points "down")               */
+    double force[3];              /* uniform body force density added to F_tot    */
     double alpha_l, alpha_g;      /* thermal diffusivities                                       */
     double L_latent, Cp, T_sat, theta_I;
     double A;                     /* script-A of Eq.(18); 10/48 in the paper      */

@@ -39,7 +39,7 @@ class lbm_params(C.Structure):
         ("dx", C.c_double), ("dt", C.c_double),
         ("rho_l", C.c_double), ("rho_g", C.c_double), ("nu_l", C.c_double), ("nu_g", C.c_double),
         ("sigma", C.c_double), ("W", C.c_double), ("M", C.c_double),
-        ("grav", C.c_double * 3),
+        ("grav", C.c_double * 3), ("force", C.c_double * 3),
         ("alpha_l", C.c_double), ("alpha_g", C.c_double),
         ("L_latent", C.c_double), ("Cp", C.c_double), ("T_sat", C.c_double), ("theta_I", C.c_double),
         ("A", C.c_double), ("eps_n", C.c_double),
@@ -99,6 +99,7 @@ def make_params(P: dict, precision: int = 64) -> lbm_params:
             s.bc_T[a][side] = float(P["bc_T"][a][side])
             s.bc_p[a][side] = float(P["bc_p"][a][side])
         s.grav[a] = float(P["grav"][a])
+        s.force[a] = float(P.get("force", (0.0, 0.0, 0.0))[a])
     for k in ("dx", "dt", "rho_l", "rho_g", "nu_l", "nu_g", "sigma", "W", "M", "alpha_l", "alpha_g",
               "L_latent", "Cp", "T_sat", "theta_I", "A", "eps_n"):
         setattr(s, k, float(P[k]))

@@ -27,7 +27,7 @@ struct Layout {
     long long N;
     int ppx, ppy, ppz, pz, xpad;
     size_t phi_pad_elems;
-    size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot, off_u, off_p, off_T, off_scratch, total;
+    size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot[2], off_u, off_p, off_T, off_scratch, total;
 };
 
 // One implementation = one (lattice set, precision, tile shape); chosen once in lbm_create.
@@ -68,6 +68,8 @@ struct lbm_ctx {
     CUtensorMap map_f[2], map_g[2], map_s[2], map_phi[2], map_pdot;
     // gather kernel with the phi halo tile staged by TMA: one box per CTA
     bool phi_tma;
+    // fused variant: K_phi folded into K_main (3D only), Pdot double-buffered
+    bool fused;
     CUtensorMap map_phi_tile[2];
     // optional per-kernel timing (lbm_set_timing): 3 events per step: before k_phi, between, after k_main
     bool timing;

@@ -3,6 +3,7 @@
 
 #include "ctx.h"
 #include "k_main.cuh"
+#include "k_main_fused.cuh"
 #include "k_main_phitma.cuh"
 #include "k_main_tma.cuh"
 #include "k_phi.cuh"
@@ -45,7 +46,8 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         F.s_in = wsp<real>(c, c->L.off_s[in]);  F.s_out = wsp<real>(c, c->L.off_s[out]);
         F.phi_new = wsp<real>(c, c->L.off_phi[phi_new]);
         F.phi_old = wsp<real>(c, c->L.off_phi[phi_old]);
-        F.pdot = wsp<real>(c, c->L.off_pdot);
+        F.pdot = wsp<real>(c, c->L.off_pdot[0]);
+        F.pdot_in = F.pdot;
         F.u = wsp<real>(c, c->L.off_u); F.p = wsp<real>(c, c->L.off_p); F.T = wsp<real>(c, c->L.off_T);
         return F;
     }
@@ -120,6 +122,29 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         return LBM_OK;
     }
 
+    // fused variant (3D): one kernel per step, see k_main_fused.cuh
+#ifndef LBM_FBX
+#define LBM_FBX 64
+#define LBM_FBY 4
+#define LBM_FLZ 32
+#endif
+    struct FusedCfg { static constexpr int BX = LBM_FBX, BY = LBM_FBY, LZ = LBM_FLZ; };
+    template <int MODE> static int launch_fused(lbm_ctx *c, DevFields<real> F, int in, int pnew) {
+        if constexpr (D == 3) {
+            F.pdot_in = wsp<real>(c, c->L.off_pdot[in]);
+            F.pdot = wsp<real>(c, c->L.off_pdot[1 - in]);
+            const dim3 grid((c->P.nx + FusedCfg::BX - 1) / FusedCfg::BX, (c->P.ny + FusedCfg::BY - 1) / FusedCfg::BY,
+                            (c->P.nz + FusedCfg::LZ - 1) / FusedCfg::LZ);
+            k_main_fused<LF, LG, LS, real, MODE, FusedCfg::BX, FusedCfg::BY, FusedCfg::LZ, MINB>
+                <<<grid, FusedCfg::BX * FusedCfg::BY, 0, c->stream>>>(dev_params<real>(c), F, wsp<real>(c, c->L.off_phi[pnew]));
+            c->launches++;
+            CK(cudaGetLastError());
+            return LBM_OK;
+        } else {
+            return LBM_E_UNSUPPORTED;
+        }
+    }
+
     static int step(lbm_ctx *c, int n) {
         const DevParams<real> &P = dev_params<real>(c);
         for (int k = 0; k < n; ++k) {
@@ -130,15 +155,21 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
                 for (auto &e : e3) CK(cudaEventCreate(&e));
                 CK(cudaEventRecord(e3[0], c->stream));
             }
-            dim3 gphi = grid_for<T>(c->P);
-            if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
-            k_phi<LG, real, T::BX, T::BY, T::BZ, PHI_NPT><<<gphi, NT, 0, c->stream>>>(
-                P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot), wsp<real>(c, c->L.off_phi[pnew]));
-            c->launches++;
-            CK(cudaGetLastError());
-            if (timed) CK(cudaEventRecord(e3[1], c->stream));
             DevFields<real> F = fields(c, in, out, pnew, pold);
-            int rc = (k == n - 1) ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
+            int rc;
+            if (c->fused) {
+                if (timed) CK(cudaEventRecord(e3[1], c->stream));
+                rc = (k == n - 1) ? launch_fused<MODE_STEP_MACRO>(c, F, in, pnew) : launch_fused<MODE_STEP>(c, F, in, pnew);
+            } else {
+                dim3 gphi = grid_for<T>(c->P);
+                if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
+                k_phi<LG, real, T::BX, T::BY, T::BZ, PHI_NPT><<<gphi, NT, 0, c->stream>>>(
+                    P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot[0]), wsp<real>(c, c->L.off_phi[pnew]));
+                c->launches++;
+                CK(cudaGetLastError());
+                if (timed) CK(cudaEventRecord(e3[1], c->stream));
+                rc = (k == n - 1) ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
+            }
             if (rc) return rc;
             if (timed) {
                 CK(cudaEventRecord(e3[2], c->stream));

@@ -27,7 +27,7 @@ template <class LF, class LG, class LS, class real, bool BC> struct SrcGlobal {
     __device__ __forceinline__ void phi_ready() const {}
     __device__ __forceinline__ real phi(int dx, int dy, int dz) const { return __ldg(pc + (dx + dy * P.ppx + dz * (int)P.pplane)); }
     __device__ __forceinline__ real phi_old() const { return __ldg(Fd.phi_old + pcoff); }
-    __device__ __forceinline__ real pdot_old() const { return Fd.pdot[g.n]; }
+    __device__ __forceinline__ real pdot_old() const { return Fd.pdot_in[g.n]; }
     // AGAIN = true: second read of a value already read for the moments (see ld_again)
     template <int I, bool AGAIN = false> __device__ __forceinline__ real f() const { return pull_one<LF, I, real, BC, AGAIN>(Fd.f_in, (unsigned)P.N, g, P.bc_f, P.bc_p); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real s() const { return pull_one<LS, I, real, BC, AGAIN>(Fd.s_in, (unsigned)P.N, g, P.bc_s, P.bc_T); }
@@ -74,9 +74,9 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
     const real rho = P.rho_l + phi * P.rho_diff;                               // Eq.(1a)
     const real mu = P.fourH * phi * (phi - real(1)) * (phi - real(0.5)) - P.K * lap;   // Eq.(14)
     const real bu = rho - P.rho_l;                                             // buoyancy factor, reading G6
-    const real Fx = mu * gx + bu * P.grav[0];                                  // Eq.(12),(13) PAPER.md:106-114
-    const real Fy = mu * gy + bu * P.grav[1];
-    const real Fz = mu * gz + bu * P.grav[2];
+    const real Fx = mu * gx + bu * P.grav[0] + P.force[0];                     // Eq.(12),(13) PAPER.md:106-114; body force PAPER.md:418
+    const real Fy = mu * gy + bu * P.grav[1] + P.force[1];
+    const real Fz = mu * gz + bu * P.grav[2] + P.force[2];
     const real grx = P.rho_diff * gx, gry = P.rho_diff * gy, grz = P.rho_diff * gz;   // grad rho
     const real alpha = P.alpha_l + phi * P.alpha_diff;                         // reading S6
     // relaxation rates: tau_bar = nu/(cs2 dt) with harmonic nu (Eq.1b); alpha/(cs2 dt);

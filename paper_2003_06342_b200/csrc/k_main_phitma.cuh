@@ -34,7 +34,7 @@ template <class LF, class LG, class LS, class real, bool BC, class TC> struct Sr
     __device__ __forceinline__ void phi_ready() const { mbar_wait(bar, 0); }
     __device__ __forceinline__ real phi(int dx, int dy, int dz) const { return tile[dx + dy * TC::BOXX + dz * (TC::BOXX * TC::BOXY)]; }
     __device__ __forceinline__ real phi_old() const { return __ldg(Fd.phi_old + pcoff); }
-    __device__ __forceinline__ real pdot_old() const { return Fd.pdot[g.n]; }
+    __device__ __forceinline__ real pdot_old() const { return Fd.pdot_in[g.n]; }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real f() const { return pull_one<LF, I, real, BC, AGAIN>(Fd.f_in, (unsigned)P.N, g, P.bc_f, P.bc_p); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real s() const { return pull_one<LS, I, real, BC, AGAIN>(Fd.s_in, (unsigned)P.N, g, P.bc_s, P.bc_T); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real gg() const { return pull_one<LG, I, real, BC, AGAIN>(Fd.g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi); }

@@ -60,7 +60,7 @@ template <class real> struct DevParams {
     real rho_l, rho_g, rho_diff, drho;   // rho_g - rho_l ; 1/rho_g - 1/rho_l
     real nu_l, nu_g, nu_prod;            // nu_l * nu_g
     real fourH, K;                       // Eq.(14),(15b)
-    real grav[3];
+    real grav[3], force[3];
     real alpha_l, alpha_diff;            // alpha_g - alpha_l
     real M, om_g, cac;                   // mobility, 1/(M/(cs2g dt)+1/2), M*(4/W)/cs2g * c
     real LCp, CpL, T_sat, theta_I, pc_coef;   // L/Cp, Cp/L, 4/(A W^2)
@@ -73,7 +73,8 @@ template <class real> struct DevFields {
     real *f_out, *g_out, *s_out;      // post-collision populations of this level
     const real *phi_new;              // padded, level n+1 (written by k_phi)
     const real *phi_old;              // padded, level n
-    real *pdot;                       // production field: read (stored, level n), then overwritten (level n+1)
+    const real *pdot_in;              // production field of level n (the stored one, reading S3)
+    real *pdot;                       // production field of level n+1 (same array as pdot_in except in the fused variant)
     real *u, *p, *T;                  // macro arrays: outputs (MODE_STEP_MACRO) or inputs (MODE_INIT)
 };
 

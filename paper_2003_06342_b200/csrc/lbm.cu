@@ -83,7 +83,7 @@ Layout make_layout(const lbm_params *p) {
     for (int b = 0; b < 2; ++b) L.off_g[b] = take(N * lattice_q(p->lat_g));
     for (int b = 0; b < 2; ++b) L.off_s[b] = take(N * lattice_q(p->lat_s));
     for (int b = 0; b < 2; ++b) L.off_phi[b] = take(L.phi_pad_elems);
-    L.off_pdot = take(N);
+    for (int b = 0; b < 2; ++b) L.off_pdot[b] = take(N);   // second buffer: fused variant only
     L.off_u = take(3 * N);
     L.off_p = take(N);
     L.off_T = take(N);
@@ -107,6 +107,7 @@ template <class real> DevParams<real> make_dev_params(const lbm_params *p, const
         }
         d.nonper[a] = p->bc_f[a][0] != LBM_F_PERIODIC;
         d.grav[a] = (real)p->grav[a];
+        d.force[a] = (real)p->force[a];
     }
     if (p->nz == 1) d.nonper[2] = 0;
     const double c = p->dx / p->dt;
@@ -219,7 +220,7 @@ bool build_tma_maps(lbm_ctx *c) {
         ok = ok && encode_rows(&c->map_phi[b], c->ws + c->L.off_phi[b], es, 3, dp, boxx);
     }
     const unsigned long long dd[3] = {nx, ny, nz};
-    ok = ok && encode_rows(&c->map_pdot, c->ws + c->L.off_pdot, es, 3, dd, boxx);
+    ok = ok && encode_rows(&c->map_pdot, c->ws + c->L.off_pdot[0], es, 3, dd, boxx);
     return ok;
 }
 
@@ -272,8 +273,9 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         // (90% of the measured HBM peak on config 4); LBM_VARIANT=tma selects the TMA-staged persistent kernel.
         const char *v = getenv("LBM_VARIANT");
         c->use_tma = (v && strcmp(v, "tma") == 0) && build_tma_maps(c);
+        c->fused = (v && strcmp(v, "fused") == 0) && p->nz > 1;
         const char *ph = getenv("LBM_PHI");   // phi halo tile of the gather kernel: "tma" (shared memory) or "ldg"
-        c->phi_tma = !c->use_tma && !(ph && strcmp(ph, "ldg") == 0) && build_phi_tile_maps(c);   // default: TMA
+        c->phi_tma = !c->use_tma && !c->fused && !(ph && strcmp(ph, "ldg") == 0) && build_phi_tile_maps(c);   // default: TMA
     }
     *out = c;
     return LBM_OK;
@@ -336,7 +338,7 @@ int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *ste
 
 long long lbm_step_count(const lbm_ctx *c) { return c ? c->nsteps : -1; }
 long long lbm_launch_count(const lbm_ctx *c) { return c ? c->launches : -1; }
-const char *lbm_variant(const lbm_ctx *c) { return c ? (c->use_tma ? "tma" : (c->phi_tma ? "gather+phi-tma" : "direct")) : ""; }
+const char *lbm_variant(const lbm_ctx *c) { return c ? (c->fused ? "fused" : c->use_tma ? "tma" : (c->phi_tma ? "gather+phi-tma" : "direct")) : ""; }
 int lbm_last_cuda_error(void) { return g_last_cuda_error; }
 
 const char *lbm_strerror(int code) {

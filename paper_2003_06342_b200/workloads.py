@@ -42,6 +42,7 @@ def base_params(nx, ny, nz=1, **over):
         rho_l=10.0, rho_g=1.0, nu_l=0.1, nu_g=0.1,
         sigma=1e-3, W=4.0, M=0.02,
         grav=[0.0, 0.0, 0.0],
+        force=[0.0, 0.0, 0.0],
         alpha_l=0.02, alpha_g=0.05,
         L_latent=1.0, Cp=0.1, T_sat=0.0, theta_I=0.0,
         A=10.0 / 48.0, eps_n=1e-5,

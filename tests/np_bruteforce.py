@@ -96,7 +96,8 @@ class NPModel:
         rho = phi * P["rho_g"] + (1 - phi) * P["rho_l"]
         mu = 4 * self.H * phi * (phi - 1) * (phi - 0.5) - self.K * lap                          # Eq.(14)
         g = np.array(P["grav"]).reshape(3, 1, 1, 1)
-        F = mu * grad + (rho - P["rho_l"]) * g                                                   # Eq.(12),(13), G6
+        fb = np.array(P.get("force", (0.0, 0.0, 0.0))).reshape(3, 1, 1, 1)
+        F = mu * grad + (rho - P["rho_l"]) * g + fb                                              # Eq.(12),(13), G6
         grho = (P["rho_g"] - P["rho_l"]) * grad
         return rho, F, grho
 

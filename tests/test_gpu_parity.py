@@ -151,6 +151,27 @@ def test_default_variant_stages_phi_by_tma_and_ldg_variant_agrees(gpu, oracle_mo
     _run_parity(gpu, oracle_mod, P, _random_state(P, 35), [1, 12], label="ldg 2d walls")
 
 
+def test_fused_variant(gpu, oracle_mod, monkeypatch):
+    """LBM_VARIANT=fused (3D): K_phi folded into K_main, phi planes with halo recomputed per CTA from g*."""
+    monkeypatch.setenv("LBM_VARIANT", "fused")
+    P = wl.base_params(70, 10, 37, grav=[1e-4, 0.0, -2e-4])      # ragged in x, y and in the z segments of 32
+    sim = gpu.LBM(P, 64)
+    assert sim.variant == "fused"
+    sim.destroy()
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 36), [1, 2, 12], label="fused 3d periodic")
+    P = wl.base_params(34, 9, 12, grav=[0.0, 0.0, -1e-4])        # z walls, Dirichlet T
+    P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
+    P["bc_T"][2] = [1.0, 0.0]
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 37), [1, 12], label="fused 3d z walls")
+    P = wl.base_params(12, 9, 8)                                 # walls on all axes, Dirichlet phi on the low faces
+    for a in range(3):
+        P["bc_f"][a] = ["wall", "wall"]; P["bc_g"][a] = ["dirichlet", "zeroflux"]; P["bc_s"][a] = ["dirichlet", "zeroflux"]
+        P["bc_phi"][a] = [0.9, 0.0]; P["bc_T"][a] = [0.2, 0.0]
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 38), [1, 3], label="fused 3d box")
+    Pc, I = wl.config4_film3d(nx=48, ny=40, nz=64, h0=12.0, amp=2.0)
+    _run_parity(gpu, oracle_mod, Pc, (I["phi"], I["T"]), [1, 50], pops=False, label="fused config4 48x40x64")
+
+
 # ---------------------------------------------------------------------------- the TMA-staged variant of K_main
 def test_tma_variant(gpu, oracle_mod, monkeypatch):
     """LBM_VARIANT=tma: persistent kernel, inputs staged through shared memory by cp.async.bulk.tensor."""

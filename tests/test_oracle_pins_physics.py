@@ -206,3 +206,34 @@ def test_gas_bubble_rises(oracle_mod):
     ph, u, _, _ = o.read_macro()
     assert (u[1] * ph).sum() / ph.sum() > 1e-3
     o.close()
+
+
+def test_layered_poiseuille_viscosity_contrast(oracle_mod):
+    """P7: two-layer Poiseuille flow, Eq.(37): fluid A (phi = 0, nu_l) below, fluid B above, equal
+    densities, driven by the uniform force F = (G, 0, 0) that replaces the pressure gradient,
+    G = u_c (eta_A + eta_B)/h^2.  Pins the harmonic viscosity interpolation Eq.(1b) and tau_f(phi).
+    Reading G9: the closed form used is the one derived from eta u'' = -G with u(+-h) = 0 and continuous u and
+    shear at y = 0, whose linear term is +(y/h)(eta_A - eta_B)/(eta_A + eta_B); Eq.(37) as printed (minus sign with
+    A on -h <= y <= 0) violates its own no-slip condition at y = -h."""
+    ny, W, nuA, nuB, uc = 100, 6.0, 0.1, 0.3, 5e-5
+    h = ny / 2.0
+    etaA, etaB = nuA, nuB
+    G = uc * (etaA + etaB) / h ** 2
+    P = wl.base_params(4, ny, 1, rho_l=1.0, rho_g=1.0, nu_l=nuA, nu_g=nuB, sigma=0.0, W=W, M=0.1, force=[G, 0, 0],
+                       phase_change=False, latent_heat=False)
+    P["bc_f"][1] = ["wall", "wall"]; P["bc_g"][1] = ["zeroflux", "zeroflux"]; P["bc_s"][1] = ["zeroflux", "zeroflux"]
+    y = np.arange(ny) + 0.5 - h
+    phi = np.tile((0.5 * (1 + np.tanh(2 * y / W)))[None, :, None], (1, 1, 4))
+    o = oracle_mod.Oracle(P)
+    o.init(phi)
+    o.step(50000)
+    ux = o.read_macro()[1][0][0, :, 0]
+    o.close()
+    yy = y / h
+    lin = yy * (etaA - etaB) / (etaA + etaB)
+    exact = np.where(y < 0, G * h * h / (2 * etaA) * (-yy ** 2 + lin + 2 * etaA / (etaA + etaB)),
+                     G * h * h / (2 * etaB) * (-yy ** 2 + lin + 2 * etaB / (etaA + etaB)))
+    assert np.abs(ux - exact).max() / exact.max() < 0.02
+    printed = np.where(y < 0, G * h * h / (2 * etaA) * (-yy ** 2 - lin + 2 * etaA / (etaA + etaB)),
+                       G * h * h / (2 * etaB) * (-yy ** 2 - lin + 2 * etaB / (etaA + etaB)))
+    assert abs(printed[0]) > 0.3 * exact.max()          # the printed branch labels do not even vanish at the wall
