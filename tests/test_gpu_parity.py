@@ -60,7 +60,7 @@ def _run_parity(gpu, oracle_mod, P, init, horizons, tol=TOL64, pops=True, label=
 
 # ---------------------------------------------------------------------------- generic small cases, all BC kinds
 def test_2d_periodic_ragged(gpu, oracle_mod):
-    P = wl.base_params(40, 28, 1, grav=[1e-4, -2e-4, 0.0])        # 2 x-tiles with a ragged tail, 4 y-tiles
+    P = wl.base_params(40, 28, 1, grav=[1e-4, -2e-4, 0.0], nu_l=0.05, nu_g=0.2, force=[2e-5, 1e-5, 0.0])   # ragged tiles
     _run_parity(gpu, oracle_mod, P, _random_state(P, 21), [1, 2, 20], label="2d periodic")
 
 
@@ -102,8 +102,10 @@ def test_2d_two_nonperiodic_axes(gpu, oracle_mod):
 
 
 def test_3d_periodic_ragged(gpu, oracle_mod):
-    P = wl.base_params(40, 10, 7, grav=[1e-4, 0.0, -2e-4])
+    P = wl.base_params(40, 10, 7, grav=[1e-4, 0.0, -2e-4], nu_l=0.2, nu_g=0.04, force=[0.0, 1e-5, -2e-5])
     _run_parity(gpu, oracle_mod, P, _random_state(P, 26), [1, 2, 15], label="3d periodic")
+    P = wl.base_params(264, 6, 5, nu_l=0.07, nu_g=0.35, alpha_l=0.04, alpha_g=0.01)     # wide tiles (nx >= 128), ragged
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 39), [1, 8], label="3d wide tiles")
 
 
 def test_3d_walls_z(gpu, oracle_mod):

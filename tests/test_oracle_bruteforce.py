@@ -50,7 +50,7 @@ def _compare(oracle_mod, P, steps, seed, TOL=TOL):
 
 
 def test_2d_periodic(oracle_mod):
-    P = wl.base_params(8, 8, 1, grav=[1e-4, -2e-4, 0.0])
+    P = wl.base_params(8, 8, 1, grav=[1e-4, -2e-4, 0.0], nu_l=0.05, nu_g=0.2, force=[2e-5, 1e-5, 0.0])
     _compare(oracle_mod, P, 12, 11)
 
 
@@ -94,7 +94,7 @@ def test_2d_two_nonperiodic_axes(oracle_mod):
 
 
 def test_3d_periodic(oracle_mod):
-    P = wl.base_params(8, 8, 8, grav=[1e-4, 0.0, -2e-4])
+    P = wl.base_params(8, 8, 8, grav=[1e-4, 0.0, -2e-4], nu_l=0.2, nu_g=0.04, force=[0.0, 1e-5, -2e-5])
     _compare(oracle_mod, P, 10, 16)
 
 
