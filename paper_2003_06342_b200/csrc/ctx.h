@@ -70,6 +70,10 @@ struct lbm_ctx {
     bool phi_tma;
     // fused variant: K_phi folded into K_main (3D only), Pdot double-buffered
     bool fused;
+    // CUDA graph of two consecutive plain steps, for launch-bound (small) grids
+    bool graph_ok;
+    cudaGraphExec_t graph2;
+    int graph_launches;
     CUtensorMap map_phi_tile[2];
     // optional per-kernel timing (lbm_set_timing): 3 events per step: before k_phi, between, after k_main
     bool timing;

@@ -145,39 +145,68 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         }
     }
 
-    static int step(lbm_ctx *c, int n) {
+    // enqueue the kernels of ONE step and flip the buffers
+    static int step_once(lbm_ctx *c, bool macro, bool timed) {
         const DevParams<real> &P = dev_params<real>(c);
-        for (int k = 0; k < n; ++k) {
-            const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
-            const bool timed = c->timing && c->ev.size() < 3 * 4096;
-            cudaEvent_t e3[3] = {nullptr, nullptr, nullptr};
-            if (timed) {
-                for (auto &e : e3) CK(cudaEventCreate(&e));
-                CK(cudaEventRecord(e3[0], c->stream));
-            }
-            DevFields<real> F = fields(c, in, out, pnew, pold);
-            int rc;
-            if (c->fused) {
-                if (timed) CK(cudaEventRecord(e3[1], c->stream));
-                rc = (k == n - 1) ? launch_fused<MODE_STEP_MACRO>(c, F, in, pnew) : launch_fused<MODE_STEP>(c, F, in, pnew);
-            } else {
-                dim3 gphi = grid_for<T>(c->P);
-                if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
-                k_phi<LG, real, T::BX, T::BY, T::BZ, PHI_NPT><<<gphi, NT, 0, c->stream>>>(
-                    P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot[0]), wsp<real>(c, c->L.off_phi[pnew]));
-                c->launches++;
-                CK(cudaGetLastError());
-                if (timed) CK(cudaEventRecord(e3[1], c->stream));
-                rc = (k == n - 1) ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
-            }
-            if (rc) return rc;
-            if (timed) {
-                CK(cudaEventRecord(e3[2], c->stream));
-                for (auto e : e3) c->ev.push_back(e);
-            }
-            c->cur = out; c->curphi = pnew; c->nsteps++;
+        const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
+        cudaEvent_t e3[3] = {nullptr, nullptr, nullptr};
+        if (timed) {
+            for (auto &e : e3) CK(cudaEventCreate(&e));
+            CK(cudaEventRecord(e3[0], c->stream));
         }
+        DevFields<real> F = fields(c, in, out, pnew, pold);
+        int rc;
+        if (c->fused) {
+            if (timed) CK(cudaEventRecord(e3[1], c->stream));
+            rc = macro ? launch_fused<MODE_STEP_MACRO>(c, F, in, pnew) : launch_fused<MODE_STEP>(c, F, in, pnew);
+        } else {
+            dim3 gphi = grid_for<T>(c->P);
+            if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
+            k_phi<LG, real, T::BX, T::BY, T::BZ, PHI_NPT><<<gphi, NT, 0, c->stream>>>(
+                P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot[0]), wsp<real>(c, c->L.off_phi[pnew]));
+            c->launches++;
+            CK(cudaGetLastError());
+            if (timed) CK(cudaEventRecord(e3[1], c->stream));
+            rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
+        }
+        if (rc) return rc;
+        if (timed) {
+            CK(cudaEventRecord(e3[2], c->stream));
+            for (auto e : e3) c->ev.push_back(e);
+        }
+        c->cur = out; c->curphi = pnew; c->nsteps++;
         return LBM_OK;
+    }
+
+    // n steps; the last one also stores u, p, T.  On small (launch-bound) grids the plain steps are replayed from a CUDA
+    // graph of two consecutive steps (the buffers alternate with period 2), captured once per context.
+    static int step(lbm_ctx *c, int n) {
+        if (n <= 0) return LBM_OK;
+        int plain = n - 1;
+        if (c->graph_ok && !c->timing && plain >= 4) {
+            if (c->cur != 0) { int rc = step_once(c, false, false); if (rc) return rc; --plain; }
+            if (!c->graph2) {
+                const long long steps0 = c->nsteps, launches0 = c->launches;
+                CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+                int rc = step_once(c, false, false);
+                if (!rc) rc = step_once(c, false, false);
+                cudaGraph_t g = nullptr;
+                cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+                c->graph_launches = (int)(c->launches - launches0);
+                c->nsteps = steps0; c->launches = launches0;      // nothing ran: capture only records
+                if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+                CK(e);
+                e = cudaGraphInstantiate(&c->graph2, g, 0);
+                cudaGraphDestroy(g);
+                CK(e);
+            }
+            while (plain >= 2) {
+                CK(cudaGraphLaunch(c->graph2, c->stream));
+                plain -= 2; c->nsteps += 2; c->launches += c->graph_launches;
+            }
+        }
+        while (plain-- > 0) { int rc = step_once(c, false, c->timing && c->ev.size() < 3 * 4096); if (rc) return rc; }
+        return step_once(c, true, c->timing && c->ev.size() < 3 * 4096);
     }
 
     static int read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T) {

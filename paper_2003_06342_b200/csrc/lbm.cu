@@ -274,6 +274,9 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         const char *v = getenv("LBM_VARIANT");
         c->use_tma = (v && strcmp(v, "tma") == 0) && build_tma_maps(c);
         c->fused = (v && strcmp(v, "fused") == 0) && p->nz > 1;
+        const char *gr = getenv("LBM_GRAPH");   // "0" disables the CUDA-graph replay of small grids
+        c->graph_ok = c->stream != nullptr && L.N <= (1ll << 21) && !(gr && strcmp(gr, "0") == 0);
+        c->graph2 = nullptr; c->graph_launches = 0;
         const char *ph = getenv("LBM_PHI");   // phi halo tile of the gather kernel: "tma" (shared memory) or "ldg"
         c->phi_tma = !c->use_tma && !c->fused && !(ph && strcmp(ph, "ldg") == 0) && build_phi_tile_maps(c);   // default: TMA
     }
@@ -357,6 +360,7 @@ const char *lbm_strerror(int code) {
 void lbm_destroy(lbm_ctx *c) {
     if (!c) return;
     for (auto e : c->ev) cudaEventDestroy(e);
+    if (c->graph2) cudaGraphExecDestroy(c->graph2);
     delete c;
 }
 

@@ -153,6 +153,25 @@ def test_default_variant_stages_phi_by_tma_and_ldg_variant_agrees(gpu, oracle_mo
     _run_parity(gpu, oracle_mod, P, _random_state(P, 35), [1, 12], label="ldg 2d walls")
 
 
+def test_cuda_graph_replay_on_side_stream(gpu, oracle_mod):
+    """Small grids replay a captured two-step CUDA graph (needs a non-default stream): same bits as plain launches."""
+    import torch
+    P = wl.base_params(40, 28, 1, grav=[1e-4, -2e-4, 0.0], nu_l=0.05, nu_g=0.2)
+    init = _random_state(P, 40)
+    o = oracle_mod.Oracle(P); o.init(*init); o.step(23)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        sim = gpu.LBM(P, 64, stream=st)
+        sim.init(*init)
+        sim.step(3)          # leaves the buffers at odd parity: the replay must re-align first
+        n0 = sim.launch_count
+        sim.step(20)         # 19 plain steps: 1 aligning + 9 graph replays, then the macro step
+        assert sim.step_count == 23 and sim.launch_count - n0 == 40
+        _compare_state(gpu, sim, o, oracle_mod, TOL64, True, "graph replay")
+        sim.destroy()
+    o.close()
+
+
 def test_fused_variant(gpu, oracle_mod, monkeypatch):
     """LBM_VARIANT=fused (3D): K_phi folded into K_main, phi planes with halo recomputed per CTA from g*."""
     monkeypatch.setenv("LBM_VARIANT", "fused")
