@@ -13,6 +13,9 @@ namespace lbm {
 // tiles of nodes per CTA (one node per thread, 256 threads).  A warp is one x-row.  Wide tiles (long contiguous
 // x-runs: fewer partially used sectors on the x-shifted pulls) are 3.5% faster on config 4 and are used when the
 // row is long enough; narrow tiles keep small grids busy.
+// wide tiles only when the ragged last tile wastes at most 4% of the threads (192 = 128 + 64 would idle 25%)
+inline bool wide_tile_pays(int nx) { return nx >= 128 && ((nx + 127) / 128 * 128 - nx) * 25 <= nx; }
+
 struct TileWide3 { static constexpr int BX = 128, BY = 2, BZ = 1; };
 struct TileNarrow3 { static constexpr int BX = 32, BY = 4, BZ = 2; };
 struct TileWide2 { static constexpr int BX = 128, BY = 2, BZ = 1; };
