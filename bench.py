@@ -36,6 +36,10 @@ def make_workload(name: str, seed_offset: int = 0):
         return wl.config4_film3d(nx=128, ny=128, nz=128, seed=4 + seed_offset)
     if name == "config3":
         return wl.config3_film2d(seed=3 + seed_offset)
+    if name.startswith("config3_"):   # e.g. config3_1024x1024, config3_4096x3072: the paper's film-boiling grids
+        nx, ny = (int(v) for v in name.split("_")[1].split("x"))
+        over = {"lat_s": "D2Q9"} if name.endswith("_q9") else {}   # _q9: three D2Q9 lattices as in the paper
+        return wl.config3_film2d(nx=nx, ny=ny, seed=3 + seed_offset, **over)
     if name.startswith("config5_"):
         return wl.config5_droplets(n=int(name.split("_")[1]), seed=5 + seed_offset)
     if name == "config1":

@@ -280,6 +280,91 @@ def test_config4_full_size_periodic_replica(gpu, oracle_mod):
         assert err <= TOL64, (name, err)
 
 
+def test_config5_full_size_384_periodic_replica(gpu, oracle_mod):
+    """Largest BASELINE.json grid (config 5, 384^3, 34 GB of state): a 96^3 droplet field replicated 4x4x4 times in the
+    periodic box must evolve as the replicated 96^3 solution, which the oracle computes; all 56.6 M outputs compared."""
+    Ps, Is = wl.config5_droplets(n=96, nspheres=12, rmin=6.0, rmax=14.0)
+    P = dict(Ps, nx=384, ny=384, nz=384)
+    phi = np.tile(Is["phi"], (4, 4, 4))
+    T = np.tile(Is["T"], (4, 4, 4))
+    steps = 4
+    sim = gpu.LBM(P, 64)
+    sim.init(phi, T)
+    del phi, T
+    sim.step(steps)
+    got = sim.read_macro()
+    sim.destroy()
+    o = oracle_mod.Oracle(Ps)
+    o.init(Is["phi"], Is["T"])
+    o.step(steps)
+    ref = o.read_macro()
+    o.close()
+    for a, r, name in zip(got, ref, ("phi", "u", "p", "T")):
+        reps = (1, 4, 4, 4) if a.ndim == 4 else (4, 4, 4)
+        err = float(np.abs(a - np.tile(r, reps)).max())
+        assert err <= TOL64, (name, err)
+
+
+def test_config3_full_size_periodic_replica(gpu, oracle_mod):
+    """Config 3 at full size (512 x 1024, 2D film boiling): 128-periodic pattern in x replicated 4 times."""
+    Ps, Is = wl.config3_film2d(nx=128, ny=1024, h0=64.0, amp=4.0)
+    P = dict(Ps, nx=512)
+    phi = np.tile(Is["phi"], (1, 1, 4)); T = np.tile(Is["T"], (1, 1, 4))
+    sim = gpu.LBM(P, 64); sim.init(phi, T); sim.step(50)
+    got = sim.read_macro(); sim.destroy()
+    o = oracle_mod.Oracle(Ps); o.init(Is["phi"], Is["T"]); o.step(50)
+    ref = o.read_macro(); o.close()
+    for a, r, name in zip(got, ref, ("phi", "u", "p", "T")):
+        reps = (1, 1, 1, 4) if a.ndim == 4 else (1, 1, 4)
+        assert float(np.abs(a - np.tile(r, reps)).max()) <= TOL64, name
+
+
+# ---------------------------------------------------------------------------- API behaviour
+def test_api_states_and_degenerate_calls(gpu, oracle_mod):
+    import ctypes as C
+    P = wl.base_params(40, 10, 7)
+    init = _random_state(P, 41)
+    sim = gpu.LBM(P, 64)
+    L = gpu.load_library()
+    assert L.lbm_step(sim._h, 1) == -5                      # LBM_E_STATE: step before init
+    assert L.lbm_read_macro(sim._h, None, None, None, None) == -5
+    with pytest.raises(ValueError):
+        sim.init(init[0][:, :, :-1])                         # wrong shape is refused by the binding
+    sim.init(init[0])                                        # T, u, p omitted: T = T_sat, u = 0, p = 0
+    o = oracle_mod.Oracle(P); o.init(init[0])
+    with pytest.raises(gpu.LBMError):
+        sim.read_pops(0, gpu.STAGE_STREAMED)                 # no streamed populations at level 0
+    sim.step(0)                                              # no-op
+    assert sim.step_count == 0
+    assert L.lbm_step(sim._h, -1) == -1
+    sim.step(3); o.step(3)
+    _compare_state(gpu, sim, o, oracle_mod, TOL64, True, "defaults")
+    phi_only = (np.empty(sim.shape), None, None, None)       # any output pointer may be NULL
+    ptr = C.c_void_p(phi_only[0].ctypes.data)
+    assert L.lbm_read_macro(sim._h, ptr, None, None, None) == 0
+    assert np.abs(phi_only[0] - o.read_macro()[0]).max() <= TOL64
+    sim.init(*init); o.init(*init)                           # re-initialisation resets the step counter and the state
+    assert sim.step_count == 0
+    sim.step(2); o.step(2)
+    _compare_state(gpu, sim, o, oracle_mod, TOL64, True, "re-init")
+    sim.destroy(); sim.destroy(); o.close()                  # destroy is idempotent
+
+
+def test_fp32_populations_and_defaults(gpu, oracle_mod):
+    P = wl.base_params(33, 17, 1, lat_s="D2Q9")
+    init = _random_state(P, 42)
+    sim = gpu.LBM(P, 32)
+    sim.init(*[a.astype(np.float32) for a in init])
+    o = oracle_mod.Oracle(P); o.init(*init)
+    sim.step(5); o.step(5)
+    for which in range(3):
+        a = sim.read_pops(which, gpu.STAGE_STREAMED)
+        assert a.dtype == np.float32
+        b = o.read_pops(which, oracle_mod.POPS_STREAMED)
+        assert np.abs(a - b).max() / np.abs(b).max() <= REL32
+    sim.destroy(); o.close()
+
+
 # ---------------------------------------------------------------------------- fp32 variant
 def test_fp32_variant_config5_reduced(gpu, oracle_mod):
     P, I = wl.config5_droplets(n=40, nspheres=6, rmin=4.0, rmax=8.0)
