@@ -51,7 +51,7 @@ int validate(const lbm_params *p) {
     if ((double)p->nx * p->ny * p->nz * 19.0 > 4294967295.0) return LBM_E_INVALID;   // 32-bit element offsets
     if (!(p->dx > 0) || !(p->dt > 0) || !(p->W > 0) || !(p->rho_l > 0) || !(p->rho_g > 0)) return LBM_E_INVALID;
     if (!(p->nu_l > 0) || !(p->nu_g > 0) || !(p->M > 0) || !(p->alpha_l > 0) || !(p->alpha_g > 0)) return LBM_E_INVALID;
-    if (!(p->Cp > 0) || p->L_latent == 0.0 || !(p->A > 0) || !(p->eps_n >= 0) || !(p->sigma >= 0)) return LBM_E_INVALID;
+    if (!(p->Cp > 0) || p->L_latent == 0.0 || !(p->A > 0) || !(p->eps_n > 0) || !(p->sigma >= 0)) return LBM_E_INVALID;
     for (int a = 0; a < 3; ++a) {
         for (int s = 0; s < 2; ++s) {
             if (p->bc_f[a][s] < 0 || p->bc_f[a][s] > 2 || p->bc_g[a][s] < 0 || p->bc_g[a][s] > 2 ||

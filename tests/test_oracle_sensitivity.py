@@ -33,3 +33,19 @@ def test_config1_is_well_conditioned_to_1000_steps(oracle_mod):
     d = max(float(np.abs(x - y).max()) for x, y in zip(a.read_macro(), b.read_macro()))
     assert d < 1e-11, d
     a.close(); b.close()
+
+
+def test_config3_film_amplifies_roundoff_by_step_1000(oracle_mod):
+    """Film boiling over the hot wall (config 3, reduced grid): 1-ulp perturbations stay tiny to N = 300 and reach
+    1e-7 or more by N = 1000 -- the reason the GPU parity horizon of configs 3-4 is N <= 300."""
+    P, I = wl.config3_film2d(nx=64, ny=192, h0=24.0, amp=3.0)
+    rng = np.random.Generator(np.random.PCG64(3))
+    a = oracle_mod.Oracle(P); a.init(I["phi"], I["T"])
+    b = oracle_mod.Oracle(P); b.init(_ulp_perturbed(I["phi"], rng), _ulp_perturbed(I["T"], rng))
+    a.step(300); b.step(300)
+    d300 = max(float(np.abs(x - y).max()) for x, y in zip(a.read_macro(), b.read_macro()))
+    a.step(700); b.step(700)
+    d1000 = max(float(np.abs(x - y).max()) for x, y in zip(a.read_macro(), b.read_macro()))
+    assert d300 < 1e-10, d300
+    assert d1000 > 1e-8, d1000
+    a.close(); b.close()
