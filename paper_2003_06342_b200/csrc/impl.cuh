@@ -16,10 +16,13 @@ namespace lbm {
 // wide tiles only when the ragged last tile wastes at most 4% of the threads (192 = 128 + 64 would idle 25%)
 inline bool wide_tile_pays(int nx) { return nx >= 128 && ((nx + 127) / 128 * 128 - nx) * 25 <= nx; }
 
-struct TileWide3 { static constexpr int BX = 128, BY = 2, BZ = 1; };
-struct TileNarrow3 { static constexpr int BX = 32, BY = 4, BZ = 2; };
-struct TileWide2 { static constexpr int BX = 128, BY = 2, BZ = 1; };
-struct TileNarrow2 { static constexpr int BX = 32, BY = 8, BZ = 1; };
+// K_main runs 128-thread CTAs on wide tiles (4 per SM in fp64: 3.3% faster than 2 x 256 threads on config 4); K_phi and
+// the utility kernels keep 256 threads (PhiTile).
+struct TileWide3Phi { static constexpr int BX = 128, BY = 2, BZ = 1; using PhiTile = TileWide3Phi; };   // also K_main's tile in fp32
+struct TileWide3 { static constexpr int BX = 128, BY = 1, BZ = 1; using PhiTile = TileWide3Phi; };
+struct TileNarrow3 { static constexpr int BX = 32, BY = 4, BZ = 2; using PhiTile = TileNarrow3; };
+struct TileWide2 { static constexpr int BX = 128, BY = 2, BZ = 1; using PhiTile = TileWide2; };
+struct TileNarrow2 { static constexpr int BX = 32, BY = 8, BZ = 1; using PhiTile = TileNarrow2; };
 
 template <class real> const DevParams<real> &dev_params(const lbm_ctx *c);
 template <> inline const DevParams<double> &dev_params<double>(const lbm_ctx *c) { return c->pd; }
@@ -34,9 +37,11 @@ template <class T> dim3 grid_for(const lbm_params &P) {
 template <class LF, class LG, class LS, class real, class T> struct Impl {
     static constexpr int D = LF::D;
     static constexpr int NT = T::BX * T::BY * T::BZ;
+    using TP = typename T::PhiTile;                       // tile of K_phi and of the utility kernels
+    static constexpr int NTP = TP::BX * TP::BY * TP::BZ;
     // resident CTAs per SM the register allocation is bounded for (measured on config 4): fp64 2 x 256 threads at 128
     // registers; fp32 4 x 256 at 64 registers (+25% over 2 CTAs although a few values spill)
-    static constexpr int MINB = sizeof(real) == 8 ? 2 : 4;
+    static constexpr int MINB = (sizeof(real) == 8 ? 2 : 4) * 256 / NT;
 #ifndef LBM_PHI_NPT
 #define LBM_PHI_NPT 2
 #endif
@@ -111,7 +116,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         else CK(cudaMemsetAsync(dp, 0, N * es, c->stream));
         for (int b = 0; b < 2; ++b)
             CK(cudaMemsetAsync(wsp<real>(c, c->L.off_phi[b]), 0, c->L.phi_pad_elems * es, c->stream));
-        k_phi_fill<real, T::BX, T::BY, T::BZ><<<grid_for<T>(c->P), NT, 0, c->stream>>>(
+        k_phi_fill<real, TP::BX, TP::BY, TP::BZ><<<grid_for<TP>(c->P), NTP, 0, c->stream>>>(
             P, scratch, wsp<real>(c, c->L.off_phi[0]), wsp<real>(c, c->L.off_phi[1]));
         c->launches++;
         CK(cudaGetLastError());
@@ -163,9 +168,9 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
             if (timed) CK(cudaEventRecord(e3[1], c->stream));
             rc = macro ? launch_fused<MODE_STEP_MACRO>(c, F, in, pnew) : launch_fused<MODE_STEP>(c, F, in, pnew);
         } else {
-            dim3 gphi = grid_for<T>(c->P);
+            dim3 gphi = grid_for<TP>(c->P);
             if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
-            k_phi<LG, real, T::BX, T::BY, T::BZ, PHI_NPT><<<gphi, NT, 0, c->stream>>>(
+            k_phi<LG, real, TP::BX, TP::BY, TP::BZ, PHI_NPT><<<gphi, NTP, 0, c->stream>>>(
                 P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot[0]), wsp<real>(c, c->L.off_phi[pnew]));
             c->launches++;
             CK(cudaGetLastError());
@@ -216,7 +221,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         const size_t N = (size_t)c->L.N, es = sizeof(real);
         if (h_phi) {
             real *scratch = wsp<real>(c, c->L.off_scratch);
-            k_phi_unpad<real, T::BX, T::BY, T::BZ><<<grid_for<T>(c->P), NT, 0, c->stream>>>(
+            k_phi_unpad<real, TP::BX, TP::BY, TP::BZ><<<grid_for<TP>(c->P), NTP, 0, c->stream>>>(
                 dev_params<real>(c), wsp<real>(c, c->L.off_phi[c->curphi]), scratch);
             c->launches++;
             CK(cudaGetLastError());
@@ -239,7 +244,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         if (c->nsteps < 1) return LBM_E_STATE;
         real *tmp = nullptr;
         CK(cudaMalloc(&tmp, bytes));   // debug path: own temporary, not the borrowed workspace
-        k_stream_only<L, real, T::BX, T::BY, T::BZ><<<grid_for<T>(c->P), NT, 0, c->stream>>>(
+        k_stream_only<L, real, TP::BX, TP::BY, TP::BZ><<<grid_for<TP>(c->P), NTP, 0, c->stream>>>(
             dev_params<real>(c), wsp<real>(c, off[1 - c->cur]), tmp, which);
         c->launches++;
         cudaError_t e = cudaGetLastError();

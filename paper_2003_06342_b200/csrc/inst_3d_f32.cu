@@ -4,7 +4,7 @@
 
 namespace lbm {
 const ImplOps *ops_3d_f32(int nx) {
-    if (wide_tile_pays(nx)) return Impl<D3Q19, D3Q7, D3Q7, float, TileWide3>::ops();
+    if (wide_tile_pays(nx)) return Impl<D3Q19, D3Q7, D3Q7, float, TileWide3Phi>::ops();
     return Impl<D3Q19, D3Q7, D3Q7, float, TileNarrow3>::ops();
 }
 }  // namespace lbm

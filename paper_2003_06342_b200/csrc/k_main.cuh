@@ -8,6 +8,15 @@
 
 namespace lbm {
 
+// population stores: written once, read by the NEXT step only
+template <class real> __device__ __forceinline__ void st_pop(real *p, real v) {
+#ifdef LBM_EXP_STCS
+    __stcs(p, v);
+#else
+    *p = v;
+#endif
+}
+
 __device__ __forceinline__ double rsqrt_(double a) { return rsqrt(a); }
 __device__ __forceinline__ float rsqrt_(float a) { return rsqrtf(a); }
 
@@ -165,7 +174,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
             constexpr real w = real(LF::w(0));
             real bar = real(0);
             if constexpr (MODE != MODE_INIT) bar = src.template f<0, true>();
-            Fd.f_out[n] = a * bar + w * (U * K1 + K2);
+            st_pop(Fd.f_out + (n), a * bar + w * (U * K1 + K2));
         }
         static_for<LF::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
@@ -178,8 +187,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
                 const real q = real(0.5) * t * t + U;
                 const real h = dot_e<LF, I, real>(Hbx, Hby, Hbz);
                 const real fb = dot_e<LF, I, real>(Fbx, Fby, Fbz);
-                Fd.f_out[(unsigned)I * N + n] = a * bi + w * ((q + t) * (K1 + h) + (K2 + fb));
-                Fd.f_out[(unsigned)J * N + n] = a * bj + w * ((q - t) * (K1 - h) + (K2 - fb));
+                st_pop(Fd.f_out + ((unsigned)I * N + n), a * bi + w * ((q + t) * (K1 + h) + (K2 + fb)));
+                st_pop(Fd.f_out + ((unsigned)J * N + n), a * bj + w * ((q - t) * (K1 - h) + (K2 - fb)));
             }
         });
     }
@@ -197,7 +206,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
             constexpr real w = real(LS::w(0));
             real bar = real(0);
             if constexpr (MODE != MODE_INIT) bar = src.template s<0, true>();
-            Fd.s_out[n] = a * bar + w * (TO * U1 + bQ);
+            st_pop(Fd.s_out + (n), a * bar + w * (TO * U1 + bQ));
         }
         static_for<LS::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
@@ -208,8 +217,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
                 if constexpr (MODE != MODE_INIT) { bi = src.template s<I, true>(); bj = src.template s<J, true>(); }
                 const real t = dot_e<LS, I, real>(tx, ty, tz);
                 const real q = real(0.5) * t * t + U1;
-                Fd.s_out[(unsigned)I * N + n] = a * bi + w * (TO * (q + t) + bQ);
-                Fd.s_out[(unsigned)J * N + n] = a * bj + w * (TO * (q - t) + bQ);
+                st_pop(Fd.s_out + ((unsigned)I * N + n), a * bi + w * (TO * (q + t) + bQ));
+                st_pop(Fd.s_out + ((unsigned)J * N + n), a * bj + w * (TO * (q - t) + bQ));
             }
         });
     }
@@ -231,7 +240,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
             constexpr real w = real(LG::w(0));
             real bar = real(0);
             if constexpr (MODE != MODE_INIT) bar = src.template gg<0>();
-            Fd.g_out[n] = a * bar + w * (PO * U1 + bP);
+            st_pop(Fd.g_out + (n), a * bar + w * (PO * U1 + bP));
         }
         static_for<LG::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
@@ -243,8 +252,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
                 const real t = dot_e<LG, I, real>(tx, ty, tz);
                 const real q = real(0.5) * t * t + U1;
                 const real cn = dot_e<LG, I, real>(bx, by, bz);
-                Fd.g_out[(unsigned)I * N + n] = a * bi + w * (PO * (q + t) + (bP + cn));
-                Fd.g_out[(unsigned)J * N + n] = a * bj + w * (PO * (q - t) + (bP - cn));
+                st_pop(Fd.g_out + ((unsigned)I * N + n), a * bi + w * (PO * (q + t) + (bP + cn)));
+                st_pop(Fd.g_out + ((unsigned)J * N + n), a * bj + w * (PO * (q - t) + (bP - cn)));
             }
         });
     }
