@@ -13,8 +13,9 @@
  * Readings of garbled / silent passages of the paper are the ones listed in DESIGN.md ("Readings");
  * tags G* / S* in comments refer to that list.
  *
- * Parity unpinned: discretisation of div(u phi) (S5), the OPEN pressure face (S12),
- * the 3D coupling terms beyond symmetry checks (A34).  Everything else is pinned by tests/test_oracle_*.py.
+ * Parity unpinned: discretisation of div(u phi) (S5) and the OPEN pressure face (S12).
+ * The 3D coupling terms (not run in 3D by the paper) are pinned by the spherical Laplace law,
+ * the symmetry tests and the brute-force comparison; everything else by tests/test_oracle_*.py.
  */
 #ifndef LBM_ORACLE_H
 #define LBM_ORACLE_H
