@@ -41,7 +41,11 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     static constexpr int NTP = TP::BX * TP::BY * TP::BZ;
     // resident CTAs per SM the register allocation is bounded for (measured on config 4): fp64 2 x 256 threads at 128
     // registers; fp32 4 x 256 at 64 registers (+25% over 2 CTAs although a few values spill)
-    static constexpr int MINB = (sizeof(real) == 8 ? 2 : 4) * 256 / NT;
+#ifndef LBM_MINB3D
+#define LBM_MINB3D (2 * 256 / NT)
+#endif
+    // fp64 2D: 3 x 256 threads at 80 registers (+5% on 4096 x 3072 over 2 CTAs)
+    static constexpr int MINB = sizeof(real) == 8 ? (D == 2 ? 3 * 256 / NT : LBM_MINB3D) : 4 * 256 / NT;
 #ifndef LBM_PHI_NPT
 #define LBM_PHI_NPT 2
 #endif
