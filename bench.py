@@ -32,7 +32,9 @@ FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback when
 def make_workload(name: str, seed_offset: int = 0):
     if name == "config4":
         return wl.config4_film3d(seed=4 + seed_offset)
-    if name == "config4_sample":     # bounded sample of config 4 for the CPU oracle: same recipe, 128^3 nodes
+    if name == "config4_sample":     # bounded sample of config 4 for the CPU oracle: same recipe, a 256x256x128 slab
+        return wl.config4_film3d(nx=256, ny=256, nz=128, seed=4 + seed_offset)
+    if name == "config4_small":      # the reference arm's per-step sample (128^3)
         return wl.config4_film3d(nx=128, ny=128, nz=128, seed=4 + seed_offset)
     if name == "config3":
         return wl.config3_film2d(seed=3 + seed_offset)
@@ -132,7 +134,7 @@ def run_reference(args):
     rank, _, world = replicas.env_rank()
     if rank != 0:
         return 0
-    sample = "config4_sample" if args.workload == "config4" else args.workload
+    sample = "config4_small" if args.workload == "config4" else args.workload
     mlups, cores, desc, ms = oracle_throughput(sample, args.steps, args.warmup)
     P, _ = (wl.config4_film3d(nx=8, ny=8, nz=8) if args.workload == "config4" else make_workload(args.workload))
     line = {
@@ -217,6 +219,17 @@ def run_ours(args):
     torch.cuda.synchronize()
     ms_e2e, lu_e2e = replicas.reduce_job(f0.elapsed_time(f1), float(N) * K, dev)
     e2e_value = replicas.job_throughput_mlups(ms_e2e, lu_e2e)
+    # the same with the host copies around EVERY step (what a per-step host round trip would cost): 3 iterations
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s0.record()
+    for _ in range(3):
+        sim.init(h_phi, h_T)
+        sim.step(1)
+        sim.read_macro(out=outs)
+    s1.record()
+    torch.cuda.synchronize()
+    ms_strict, lu_strict = replicas.reduce_job(s0.elapsed_time(s1), float(N) * 3, dev)
+    e2e_strict = replicas.job_throughput_mlups(ms_strict, lu_strict)
     finite = bool(torch.isfinite(outs[0]).all() and torch.isfinite(outs[3]).all())
 
     if rank != 0:
@@ -247,7 +260,7 @@ def run_ours(args):
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         sample = "config4_sample" if args.workload == "config4" else ("config5_128" if args.workload.startswith("config5") else args.workload)
-        steps_cpu = 6 if sample != "config3" else 20
+        steps_cpu = 16 if sample == "config4_sample" else (6 if sample != "config3" else 20)   # about 10-30 s of CPU work
         mlups, cores, desc, _ = oracle_throughput(sample, steps_cpu, 1)
         cpu = {"value": mlups, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": desc}
 
@@ -263,7 +276,9 @@ def run_ours(args):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "MLUPS", "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                 "region": "lbm_init(host phi,T) + lbm_step(%d) + lbm_read_macro(host phi,u,p,T), pinned host buffers" % K,
-                "ms": ms_e2e},
+                "ms": ms_e2e,
+                "per_step_io": {"value": e2e_strict, "unit": "MLUPS", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                                "region": "3 x [lbm_init(host) + lbm_step(1) + lbm_read_macro(host)]"}},
         "gpu_launches": launches,
         "roofline": roofline,
         "cpu_baseline": cpu,
