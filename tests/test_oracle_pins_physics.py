@@ -263,3 +263,37 @@ def test_laplace_pressure_jump_3d_sphere(oracle_mod):
     assert 0.92 < ratio < 0.99, ratio                  # 0.952 measured; sigma/R (the 2D law) would read 0.476
     assert np.abs(u).max() < 5e-6
     assert abs(phi.sum() - phi0.sum()) / phi0.sum() < 1e-12
+
+
+@pytest.mark.parametrize("dims,u0", [((64, 48, 1), (0.04, -0.02, 0.0)), ((32, 28, 28), (0.03, 0.02, -0.03))])
+def test_uniform_advection_of_phi_and_T(oracle_mod, dims, u0):
+    """Galilean translation: with rho_l = rho_g and sigma = 0 a uniform velocity u0 is an exact fixed point of the NS
+    lattice (F_tot = 0, grad rho = 0), so the CAC equation advects a drop and the heat equation advects a warm blob
+    with exactly u0 (Eq.11c, 11d with m''' = 0): the centroids move by u0 t.  Pins the first moments of
+    g_eq = phi Gamma_i(u) (Eq.29b/31b) and s_eq = T Gamma_i(u) (Eq.33b) on every scalar lattice."""
+    nx, ny, nz = dims
+    P = wl.base_params(nx, ny, nz, rho_l=1.0, rho_g=1.0, sigma=0.0, phase_change=False, latent_heat=False,
+                       alpha_l=0.01, alpha_g=0.01)
+    z, y, x = np.meshgrid(np.arange(nz) + 0.5, np.arange(ny) + 0.5, np.arange(nx) + 0.5, indexing="ij")
+    c0 = np.array([nx / 2.0, ny / 2.0, nz / 2.0])
+    r = np.sqrt((x - c0[0]) ** 2 + (y - c0[1]) ** 2 + ((z - c0[2]) ** 2 if nz > 1 else 0))
+    R = 6.0 if nz == 1 else 4.0                                  # small enough that nothing wraps around the box
+    phi0 = 0.5 * (1 - np.tanh(2 * (R - r) / P["W"]))             # liquid drop (phi = 0) in gas
+    T0 = np.exp(-(r / (0.6 * R + 0.6)) ** 2)
+    u = np.zeros((3, nz, ny, nx))
+    for a in range(3):
+        u[a] = u0[a]
+    o = oracle_mod.Oracle(P)
+    o.init(phi0, T0, u, None)
+    steps = 200 if nz == 1 else 100
+    o.step(steps)
+    phi, un, _, T = o.read_macro()
+    o.close()
+    assert np.abs(un - u).max() < 1e-13                          # the flow stays uniform
+    coords = (x, y, z)
+    for field0, field in ((1 - phi0, 1 - phi), (T0, T)):
+        for a in range(3 if nz > 1 else 2):
+            cen0 = (coords[a] * field0).sum() / field0.sum()
+            cen = (coords[a] * field).sum() / field.sum()
+            assert abs((cen - cen0) - u0[a] * steps) < 0.02 * abs(u0[a] * steps) + 1e-3, (a, cen - cen0, u0[a] * steps)
+    assert abs(phi.sum() - phi0.sum()) < 1e-9 * phi0.sum() and abs(T.sum() - T0.sum()) < 1e-9 * T0.sum()
