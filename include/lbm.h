@@ -48,6 +48,8 @@ enum {
 /* flags */
 #define LBM_FLAG_PHASE_CHANGE 1u /* production rate Eq.(18) on (otherwise m''' = 0)        */
 #define LBM_FLAG_LATENT_HEAT 2u  /* source of the heat equation Eq.(33c,d),(34) on          */
+#define LBM_FLAG_PRESCRIBED_U 4u /* u stays the field given to lbm_init (Zalesak / vortex verifications); */
+                                 /* f is still stepped (its p is reported) but its first moment is ignored             */
 
 /* error codes */
 enum {

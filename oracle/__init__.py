@@ -25,6 +25,7 @@ F_KINDS = {"periodic": 0, "wall": 1, "open": 2}
 S_KINDS = {"periodic": 0, "zeroflux": 1, "dirichlet": 2}
 FLAG_PHASE_CHANGE = 1
 FLAG_LATENT_HEAT = 2
+FLAG_PRESCRIBED_U = 4
 CAC_MODIFIED_EQ = 0
 CAC_SOURCE = 1
 POPS_POSTCOLLISION = 0
@@ -103,7 +104,8 @@ def fill_params(P: dict) -> _Params:
     for a in range(3):
         s.grav[a] = float(P["grav"][a])
         s.force[a] = float(P.get("force", (0.0, 0.0, 0.0))[a])
-    s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0)
+    s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0) | (
+        FLAG_PRESCRIBED_U if P.get("prescribed_u", False) else 0)
     return s
 
 

@@ -476,6 +476,8 @@ static void pass_moments(oracle_ctx *c)
             for (int a = 0; a < 3; ++a) m1[a] += fi * cc * c->Lf.e[i][a];
         }
         for (int a = 0; a < 3; ++a) u[a] = (m1[a] / cs2f + 0.5 * dt * F[a]) / rho;
+        /* prescribed-velocity verifications (Zalesak disk, vortex): u stays the given field */
+        if (P->flags & ORA_PRESCRIBED_U) for (int a = 0; a < 3; ++a) u[a] = c->u[(long)a * N + n];
         /* 5: m''' from the stored Pdot; D = div(u phi) (S5) */
         double mdot = P->rho_g * c->pdot[n];
         double D = u[0] * grad[0] + u[1] * grad[1] + u[2] * grad[2] + phi * mdot * drho;

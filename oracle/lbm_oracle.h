@@ -34,7 +34,8 @@ enum { ORA_S_PERIODIC = 0, ORA_S_ZEROFLUX = 1 /* bounce-back */,
        ORA_S_DIRICHLET = 2 /* anti-bounce-back */ };
 /* flags */
 enum { ORA_PHASE_CHANGE = 1u /* Eq.(18) production rate on */,
-       ORA_LATENT_HEAT = 2u /* Eq.(33c,d),(34) source of the heat equation on */ };
+       ORA_LATENT_HEAT = 2u /* Eq.(33c,d),(34) source of the heat equation on */,
+       ORA_PRESCRIBED_U = 4u /* u is the field given to oracle_init and is not updated from f */ };
 /* conservative Allen-Cahn collision form */
 enum { ORA_CAC_MODIFIED_EQ = 0 /* Eq.(31a,b) */, ORA_CAC_SOURCE = 1 /* Eq.(29a,b),(30a,b) */ };
 /* stage selector of oracle_read_pops */

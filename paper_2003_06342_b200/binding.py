@@ -20,6 +20,7 @@ F_KINDS = {"periodic": 0, "wall": 1, "open": 2}
 S_KINDS = {"periodic": 0, "zeroflux": 1, "dirichlet": 2}
 FLAG_PHASE_CHANGE = 1
 FLAG_LATENT_HEAT = 2
+FLAG_PRESCRIBED_U = 4
 POPS_F, POPS_G, POPS_S = 0, 1, 2
 STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 
@@ -103,7 +104,8 @@ def make_params(P: dict, precision: int = 64) -> lbm_params:
     for k in ("dx", "dt", "rho_l", "rho_g", "nu_l", "nu_g", "sigma", "W", "M", "alpha_l", "alpha_g",
               "L_latent", "Cp", "T_sat", "theta_I", "A", "eps_n"):
         setattr(s, k, float(P[k]))
-    s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0)
+    s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0) | (
+        FLAG_PRESCRIBED_U if P.get("prescribed_u", False) else 0)
     return s
 
 

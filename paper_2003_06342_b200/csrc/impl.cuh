@@ -65,7 +65,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     }
 
     template <int MODE> static int launch_main(lbm_ctx *c, const DevFields<real> &F, int in = 0, int pnew = 0) {
-        if constexpr (MODE != MODE_INIT) {
+        if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU) {
             if (c->use_tma) {
                 using C = TmaCfg<LF, LG, LS, real>;
                 auto kern = k_main_tma<LF, LG, LS, real, MODE>;
@@ -86,7 +86,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
                 return LBM_OK;
             }
         }
-        if constexpr (MODE != MODE_INIT) {
+        if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU) {
             if (c->phi_tma) {
                 k_main_phitma<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB>
                     <<<grid_for<T>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F, c->map_phi_tile[pnew]);
@@ -168,7 +168,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         }
         DevFields<real> F = fields(c, in, out, pnew, pold);
         int rc;
-        if (c->fused) {
+        if (c->fused && !P.prescribed_u) {
             if (timed) CK(cudaEventRecord(e3[1], c->stream));
             rc = macro ? launch_fused<MODE_STEP_MACRO>(c, F, in, pnew) : launch_fused<MODE_STEP>(c, F, in, pnew);
         } else {
@@ -179,7 +179,8 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
             c->launches++;
             CK(cudaGetLastError());
             if (timed) CK(cudaEventRecord(e3[1], c->stream));
-            rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
+            if (P.prescribed_u) rc = launch_main<MODE_STEP_PU>(c, F, in, pnew);   // direct kernel only
+            else rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
         }
         if (rc) return rc;
         if (timed) {

@@ -119,6 +119,9 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
         ux = (cm * mx + P.hdt * Fx) * inv_rho;
         uy = (cm * my + P.hdt * Fy) * inv_rho;
         uz = (cm * mz + P.hdt * Fz) * inv_rho;
+        if constexpr (MODE == MODE_STEP_PU) {   // Zalesak / vortex verifications: u is the field given at init
+            ux = Fd.u[n]; uy = Fd.u[N + n]; uz = (LF::D == 3) ? Fd.u[2 * N + n] : real(0);
+        }
         // ---- H1 (time derivative), H5: heat moment with the STORED production rate (reading S3; Eq.34)
         dtphi = (phi - src.phi_old()) * P.inv_dt;                              // reading S4
         const real mdot_old = P.rho_g * src.pdot_old();
@@ -140,6 +143,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
         Fd.u[n] = ux; Fd.u[N + n] = uy; Fd.u[2 * N + n] = uz;
         Fd.p[n] = p; Fd.T[n] = T;
     }
+    if constexpr (MODE == MODE_STEP_PU) { Fd.p[n] = p; Fd.T[n] = T; }
 
     // ---- H7: sources, equilibria, BGK (Eq.25)
     const real mdot = P.rho_g * pdot;

@@ -20,7 +20,9 @@
 namespace lbm {
 
 enum { BC_PERIODIC = 0, BC_BOUNCE = 1 /* wall / zero-flux */, BC_ANTI = 2 /* open / Dirichlet */ };
-enum { MODE_STEP = 0, MODE_STEP_MACRO = 1, MODE_INIT = 2 };
+// MODE_STEP_PU: prescribed-velocity step (LBM_FLAG_PRESCRIBED_U): u is read from the macro array instead of Eq.(28a),
+// p and T are stored every step.  A separate instantiation so that the production kernels carry no trace of it.
+enum { MODE_STEP = 0, MODE_STEP_MACRO = 1, MODE_INIT = 2, MODE_STEP_PU = 3 };
 
 // ---- compile-time loop over directions ---------------------------------------------------------------
 template <class F, int... I>
@@ -65,7 +67,7 @@ template <class real> struct DevParams {
     real M, om_g, cac;                   // mobility, 1/(M/(cs2g dt)+1/2), M*(4/W)/cs2g * c
     real LCp, CpL, T_sat, theta_I, pc_coef;   // L/Cp, Cp/L, 4/(A W^2)
     real eps_n2;
-    int phase_change, latent_heat;
+    int phase_change, latent_heat, prescribed_u;
 };
 
 template <class real> struct DevFields {

@@ -136,6 +136,7 @@ template <class real> DevParams<real> make_dev_params(const lbm_params *p, const
     d.eps_n2 = (real)(p->eps_n * p->eps_n);
     d.phase_change = (p->flags & LBM_FLAG_PHASE_CHANGE) ? 1 : 0;
     d.latent_heat = (p->flags & LBM_FLAG_LATENT_HEAT) ? 1 : 0;
+    d.prescribed_u = (p->flags & LBM_FLAG_PRESCRIBED_U) ? 1 : 0;
     return d;
 }
 

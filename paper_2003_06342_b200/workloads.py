@@ -46,7 +46,7 @@ def base_params(nx, ny, nz=1, **over):
         alpha_l=0.02, alpha_g=0.05,
         L_latent=1.0, Cp=0.1, T_sat=0.0, theta_I=0.0,
         A=10.0 / 48.0, eps_n=1e-5,
-        phase_change=True, latent_heat=True,
+        phase_change=True, latent_heat=True, prescribed_u=False,
     )
     P.update(over)
     return P

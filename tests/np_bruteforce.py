@@ -209,7 +209,8 @@ class NPModel:
             rho, F, grho = self._closures(self.phi, self.grad, self.lap)
             cs2 = self.e2f * c * c
             m1 = c * np.tensordot(self.ef.astype(float).T, self.pops["f"], axes=(1, 0))
-            self.u = (m1 / cs2 + 0.5 * dt * F) / rho                                               # Eq.(28a)
+            if not P.get("prescribed_u", False):
+                self.u = (m1 / cs2 + 0.5 * dt * F) / rho                                           # Eq.(28a)
             drho = 1 / P["rho_g"] - 1 / P["rho_l"]
             mdot = P["rho_g"] * self.pdot
             D = (self.u * self.grad).sum(axis=0) + self.phi * mdot * drho

@@ -128,6 +128,14 @@ def test_3d_flags_off(gpu, oracle_mod):
     _run_parity(gpu, oracle_mod, P, _random_state(P, 29), [1, 15], label="3d flags off")
 
 
+def test_prescribed_velocity_mode(gpu, oracle_mod):
+    """LBM_FLAG_PRESCRIBED_U: u stays the field given at init (Zalesak / vortex verifications)."""
+    P = wl.base_params(40, 28, 1, prescribed_u=True, nu_l=0.05, nu_g=0.2)
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 43), [1, 15], label="2d prescribed u")
+    P = wl.base_params(136, 6, 5, prescribed_u=True)
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 44), [1, 8], label="3d prescribed u")
+
+
 def test_minimal_grids(gpu, oracle_mod):
     for dims in ((2, 2, 1), (3, 2, 2), (2, 5, 3)):
         P = wl.base_params(*dims)

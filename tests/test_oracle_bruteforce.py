@@ -107,6 +107,11 @@ def test_3d_walls_z(oracle_mod):
     _compare(oracle_mod, P, 10, 17)
 
 
+def test_2d_prescribed_velocity(oracle_mod):
+    P = wl.base_params(8, 8, 1, prescribed_u=True, nu_l=0.05, nu_g=0.2)
+    _compare(oracle_mod, P, 10, 19)
+
+
 def test_3d_flags_off(oracle_mod):
     P = wl.base_params(6, 8, 6, phase_change=False, latent_heat=False)
     _compare(oracle_mod, P, 10, 18)

@@ -297,3 +297,33 @@ def test_uniform_advection_of_phi_and_T(oracle_mod, dims, u0):
             cen = (coords[a] * field).sum() / field.sum()
             assert abs((cen - cen0) - u0[a] * steps) < 0.02 * abs(u0[a] * steps) + 1e-3, (a, cen - cen0, u0[a] * steps)
     assert abs(phi.sum() - phi0.sum()) < 1e-9 * phi0.sum() and abs(T.sum() - T0.sum()) < 1e-9 * T0.sum()
+
+
+def test_zalesak_slotted_disk_rotation(oracle_mod):
+    """Prescribed-velocity verification of the CAC equation: a slotted disk in solid-body rotation
+    u = omega (-(y - yc), x - xc) is upside down after half a turn and back after one turn ("the contour is superimposed
+    to the initial one although the slot corners are slightly rounded").  64 x 64, R = 20, W = 3, M = 0.005."""
+    n, R, W, Tturn = 64, 20.0, 3.0, 4000
+    P = wl.base_params(n, n, 1, W=W, M=0.005, rho_l=1.0, rho_g=1.0, sigma=0.0, phase_change=False, latent_heat=False,
+                       prescribed_u=True)
+    y, x = np.meshgrid(np.arange(n) + 0.5, np.arange(n) + 0.5, indexing="ij")
+    xc = yc = n / 2.0
+    d = np.sqrt((x - xc) ** 2 + (y - yc) ** 2)
+    phi0 = 0.5 * (1 + np.tanh(2 * (R - d) / W))
+    phi0[(np.abs(x - xc) <= R / 6) & (y >= yc - 1.1 * R) & (y <= yc)] = 0.0
+    om = 2 * np.pi / Tturn
+    u = np.zeros((3, 1, n, n))
+    u[0, 0] = -om * (y - yc)
+    u[1, 0] = om * (x - xc)
+    o = oracle_mod.Oracle(P)
+    o.init(phi0[None], None, u, None)
+    o.step(Tturn // 2)
+    half = o.read_macro()[0][0].copy()
+    o.step(Tturn - Tturn // 2)
+    full, un, _, _ = o.read_macro()
+    o.close()
+    assert np.all(un == u)                                        # the velocity is not touched
+    assert np.abs(half - phi0[::-1, ::-1]).mean() < 0.02          # half a turn = point reflection
+    assert np.abs(half - phi0).mean() > 0.04
+    assert np.abs(full[0] - phi0).mean() < 0.02                   # back after one turn
+    assert abs(full.sum() - phi0.sum()) < 1e-10 * phi0.sum()
