@@ -127,6 +127,12 @@ int lbm_init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, co
  * The last of the n steps also stores u, p, T for lbm_read_macro. */
 int lbm_step(lbm_ctx *c, int n);
 
+/* LBM_FLAG_PRESCRIBED_U only: replace the prescribed velocity by the HOST array h_u ([3][nz][ny][nx], element type
+ * = precision; the third component is ignored in 2D).  The field is u of the NEXT time level: the next step takes its
+ * moments (T, p) and collides with it (time-dependent velocity of the reversing vortex).
+ * Synchronises the stream.  LBM_E_INVALID without the flag, LBM_E_STATE before lbm_init. */
+int lbm_set_velocity(lbm_ctx *c, const void *h_u);
+
 /* Copy the macroscopic fields of the current time level to HOST arrays; any pointer may be NULL.
  * h_u is [3][z][y][x].  Synchronises. */
 int lbm_read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T);

@@ -76,6 +76,7 @@ def lib():
         L.oracle_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
         L.oracle_read_aux.argtypes = [C.c_void_p, dp, dp, dp, dp]
         L.oracle_set_cac_form.argtypes = [C.c_void_p, C.c_int]
+        L.oracle_set_velocity.argtypes = [C.c_void_p, dp]
         L.oracle_num_threads.restype = C.c_int
         L.oracle_lattice.argtypes = [C.c_int, C.POINTER(C.c_int), dp, dp]
         _lib = L
@@ -169,6 +170,11 @@ class Oracle:
 
     def set_cac_form(self, form):
         lib().oracle_set_cac_form(self._h, int(form))
+
+    def set_velocity(self, u):
+        """Prescribed-velocity mode: u of the next time level."""
+        u = self._arr(u, (3,) + self.shape)
+        assert lib().oracle_set_velocity(self._h, _ptr(u)) == 0
 
     def read_macro(self):
         phi = np.empty(self.shape)

@@ -43,6 +43,8 @@ struct oracle_ctx {
     double *f, *g, *s, *fpost, *gpost, *spost;
     /* macroscopic fields at level n */
     double *phi, *phi_prev, *dtphi, *u, *p, *T, *pdot;
+    /* prescribed-velocity mode: u of the NEXT time level, given by oracle_set_velocity (NULL: u does not change) */
+    double *u_next;
     /* derived fields of phi at level n */
     double *grad, *lap;
 };
@@ -195,11 +197,23 @@ void oracle_destroy(oracle_ctx *c)
     if (!c) return;
     free(c->f); free(c->g); free(c->s); free(c->fpost); free(c->gpost); free(c->spost);
     free(c->phi); free(c->phi_prev); free(c->dtphi); free(c->u); free(c->p); free(c->T); free(c->pdot);
-    free(c->grad); free(c->lap);
+    free(c->grad); free(c->lap); free(c->u_next);
     free(c);
 }
 
 void oracle_set_cac_form(oracle_ctx *c, int form) { if (c) c->cac_form = form; }
+
+/* Time-dependent prescribed velocity (reversing vortex: u'(x,t) = u(x) cos(pi t / 2 T_f)): the field
+ * given here is u at the NEXT time level; the moments pass of the next step takes it as u^{n+1}.  The collision
+ * of the next step still sees u^n, the field of the level it collides at. */
+int oracle_set_velocity(oracle_ctx *c, const double *u)
+{
+    if (!c || !u || !(c->P.flags & ORA_PRESCRIBED_U)) return -1;
+    if (!c->u_next) c->u_next = (double *)malloc(3 * (size_t)c->N * sizeof(double));
+    if (!c->u_next) return -1;
+    memcpy(c->u_next, u, 3 * (size_t)c->N * sizeof(double));
+    return 0;
+}
 
 /* ------------------------------------------------------------------------------------------------
  * phi at a possibly out-of-domain position (reading S8-iv): the value a ghost layer filled axis by
@@ -477,7 +491,10 @@ static void pass_moments(oracle_ctx *c)
         }
         for (int a = 0; a < 3; ++a) u[a] = (m1[a] / cs2f + 0.5 * dt * F[a]) / rho;
         /* prescribed-velocity verifications (Zalesak disk, vortex): u stays the given field */
-        if (P->flags & ORA_PRESCRIBED_U) for (int a = 0; a < 3; ++a) u[a] = c->u[(long)a * N + n];
+        if (P->flags & ORA_PRESCRIBED_U) {
+            const double *up = c->u_next ? c->u_next : c->u;   /* u(x, t^{n+1}) */
+            for (int a = 0; a < 3; ++a) u[a] = up[(long)a * N + n];
+        }
         /* 5: m''' from the stored Pdot; D = div(u phi) (S5) */
         double mdot = P->rho_g * c->pdot[n];
         double D = u[0] * grad[0] + u[1] * grad[1] + u[2] * grad[2] + phi * mdot * drho;

@@ -76,6 +76,8 @@ int oracle_read_pops(oracle_ctx *c, int which, int stage, double *out);
 /* auxiliary fields for the pins: grad phi [3][N], laplacian [N], production rate Pdot [N], dphi/dt [N] */
 int oracle_read_aux(oracle_ctx *c, double *grad, double *lap, double *pdot, double *dtphi);
 void oracle_set_cac_form(oracle_ctx *c, int form);
+/* ORA_PRESCRIBED_U only: u [3][z][y][x] of the next time level (time-dependent prescribed velocity) */
+int oracle_set_velocity(oracle_ctx *c, const double *u);
 int oracle_num_threads(void);
 /* lattice table access for the pins: returns Q, fills e[Q][3], w[Q], *e2 */
 int oracle_lattice(int id, int *e, double *w, double *e2);

@@ -24,7 +24,7 @@ FLAG_PRESCRIBED_U = 4
 POPS_F, POPS_G, POPS_S = 0, 1, 2
 STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 
-EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_read_macro", "lbm_read_pops",
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_read_macro", "lbm_read_pops",
            "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
@@ -67,6 +67,7 @@ def load_library():
         L.lbm_create.argtypes = [C.POINTER(lbm_params), C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]
         L.lbm_init.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_step.argtypes = [C.c_void_p, C.c_int]
+        L.lbm_set_velocity.argtypes = [C.c_void_p, C.c_void_p]
         L.lbm_read_macro.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_sync.argtypes = [C.c_void_p]
@@ -184,6 +185,10 @@ class LBM:
 
     def step(self, n: int = 1):
         _check(self._L.lbm_step(self._h, int(n)), "lbm_step")
+
+    def set_velocity(self, u):
+        ptr, keep = _host_ptr(u, self.dtype, (3,) + self.shape, "u")
+        _check(self._L.lbm_set_velocity(self._h, C.c_void_p(ptr)), "lbm_set_velocity")
 
     def read_macro(self, out=None):
         """Returns (phi, u, p, T) as numpy arrays; ``out`` may give preallocated host arrays/tensors (pinned)."""

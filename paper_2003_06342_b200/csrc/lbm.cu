@@ -290,6 +290,15 @@ int lbm_init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, co
     return c->ops->init(c, h_phi, h_T, h_u, h_p);
 }
 
+int lbm_set_velocity(lbm_ctx *c, const void *h_u) {
+    if (!c || !h_u || !(c->P.flags & LBM_FLAG_PRESCRIBED_U)) return LBM_E_INVALID;
+    if (!c->inited) return LBM_E_STATE;
+    const size_t es = c->P.precision == 64 ? 8 : 4;
+    CK(cudaMemcpyAsync(c->ws + c->L.off_u, h_u, 3 * (size_t)c->L.N * es, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return LBM_OK;
+}
+
 int lbm_step(lbm_ctx *c, int n) {
     if (!c || n < 0) return LBM_E_INVALID;
     if (!c->inited) return LBM_E_STATE;

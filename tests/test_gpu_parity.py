@@ -136,6 +136,38 @@ def test_prescribed_velocity_mode(gpu, oracle_mod):
     _run_parity(gpu, oracle_mod, P, _random_state(P, 44), [1, 8], label="3d prescribed u")
 
 
+def test_time_dependent_prescribed_velocity(gpu, oracle_mod):
+    """lbm_set_velocity: the given field is u of the next time level on both sides (reversing vortex)."""
+    P = wl.base_params(40, 28, 1, prescribed_u=True)
+    st = _random_state(P, 45)
+    rng = np.random.Generator(np.random.PCG64(46))
+    o = oracle_mod.Oracle(P)
+    o.init(*st)
+    g = gpu.LBM(P, 64)
+    g.init(*st)
+    for k in range(6):
+        u = 0.02 * rng.uniform(-1, 1, size=(3,) + o.shape)
+        u[2] = 0.0
+        o.set_velocity(u)
+        g.set_velocity(u)
+        o.step(1 + k % 2)
+        g.step(1 + k % 2)
+        _compare_state(gpu, g, o, oracle_mod, TOL64, True, "set_velocity %d" % k)
+    g.destroy()
+    # the call is refused before lbm_init and without the flag
+    g = gpu.LBM(P, 64)
+    with pytest.raises(gpu.LBMError):
+        g.set_velocity(np.zeros((3,) + o.shape))
+    g.destroy()
+    o.close()
+    P2 = wl.base_params(8, 8, 1)
+    g = gpu.LBM(P2, 64)
+    g.init(np.full((1, 8, 8), 0.5))
+    with pytest.raises(gpu.LBMError):
+        g.set_velocity(np.zeros((3, 1, 8, 8)))
+    g.destroy()
+
+
 def test_minimal_grids(gpu, oracle_mod):
     for dims in ((2, 2, 1), (3, 2, 2), (2, 5, 3)):
         P = wl.base_params(*dims)

@@ -327,3 +327,30 @@ def test_zalesak_slotted_disk_rotation(oracle_mod):
     assert np.abs(half - phi0).mean() > 0.04
     assert np.abs(full[0] - phi0).mean() < 0.02                   # back after one turn
     assert abs(full.sum() - phi0.sum()) < 1e-10 * phi0.sum()
+
+
+def test_disk_in_reversing_vortex_returns(oracle_mod):
+    """Second CAC verification: a disk deformed by the vortex u = u0 (-cos pi(x-1/2) sin pi(y-1/2),
+    sin pi(x-1/2) cos pi(y-1/2)) whose amplitude follows cos(pi t / 2 T_f) is strongly stretched at t = T_f and is the
+    initial disk again at t = 2 T_f.  64 x 64, R = 12 at (32, 19), T_f = 1000 steps, u0 = 0.05."""
+    n, R, W, Tf, u0 = 64, 12.0, 3.0, 1000, 0.05
+    P = wl.base_params(n, n, 1, W=W, M=0.005, rho_l=1.0, rho_g=1.0, sigma=0.0, phase_change=False, latent_heat=False,
+                       prescribed_u=True)
+    y, x = np.meshgrid(np.arange(n) + 0.5, np.arange(n) + 0.5, indexing="ij")
+    X, Y = x / n, y / n
+    phi0 = 0.5 * (1 + np.tanh(2 * (R - np.sqrt((x - 32) ** 2 + (y - 19) ** 2)) / W))
+    ub = np.zeros((3, 1, n, n))
+    ub[0, 0] = -u0 * np.cos(np.pi * (X - 0.5)) * np.sin(np.pi * (Y - 0.5))
+    ub[1, 0] = u0 * np.sin(np.pi * (X - 0.5)) * np.cos(np.pi * (Y - 0.5))
+    o = oracle_mod.Oracle(P)
+    o.init(phi0[None], None, ub, None)
+    for k in range(2 * Tf):
+        o.set_velocity(ub * np.cos(np.pi * (k + 1) / (2 * Tf)))
+        o.step(1)
+        if k + 1 == Tf:
+            mid = o.read_macro()[0][0].copy()
+    fin = o.read_macro()[0][0]
+    o.close()
+    assert np.abs(mid - phi0).mean() > 0.1            # far from the disk at the turning point
+    assert np.abs(fin - phi0).mean() < 0.005          # and back on it at 2 T_f
+    assert abs(fin.sum() - phi0.sum()) < 1e-10 * phi0.sum()
