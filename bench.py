@@ -287,6 +287,65 @@ def run_ours(args):
     return 0
 
 
+def run_slabs(args):
+    """Slab decomposition of the workload along its slowest axis (paper's multi-GPU mode).
+
+    --slabs N (one process, one GPU): the N slabs run one after the other on one stream -- measures what the
+    decomposition costs (ghost layers, pack/unpack launches, shorter launches), not a speed-up.
+    --parallelism slabs under torchrun: one slab per rank, WEAK scaling (config 4 stacked N times along z), ghost layers
+    exchanged with NCCL point-to-point calls between the two phases of every step."""
+    import torch
+    from paper_2003_06342_b200 import slabs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU path")
+    rank, local_rank, world = replicas.init_process_group("nccl")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    K, W, prec = args.steps, args.warmup, args.precision
+    if args.parallelism == "slabs":
+        if not args.workload.startswith("config4"):
+            raise SystemExit("bench.py: --parallelism slabs is defined for config4 (stacked along z)")
+        P, _ = wl.config4_film3d(16, 16, 16)                      # parameters only
+        P.update(nx=256, ny=256, nz=512 * world)
+        sim = slabs.DistSlab(P, rank, world, prec)
+        z0, z1 = sim.slab.layer_range()
+        _, I = wl.config4_film3d(256, 256, 512 * world, zrange=(z0, z1))
+        sim.init(I["phi"], I["T"], local=True)
+        n_slabs, mode = world, "slabs x%d (one per rank, NCCL p2p ghost exchange)" % world
+        owned = sim.slab.P["slab"]["count"] * 256 * 256
+    else:
+        P, I = make_workload(args.workload)
+        sim = slabs.SlabGroup(P, args.slabs, prec)
+        sim.init(I["phi"], I["T"])
+        n_slabs, mode = args.slabs, "slabs x%d in one process on one GPU (sequential)" % args.slabs
+        owned = P["nx"] * P["ny"] * P["nz"]
+    del I
+    sim.step(W)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    replicas.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    sim.step(K)
+    e1.record()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    ms_job, lu_job = replicas.reduce_job(e0.elapsed_time(e1), float(owned) * K, dev)
+    phi = sim.read_macro()[0]
+    finite = bool(np.isfinite(phi).all())
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC if prec == 64 else "MLUPS (full coupled step, fp32)",
+            "value": replicas.job_throughput_mlups(ms_job, lu_job), "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_job / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "grid": [P["nx"], P["ny"], P["nz"]], "parallelism": mode,
+                       "slabs": n_slabs, "finite": finite}}))
+    sim.destroy()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -296,6 +355,9 @@ def main():
     ap.add_argument("--precision", type=int, default=64, choices=(32, 64))
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--parallelism", default="replicas", choices=("replicas", "slabs"),
+                    help="N > 1: independent replicas (default, the bench contract) or one slab of a stacked domain per rank")
+    ap.add_argument("--slabs", type=int, default=0, help="cut the workload into this many slabs on ONE GPU (overhead measurement)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
@@ -304,6 +366,8 @@ def main():
             args.steps = 20          # bounded: the oracle runs at a few MLUPS
         args.warmup = min(args.warmup, 2)
         return run_reference(args)
+    if args.slabs > 0 or args.parallelism == "slabs":
+        return run_slabs(args)
     return run_ours(args)
 
 

@@ -75,8 +75,16 @@ enum {
  * nz == 1 selects 2D (lattices must be D2Q*), nz > 1 selects 3D (D3Q*).
  * Supported lattice sets (f, g, s): (D2Q9, D2Q9, D2Q5), (D2Q9, D2Q9, D2Q9), (D3Q19, D3Q7, D3Q7).
  * bc_*[axis][side]: axis 0,1,2 = x,y,z; side 0 = low face, 1 = high face.  A periodic face must be
- * periodic on both sides and for all three distributions.  Walls sit half a cell outside the first/last
- * node (node i is at (i + 1/2) dx).
+ * periodic on both sides and for all three distributions (except next to a ghost layer, see halo).
+ * Walls sit half a cell outside the first/last node (node i is at (i + 1/2) dx).
+ *
+ * halo[side] (slab decomposition of the paper's multi-GPU runs): the context holds one slab of a
+ * larger domain cut along the SLOWEST axis (z in 3D, y in 2D).  halo[0] = 1 declares the first layer of that axis,
+ * halo[1] = 1 the last one, a GHOST layer: a copy of the neighbouring slab's boundary layer, refreshed by the
+ * caller with lbm_halo_pack / lbm_halo_unpack between the two phases of a step (lbm_step_phase).  nz (ny in 2D)
+ * COUNTS the ghost layers; the three face kinds on a ghost side must be PERIODIC (the ghost layer is updated like any
+ * node and its results are discarded), while the other side of the axis keeps its own kind.  Arrays given to
+ * lbm_init and returned by lbm_read_* include the ghost layers; lbm_init wants valid phi, T, u, p there.
  */
 typedef struct lbm_params {
     int nx, ny, nz;
@@ -100,6 +108,7 @@ typedef struct lbm_params {
     double A;               /* script-A of Eq.(18): 10/48 in the paper               */
     double eps_n;           /* n = grad phi / sqrt(|grad phi|^2 + eps_n^2) (reading S7)   */
     unsigned flags;         /* LBM_FLAG_*                                                           */
+    int halo[2];            /* ghost layer on the low / high side of the slowest axis (0 or 1)      */
 } lbm_params;
 
 typedef struct lbm_ctx lbm_ctx;
@@ -132,6 +141,27 @@ int lbm_step(lbm_ctx *c, int n);
  * moments (T, p) and collides with it (time-dependent velocity of the reversing vortex).
  * Synchronises the stream.  LBM_E_INVALID without the flag, LBM_E_STATE before lbm_init. */
 int lbm_set_velocity(lbm_ctx *c, const void *h_u);
+
+/* ---- slab decomposition (contexts with halo[0] | halo[1]; lbm_step itself returns LBM_E_STATE for them) ----------
+ * One step of a slab is   lbm_step_phase(c, 0, .)  -> exchange LBM_HALO_PHI ->  lbm_step_phase(c, 1, macros)
+ * -> exchange LBM_HALO_POPS.   After lbm_init one LBM_HALO_POPS exchange is due before the first step.
+ * phase 0 = K_phi (phi^{n+1} of every layer, Eq.32); phase 1 = K_main (moments, production, collisions) and the
+ * buffer flip; store_macros != 0 also stores u, p, T.  Both are asynchronous on the context's stream.
+ *
+ * An exchange of `what` towards `side`: the sender packs its boundary layer next to its ghost side with
+ * lbm_halo_pack(c, what, side, d_buf) into a DEVICE buffer of lbm_halo_bytes(c, what) bytes, the buffer travels to the
+ * neighbour on that side (NCCL send/recv, a peer copy, or the same buffer when both slabs live in one process), and the
+ * neighbour unpacks it into its ghost layer of the OPPOSITE side with lbm_halo_unpack(c, what, 1 - side, d_buf).
+ *   LBM_HALO_PHI : the padded phi^{n+1} layer (with its in-layer ghost images);
+ *   LBM_HALO_POPS: the post-collision populations that stream across the cut, i.e. those with e_axis = +1 for
+ *                  side 1 and e_axis = -1 for side 0 (5 + 1 + 1 of D3Q19/D3Q7/D3Q7; 3 + 3 + 1 or 3 in 2D), whole layers.
+ * pack / unpack are one kernel launch each, asynchronous on the context's stream; the caller orders the transfer
+ * after the pack and the unpack after the transfer.  LBM_E_INVALID if the context has no ghost layer on that side. */
+enum { LBM_HALO_PHI = 0, LBM_HALO_POPS = 1 };
+int lbm_step_phase(lbm_ctx *c, int phase, int store_macros);
+int lbm_halo_bytes(const lbm_ctx *c, int what, size_t *bytes);
+int lbm_halo_pack(lbm_ctx *c, int what, int side, void *d_buf);
+int lbm_halo_unpack(lbm_ctx *c, int what, int side, const void *d_buf);
 
 /* Copy the macroscopic fields of the current time level to HOST arrays; any pointer may be NULL.
  * h_u is [3][z][y][x].  Synchronises. */

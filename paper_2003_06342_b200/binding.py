@@ -23,8 +23,9 @@ FLAG_LATENT_HEAT = 2
 FLAG_PRESCRIBED_U = 4
 POPS_F, POPS_G, POPS_S = 0, 1, 2
 STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
+HALO_PHI, HALO_POPS = 0, 1
 
-EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_read_macro", "lbm_read_pops",
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops",
            "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
@@ -45,6 +46,7 @@ class lbm_params(C.Structure):
         ("L_latent", C.c_double), ("Cp", C.c_double), ("T_sat", C.c_double), ("theta_I", C.c_double),
         ("A", C.c_double), ("eps_n", C.c_double),
         ("flags", C.c_uint),
+        ("halo", C.c_int * 2),
     ]
 
 
@@ -68,6 +70,10 @@ def load_library():
         L.lbm_init.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_step.argtypes = [C.c_void_p, C.c_int]
         L.lbm_set_velocity.argtypes = [C.c_void_p, C.c_void_p]
+        L.lbm_step_phase.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.lbm_halo_bytes.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_size_t)]
+        L.lbm_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.lbm_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_read_macro.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_sync.argtypes = [C.c_void_p]
@@ -107,6 +113,8 @@ def make_params(P: dict, precision: int = 64) -> lbm_params:
         setattr(s, k, float(P[k]))
     s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0) | (
         FLAG_PRESCRIBED_U if P.get("prescribed_u", False) else 0)
+    halo = P.get("halo", (0, 0))
+    s.halo[0], s.halo[1] = int(halo[0]), int(halo[1])
     return s
 
 
@@ -185,6 +193,26 @@ class LBM:
 
     def step(self, n: int = 1):
         _check(self._L.lbm_step(self._h, int(n)), "lbm_step")
+
+    # slab contexts (P["halo"]): the two phases of a step and the ghost-layer buffers, see include/lbm.h
+    def step_phase(self, phase: int, store_macros: bool = False):
+        _check(self._L.lbm_step_phase(self._h, int(phase), 1 if store_macros else 0), "lbm_step_phase")
+
+    def halo_bytes(self, what: int) -> int:
+        n = C.c_size_t()
+        _check(self._L.lbm_halo_bytes(self._h, int(what), C.byref(n)), "lbm_halo_bytes")
+        return int(n.value)
+
+    def _dev_buf(self, what, buf):
+        if buf.device.type != "cuda" or not buf.is_contiguous() or buf.numel() * buf.element_size() < self.halo_bytes(what):
+            raise ValueError("halo buffer: contiguous CUDA tensor of at least %d bytes expected" % self.halo_bytes(what))
+        return C.c_void_p(buf.data_ptr())
+
+    def halo_pack(self, what: int, side: int, buf):
+        _check(self._L.lbm_halo_pack(self._h, int(what), int(side), self._dev_buf(what, buf)), "lbm_halo_pack")
+
+    def halo_unpack(self, what: int, side: int, buf):
+        _check(self._L.lbm_halo_unpack(self._h, int(what), int(side), self._dev_buf(what, buf)), "lbm_halo_unpack")
 
     def set_velocity(self, u):
         ptr, keep = _host_ptr(u, self.dtype, (3,) + self.shape, "u")

@@ -34,6 +34,7 @@ struct Layout {
 struct ImplOps {
     int (*init)(lbm_ctx *, const void *, const void *, const void *, const void *);
     int (*step)(lbm_ctx *, int);
+    int (*step_phase)(lbm_ctx *, int, int);
     int (*read_macro)(lbm_ctx *, void *, void *, void *, void *);
     int (*read_pops)(lbm_ctx *, int, int, void *);
     int bx, by, bz;   // tile of nodes per CTA
@@ -59,6 +60,7 @@ struct lbm_ctx {
     int cur;       // buffer holding the post-collision populations of the current level
     int curphi;    // padded phi buffer of the current level
     bool inited;
+    int phase;     // slab contexts: the phase lbm_step_phase expects next (0 or 1)
     long long nsteps, launches;
     lbm::DevParams<double> pd;
     lbm::DevParams<float> pf;

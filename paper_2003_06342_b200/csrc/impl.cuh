@@ -130,7 +130,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         if (rc) return rc;
         CK(cudaStreamSynchronize(c->stream));
         c->nsteps = 0;
-        c->inited = true;
+        c->inited = true; c->phase = 0;
         return LBM_OK;
     }
 
@@ -157,37 +157,63 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         }
     }
 
-    // enqueue the kernels of ONE step and flip the buffers
-    static int step_once(lbm_ctx *c, bool macro, bool timed) {
+    // phase 0 of a step: K_phi (phi^{n+1} of every node, Eq.32)
+    static int launch_phi(lbm_ctx *c) {
+        const DevParams<real> &P = dev_params<real>(c);
+        const int in = c->cur, pnew = 1 - c->curphi;
+        dim3 gphi = grid_for<TP>(c->P);
+        if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
+        k_phi<LG, real, TP::BX, TP::BY, TP::BZ, PHI_NPT><<<gphi, NTP, 0, c->stream>>>(
+            P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot[0]), wsp<real>(c, c->L.off_phi[pnew]));
+        c->launches++;
+        CK(cudaGetLastError());
+        return LBM_OK;
+    }
+
+    // phase 1 of a step: K_main, then the buffers flip
+    static int launch_collide(lbm_ctx *c, bool macro) {
         const DevParams<real> &P = dev_params<real>(c);
         const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
+        DevFields<real> F = fields(c, in, out, pnew, pold);
+        int rc;
+        if (P.prescribed_u) rc = launch_main<MODE_STEP_PU>(c, F, in, pnew);   // direct kernel only
+        else rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
+        if (rc) return rc;
+        c->cur = out; c->curphi = pnew; c->nsteps++;
+        return LBM_OK;
+    }
+
+    // the two phases separately, for slab contexts whose ghost layers are exchanged in between (include/lbm.h)
+    static int step_phase(lbm_ctx *c, int phase, int macro) {
+        return phase == 0 ? launch_phi(c) : launch_collide(c, macro != 0);
+    }
+
+    // enqueue the kernels of ONE step and flip the buffers
+    static int step_once(lbm_ctx *c, bool macro, bool timed) {
         cudaEvent_t e3[3] = {nullptr, nullptr, nullptr};
         if (timed) {
             for (auto &e : e3) CK(cudaEventCreate(&e));
             CK(cudaEventRecord(e3[0], c->stream));
         }
-        DevFields<real> F = fields(c, in, out, pnew, pold);
         int rc;
-        if (c->fused && !P.prescribed_u) {
+        if (c->fused && !dev_params<real>(c).prescribed_u) {
+            const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
+            DevFields<real> F = fields(c, in, out, pnew, pold);
             if (timed) CK(cudaEventRecord(e3[1], c->stream));
             rc = macro ? launch_fused<MODE_STEP_MACRO>(c, F, in, pnew) : launch_fused<MODE_STEP>(c, F, in, pnew);
+            if (rc) return rc;
+            c->cur = out; c->curphi = pnew; c->nsteps++;
         } else {
-            dim3 gphi = grid_for<TP>(c->P);
-            if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
-            k_phi<LG, real, TP::BX, TP::BY, TP::BZ, PHI_NPT><<<gphi, NTP, 0, c->stream>>>(
-                P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot[0]), wsp<real>(c, c->L.off_phi[pnew]));
-            c->launches++;
-            CK(cudaGetLastError());
+            rc = launch_phi(c);
+            if (rc) return rc;
             if (timed) CK(cudaEventRecord(e3[1], c->stream));
-            if (P.prescribed_u) rc = launch_main<MODE_STEP_PU>(c, F, in, pnew);   // direct kernel only
-            else rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
+            rc = launch_collide(c, macro);
+            if (rc) return rc;
         }
-        if (rc) return rc;
         if (timed) {
             CK(cudaEventRecord(e3[2], c->stream));
             for (auto e : e3) c->ev.push_back(e);
         }
-        c->cur = out; c->curphi = pnew; c->nsteps++;
         return LBM_OK;
     }
 
@@ -268,7 +294,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     }
 
     static const ImplOps *ops() {
-        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::read_macro, &Impl::read_pops, T::BX, T::BY, T::BZ};
+        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::step_phase, &Impl::read_macro, &Impl::read_pops, T::BX, T::BY, T::BZ};
         return &o;
     }
 };

@@ -27,15 +27,18 @@ __device__ __forceinline__ void store_phi_with_images(real *__restrict__ phi_pad
     for (int a = 0; a < 3; ++a) {
         cnt[a] = 1; off[a][0] = 0; kind[a][0] = BC_PERIODIC; bval[a][0] = real(0);
         if (a == 2 && !P.pz) continue;
+        // A periodic-kind face opposite a non-periodic one is the ghost side of a slab (include/lbm.h, halo): its layer has
+        // no image -- the pad layer one period away belongs to the physical face there.
+        const bool both_per = P.bc_g[a][0] == BC_PERIODIC && P.bc_g[a][1] == BC_PERIODIC;
         if (g.lo[a]) {
-            const int k = cnt[a]++;
-            if (P.bc_g[a][0] == BC_PERIODIC) { off[a][k] = (long long)len[a] * stride[a]; kind[a][k] = BC_PERIODIC; bval[a][k] = real(0); }
-            else { off[a][k] = -stride[a]; kind[a][k] = P.bc_g[a][0]; bval[a][k] = P.bc_phi[a][0]; }
+            if (P.bc_g[a][0] == BC_PERIODIC) {
+                if (both_per) { const int k = cnt[a]++; off[a][k] = (long long)len[a] * stride[a]; kind[a][k] = BC_PERIODIC; bval[a][k] = real(0); }
+            } else { const int k = cnt[a]++; off[a][k] = -stride[a]; kind[a][k] = P.bc_g[a][0]; bval[a][k] = P.bc_phi[a][0]; }
         }
         if (g.hi[a]) {
-            const int k = cnt[a]++;
-            if (P.bc_g[a][1] == BC_PERIODIC) { off[a][k] = -(long long)len[a] * stride[a]; kind[a][k] = BC_PERIODIC; bval[a][k] = real(0); }
-            else { off[a][k] = stride[a]; kind[a][k] = P.bc_g[a][1]; bval[a][k] = P.bc_phi[a][1]; }
+            if (P.bc_g[a][1] == BC_PERIODIC) {
+                if (both_per) { const int k = cnt[a]++; off[a][k] = -(long long)len[a] * stride[a]; kind[a][k] = BC_PERIODIC; bval[a][k] = real(0); }
+            } else { const int k = cnt[a]++; off[a][k] = stride[a]; kind[a][k] = P.bc_g[a][1]; bval[a][k] = P.bc_phi[a][1]; }
         }
     }
     for (int i2 = 0; i2 < cnt[2]; ++i2)

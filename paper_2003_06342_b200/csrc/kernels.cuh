@@ -54,6 +54,7 @@ template <class real> struct DevParams {
     int bc_f[3][2], bc_g[3][2], bc_s[3][2];   // BC_* per face (f: wall->BOUNCE, open->ANTI)
     real bc_phi[3][2], bc_T[3][2], bc_p[3][2];
     int nonper[3];         // axis has non-periodic faces
+    unsigned bcfaces;      // bit 2*axis + side: that face is non-periodic
     real dt, hdt, c, inv_dx, inv_dx2;
     real cs2f, cs2g, cs2s;           // e2 * c^2 per lattice
     real inv_cs2f, inv_cs2g, inv_cs2s;   // reciprocals, and c / cs2 per lattice (host-computed: no per-node divisions)
@@ -175,9 +176,12 @@ __device__ __forceinline__ bool tile_touches_bc(const DevParams<real> &P, int x0
     return false;
 #endif
     bool t = false;
-    if (P.nonper[0]) t |= (x0 == 0) || (x0 + bx >= P.nx);
-    if (P.nonper[1]) t |= (y0 == 0) || (y0 + by >= P.ny);
-    if (P.nonper[2]) t |= (z0 == 0) || (z0 + bz >= P.nz);
+    // per face (bit 2*axis + side of P.bcfaces): the ghost side of a slab is periodic-kind although the other end of the
+    // axis is a physical face
+    const unsigned m = P.bcfaces;
+    if (m & 3u) t |= (x0 == 0 && (m & 1u)) || (x0 + bx >= P.nx && (m & 2u));
+    if (m & 12u) t |= (y0 == 0 && (m & 4u)) || (y0 + by >= P.ny && (m & 8u));
+    if (m & 48u) t |= (z0 == 0 && (m & 16u)) || (z0 + bz >= P.nz && (m & 32u));
     return t;
 }
 

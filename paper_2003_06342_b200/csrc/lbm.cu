@@ -57,10 +57,27 @@ int validate(const lbm_params *p) {
             if (p->bc_f[a][s] < 0 || p->bc_f[a][s] > 2 || p->bc_g[a][s] < 0 || p->bc_g[a][s] > 2 ||
                 p->bc_s[a][s] < 0 || p->bc_s[a][s] > 2) return LBM_E_INVALID;
         }
-        const bool per = p->bc_f[a][0] == LBM_F_PERIODIC;
-        if ((p->bc_f[a][1] == LBM_F_PERIODIC) != per || (p->bc_g[a][0] == LBM_S_PERIODIC) != per ||
-            (p->bc_g[a][1] == LBM_S_PERIODIC) != per || (p->bc_s[a][0] == LBM_S_PERIODIC) != per ||
-            (p->bc_s[a][1] == LBM_S_PERIODIC) != per) return LBM_E_INVALID;
+        // a face is periodic for all three distributions or for none
+        for (int s = 0; s < 2; ++s) {
+            const bool per = p->bc_f[a][s] == LBM_F_PERIODIC;
+            if ((p->bc_g[a][s] == LBM_S_PERIODIC) != per || (p->bc_s[a][s] == LBM_S_PERIODIC) != per) return LBM_E_INVALID;
+        }
+        // both faces of an axis are periodic together, unless a ghost layer of a slab sits on the periodic side
+        const bool per0 = p->bc_f[a][0] == LBM_F_PERIODIC, per1 = p->bc_f[a][1] == LBM_F_PERIODIC;
+        const int slab_axis = three_d ? 2 : 1;
+        if (per0 != per1) {
+            if (a != slab_axis) return LBM_E_INVALID;
+            if (!(per0 ? p->halo[0] : p->halo[1])) return LBM_E_INVALID;
+        }
+    }
+    {   // ghost layers: 0 or 1 per side, on a periodic-kind face, and at least one owned layer in between
+        const int slab_axis = three_d ? 2 : 1;
+        const int len = three_d ? p->nz : p->ny;
+        for (int s = 0; s < 2; ++s) {
+            if (p->halo[s] != 0 && p->halo[s] != 1) return LBM_E_INVALID;
+            if (p->halo[s] && p->bc_f[slab_axis][s] != LBM_F_PERIODIC) return LBM_E_INVALID;
+        }
+        if (len - p->halo[0] - p->halo[1] < 1) return LBM_E_INVALID;
     }
     return LBM_OK;
 }
@@ -105,11 +122,15 @@ template <class real> DevParams<real> make_dev_params(const lbm_params *p, const
             d.bc_T[a][s] = (real)p->bc_T[a][s];
             d.bc_p[a][s] = (real)p->bc_p[a][s];
         }
-        d.nonper[a] = p->bc_f[a][0] != LBM_F_PERIODIC;
+        d.nonper[a] = p->bc_f[a][0] != LBM_F_PERIODIC || p->bc_f[a][1] != LBM_F_PERIODIC;   // one side may be a slab ghost side
         d.grav[a] = (real)p->grav[a];
         d.force[a] = (real)p->force[a];
     }
     if (p->nz == 1) d.nonper[2] = 0;
+    d.bcfaces = 0;
+    for (int a = 0; a < (p->nz == 1 ? 2 : 3); ++a)
+        for (int s = 0; s < 2; ++s)
+            if (p->bc_f[a][s] != LBM_F_PERIODIC) d.bcfaces |= 1u << (2 * a + s);
     const double c = p->dx / p->dt;
     auto e2 = [](int id) { return id == LBM_D3Q7 ? 0.25 : 1.0 / 3.0; };
     const double cs2f = e2(p->lat_f) * c * c, cs2g = e2(p->lat_g) * c * c, cs2s = e2(p->lat_s) * c * c;
@@ -266,7 +287,7 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
     }
     c->ws = static_cast<char *>(d_workspace);
     c->stream = static_cast<cudaStream_t>(cuda_stream);
-    c->cur = 0; c->curphi = 0; c->inited = false; c->nsteps = 0; c->launches = 0; c->timing = false;
+    c->cur = 0; c->curphi = 0; c->phase = 0; c->inited = false; c->nsteps = 0; c->launches = 0; c->timing = false;
     c->pd = make_dev_params<double>(p, L);
     c->pf = make_dev_params<float>(p, L);
     c->num_sms = prop.multiProcessorCount;
@@ -274,7 +295,7 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         // (90% of the measured HBM peak on config 4); LBM_VARIANT=tma selects the TMA-staged persistent kernel.
         const char *v = getenv("LBM_VARIANT");
         c->use_tma = (v && strcmp(v, "tma") == 0) && build_tma_maps(c);
-        c->fused = (v && strcmp(v, "fused") == 0) && p->nz > 1;
+        c->fused = (v && strcmp(v, "fused") == 0) && p->nz > 1 && !(p->halo[0] | p->halo[1]);   // slabs need the two phases
         const char *gr = getenv("LBM_GRAPH");   // "0" disables the CUDA-graph replay of small grids
         c->graph_ok = c->stream != nullptr && L.N <= (1ll << 21) && !(gr && strcmp(gr, "0") == 0);
         c->graph2 = nullptr; c->graph_launches = 0;
@@ -301,8 +322,16 @@ int lbm_set_velocity(lbm_ctx *c, const void *h_u) {
 
 int lbm_step(lbm_ctx *c, int n) {
     if (!c || n < 0) return LBM_E_INVALID;
-    if (!c->inited) return LBM_E_STATE;
+    if (!c->inited || (c->P.halo[0] | c->P.halo[1])) return LBM_E_STATE;   // slabs step by phases (ghost exchange in between)
     return c->ops->step(c, n);
+}
+
+int lbm_step_phase(lbm_ctx *c, int phase, int store_macros) {
+    if (!c || (phase != 0 && phase != 1)) return LBM_E_INVALID;
+    if (!c->inited || phase != c->phase) return LBM_E_STATE;
+    const int rc = c->ops->step_phase(c, phase, store_macros);
+    if (rc == LBM_OK) c->phase = 1 - phase;
+    return rc;
 }
 
 int lbm_read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T) {

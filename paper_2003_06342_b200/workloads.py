@@ -116,10 +116,11 @@ def config3_film2d(nx=512, ny=1024, h0=64.0, amp=4.0, seed=3, noise=1e-6, **over
     return P, dict(phi=phi, T=T, u=None, p=None, seed=seed, name="config3_film2d_%dx%d" % (nx, ny))
 
 
-def config4_film3d(nx=256, ny=256, nz=512, h0=32.0, amp=3.0, seed=4, **over):
+def config4_film3d(nx=256, ny=256, nz=512, h0=32.0, amp=3.0, seed=4, zrange=None, **over):
     """Config 4: 3D film boiling, x,y periodic, walls in z, heated bottom plate (configs[3]).
 
-    h(x,y) = h0 + amp/2 [cos(2 pi x/nx) + cos(2 pi y/ny)] + sum_k a_k sin(2 pi (m_k x/nx + n_k y/ny) + psi_k)."""
+    h(x,y) = h0 + amp/2 [cos(2 pi x/nx) + cos(2 pi y/ny)] + sum_k a_k sin(2 pi (m_k x/nx + n_k y/ny) + psi_k).
+    zrange = (z0, z1): return the fields of layers z0..z1-1 only (one slab of a decomposed run); P is still global."""
     P = base_params(nx, ny, nz, grav=[0.0, 0.0, -1e-5], **over)
     _film_bcs(P, 2)
     rng = np.random.Generator(np.random.PCG64(seed))
@@ -131,9 +132,12 @@ def config4_film3d(nx=256, ny=256, nz=512, h0=32.0, amp=3.0, seed=4, **over):
     h = h0 + 0.5 * amp * (np.cos(2.0 * np.pi * x / nx) + np.cos(2.0 * np.pi * y / ny))
     for k in range(8):
         h = h + a[k] * np.sin(2.0 * np.pi * (m[k] * x / nx + n[k] * y / ny) + psi[k])
-    phi = np.empty((nz, ny, nx))
-    T = np.empty((nz, ny, nx))
-    for k0 in range(0, nz, 32):  # slabs keep the temporaries small at 256x256x512
+    if zrange is not None:
+        z = z[zrange[0]:zrange[1]]
+    nzl = z.shape[0]
+    phi = np.empty((nzl, ny, nx))
+    T = np.empty((nzl, ny, nx))
+    for k0 in range(0, nzl, 32):  # chunks keep the temporaries small at 256x256x512
         zz = z[k0:k0 + 32]
         phi[k0:k0 + 32] = 0.5 * (1.0 - np.tanh(2.0 * (zz - h) / P["W"]))
         T[k0:k0 + 32] = P["T_sat"] + np.maximum(0.0, 1.0 - zz / h)

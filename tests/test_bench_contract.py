@@ -49,3 +49,9 @@ def test_our_arm_line():
     assert d["e2e"]["per_step_io"]["value"] < d["e2e"]["value"]
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+
+
+@pytest.mark.gpu
+def test_slab_overhead_line():
+    d = _run(["--workload", "config5_128", "--slabs", "2", "--steps", "4", "--warmup", "3"])
+    assert d["config"]["slabs"] == 2 and d["config"]["finite"] and d["value"] > 0
