@@ -40,7 +40,9 @@ def make_workload(name: str, seed_offset: int = 0):
         return wl.config3_film2d(seed=3 + seed_offset)
     if name.startswith("config3_"):   # e.g. config3_1024x1024, config3_4096x3072: the paper's film-boiling grids
         nx, ny = (int(v) for v in name.split("_")[1].split("x"))
-        over = {"lat_s": "D2Q9"} if name.endswith("_q9") else {}   # _q9: three D2Q9 lattices as in the paper
+        over = {"lat_s": "D2Q9"} if "_q9" in name else {}   # _q9: three D2Q9 lattices as in the paper
+        if name.endswith("_mm"):                             # _mm: 16-mode interface of the paper's 8-GPU run, Eq.(44)
+            over.update(modes=16, amp=1.0)
         return wl.config3_film2d(nx=nx, ny=ny, seed=3 + seed_offset, **over)
     if name.startswith("config5_"):
         return wl.config5_droplets(n=int(name.split("_")[1]), seed=5 + seed_offset)

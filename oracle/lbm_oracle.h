@@ -13,7 +13,12 @@
  * Readings of garbled / silent passages of the paper are the ones listed in DESIGN.md ("Readings");
  * tags G* / S* in comments refer to that list.
  *
- * Parity unpinned: discretisation of div(u phi) (S5) and the OPEN pressure face (S12).
+ * Parity unpinned: nothing outright; two READINGS the paper cannot confirm stay readings.
+ * div(u phi) (S5) is pinned as far as the paper's equations reach: u.grad(phi) by Galilean invariance of the latent-heat
+ * source, phi div u by the Eq.(11a) mass balance; only "pointwise product, not a stencil divergence" is a choice.
+ * The OPEN pressure face (S12, not in the paper) is pinned in the role config 2 gives it -- normal outflow at a fixed
+ * pressure: exact hydrostatic column, outflow = integrated mass source; its behaviour under shear is not (a 32 x 16
+ * pressure-driven channel carries 6.5 % more flux than Poiseuille's law, entry effect of the plain anti-bounce-back).
  * The 3D coupling terms (not run in 3D by the paper) are pinned by the spherical Laplace law,
  * the symmetry tests and the brute-force comparison; everything else by tests/test_oracle_*.py.
  */

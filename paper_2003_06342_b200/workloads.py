@@ -104,13 +104,23 @@ def _film_bcs(P, axis):
     P["bc_T"][axis] = [P["T_sat"] + 1.0, P["T_sat"]]
 
 
-def config3_film2d(nx=512, ny=1024, h0=64.0, amp=4.0, seed=3, noise=1e-6, **over):
-    """Config 3: 2D film boiling, x periodic, no-slip walls bottom/top, heated bottom wall (configs[2])."""
+def config3_film2d(nx=512, ny=1024, h0=64.0, amp=4.0, seed=3, noise=1e-6, modes=0, **over):
+    """Config 3: 2D film boiling, x periodic, no-slip walls bottom/top, heated bottom wall (configs[2]).
+
+    modes = 0: single-mode interface Eq.(42), one period across the box.  modes = m > 0: the multi-mode
+    interface of the paper's 4096 x 3072 run, Eq.(44): h = h0 + amp sum_i sin(2 pi x / lambda_i) with m
+    wavelengths drawn uniformly from [0.5, 1.5 sqrt(3)] lambda_c, lambda_c = 2 pi sqrt(sigma / ((rho_l - rho_g) g))
+    (PAPER.md:526)."""
     P = base_params(nx, ny, 1, grav=[0.0, -1e-5, 0.0], **over)
     _film_bcs(P, 1)
     rng = np.random.Generator(np.random.PCG64(seed))
     x, y, _ = _coords(P)
-    h = h0 + amp * np.sin(2.0 * np.pi * x / nx)
+    if modes > 0:
+        lam_c = 2.0 * np.pi * math.sqrt(P["sigma"] / ((P["rho_l"] - P["rho_g"]) * abs(P["grav"][1])))
+        lam = rng.uniform(0.5 * lam_c, 1.5 * math.sqrt(3.0) * lam_c, size=modes)
+        h = h0 + amp * sum(np.sin(2.0 * np.pi * x / l) for l in lam)
+    else:
+        h = h0 + amp * np.sin(2.0 * np.pi * x / nx)
     phi = 0.5 * (1.0 - np.tanh(2.0 * (y - h) / P["W"])) + _noise(rng, (1, ny, nx), noise)
     T = P["T_sat"] + np.maximum(0.0, 1.0 - y / h)
     return P, dict(phi=phi, T=T, u=None, p=None, seed=seed, name="config3_film2d_%dx%d" % (nx, ny))
