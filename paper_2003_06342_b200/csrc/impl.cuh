@@ -10,18 +10,20 @@
 
 namespace lbm {
 
-// tiles of nodes per CTA (one node per thread, 256 threads).  A warp is one x-row.  Wide tiles (long contiguous
-// x-runs: fewer partially used sectors on the x-shifted pulls) are 3.5% faster on config 4 and are used when the
-// row is long enough; narrow tiles keep small grids busy.
-// wide tiles only when the ragged last tile wastes at most 4% of the threads (192 = 128 + 64 would idle 25%)
+// Tiles of nodes per CTA (one node per thread).  A warp is one x-row.  Wide tiles (long contiguous x-runs: fewer partially
+// used sectors on the x-shifted pulls) are 3.5% faster on config 4 and are used when the row is long enough; narrow tiles
+// keep small grids busy.  Wide tiles only when the ragged last tile wastes at most 4% of the threads (192 = 128 + 64
+// would idle 25%).
 inline bool wide_tile_pays(int nx) { return nx >= 128 && ((nx + 127) / 128 * 128 - nx) * 25 <= nx; }
 
-// K_main runs 128-thread CTAs on wide tiles (4 per SM in fp64: 3.3% faster than 2 x 256 threads on config 4); K_phi and
-// the utility kernels keep 256 threads (PhiTile).
-struct TileWide3Phi { static constexpr int BX = 128, BY = 2, BZ = 1; using PhiTile = TileWide3Phi; };   // also K_main's tile in fp32
+// K_phi and the utility kernels always run 256-thread tiles (PhiTile).  K_main on wide tiles runs 128-thread CTAs, one
+// x-row each (finer CTA turnover at the same number of warps: +3% fp64 3D, +7% fp64 2D, +7% fp32 2D), except in fp32 3D
+// where 128 x 2 is faster (measured).
+struct TileWide3Phi { static constexpr int BX = 128, BY = 2, BZ = 1; using PhiTile = TileWide3Phi; };   // fp32 3D K_main too
 struct TileWide3 { static constexpr int BX = 128, BY = 1, BZ = 1; using PhiTile = TileWide3Phi; };
 struct TileNarrow3 { static constexpr int BX = 32, BY = 4, BZ = 2; using PhiTile = TileNarrow3; };
 struct TileWide2 { static constexpr int BX = 128, BY = 2, BZ = 1; using PhiTile = TileWide2; };
+struct TileWide2K { static constexpr int BX = 128, BY = 1, BZ = 1; using PhiTile = TileWide2; };
 struct TileNarrow2 { static constexpr int BX = 32, BY = 8, BZ = 1; using PhiTile = TileNarrow2; };
 
 template <class real> const DevParams<real> &dev_params(const lbm_ctx *c);
@@ -39,13 +41,16 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     static constexpr int NT = T::BX * T::BY * T::BZ;
     using TP = typename T::PhiTile;                       // tile of K_phi and of the utility kernels
     static constexpr int NTP = TP::BX * TP::BY * TP::BZ;
-    // resident CTAs per SM the register allocation is bounded for (measured on config 4): fp64 2 x 256 threads at 128
-    // registers; fp32 4 x 256 at 64 registers (+25% over 2 CTAs although a few values spill)
-#ifndef LBM_MINB3D
-#define LBM_MINB3D (2 * 256 / NT)
+    // Threads per SM the register allocation is bounded for (__launch_bounds__ minimum CTAs = threads / NT), measured:
+    //   fp64 3D: 512 (128 registers, no spill on the interior path); more spills cost more than the warps bring
+    //   fp64 2D, 128-thread CTAs: 896 with the D2Q5 heat lattice (72 registers), 640 with D2Q9 (96); 256-thread tiles 768
+    //   fp32   : 1024 (64 registers; +25% over 512 although a few values spill); 2D 128-thread CTAs 1280 (48 registers)
+#ifndef LBM_THREADS3D
+#define LBM_THREADS3D 512
 #endif
-    // fp64 2D: 3 x 256 threads at 80 registers (+5% on 4096 x 3072 over 2 CTAs)
-    static constexpr int MINB = sizeof(real) == 8 ? (D == 2 ? 3 * 256 / NT : LBM_MINB3D) : 4 * 256 / NT;
+    static constexpr int THREADS64 = D == 3 ? LBM_THREADS3D : (NT == 128 ? (LS::Q == 5 ? 896 : 640) : 768);
+    static constexpr int THREADS32 = (D == 2 && NT == 128) ? 1280 : 1024;
+    static constexpr int MINB = (sizeof(real) == 8 ? THREADS64 : THREADS32) / NT;
 #ifndef LBM_PHI_NPT
 #define LBM_PHI_NPT 2
 #endif

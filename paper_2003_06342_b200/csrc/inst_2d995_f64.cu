@@ -4,7 +4,7 @@
 
 namespace lbm {
 const ImplOps *ops_2d995_f64(int nx) {
-    if (wide_tile_pays(nx)) return Impl<D2Q9, D2Q9, D2Q5, double, TileWide2>::ops();
+    if (wide_tile_pays(nx)) return Impl<D2Q9, D2Q9, D2Q5, double, TileWide2K>::ops();
     return Impl<D2Q9, D2Q9, D2Q5, double, TileNarrow2>::ops();
 }
 }  // namespace lbm

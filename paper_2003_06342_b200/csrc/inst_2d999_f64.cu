@@ -4,7 +4,7 @@
 
 namespace lbm {
 const ImplOps *ops_2d999_f64(int nx) {
-    if (wide_tile_pays(nx)) return Impl<D2Q9, D2Q9, D2Q9, double, TileWide2>::ops();
+    if (wide_tile_pays(nx)) return Impl<D2Q9, D2Q9, D2Q9, double, TileWide2K>::ops();
     return Impl<D2Q9, D2Q9, D2Q9, double, TileNarrow2>::ops();
 }
 }  // namespace lbm
