@@ -32,6 +32,8 @@ FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback when
 def make_workload(name: str, seed_offset: int = 0):
     if name == "config4":
         return wl.config4_film3d(seed=4 + seed_offset)
+    if name == "config4_q15":        # same grid and recipe with the paper's D3Q15 Navier-Stokes lattice
+        return wl.config4_film3d(seed=4 + seed_offset, lat_f="D3Q15")
     if name == "config4_sample":     # bounded sample of config 4 for the CPU oracle: same recipe, a 256x256x128 slab
         return wl.config4_film3d(nx=256, ny=256, nz=128, seed=4 + seed_offset)
     if name == "config4_small":      # the reference arm's per-step sample (128^3)
@@ -238,7 +240,7 @@ def run_ours(args):
         return 0
 
     # ---- roofline of the dominant kernel (K_main), algorithmic bytes / live CUDA-event duration
-    q = {"D2Q5": 5, "D2Q9": 9, "D3Q7": 7, "D3Q19": 19}
+    q = {"D2Q5": 5, "D2Q9": 9, "D3Q7": 7, "D3Q19": 19, "D3Q15": 15}
     Q = q[P["lat_f"]] + q[P["lat_g"]] + q[P["lat_s"]]
     main_vals = (Q + 3) + (Q + 1)                    # reads: pops, phi^{n+1}, phi^n, Pdot; writes: pops, Pdot
     phi_vals = q[P["lat_g"]] + 1 + 1

@@ -30,7 +30,7 @@ extern "C" {
 #endif
 
 /* lattices, PAPER.md:190 (D2Q5 is not in the paper: DESIGN.md reading S1) */
-enum { LBM_D2Q5 = 0, LBM_D2Q9 = 1, LBM_D3Q7 = 2, LBM_D3Q19 = 3 };
+enum { LBM_D2Q5 = 0, LBM_D2Q9 = 1, LBM_D3Q7 = 2, LBM_D3Q19 = 3, LBM_D3Q15 = 4 };
 
 /* boundary rule of f on a face */
 enum {
@@ -73,7 +73,7 @@ enum {
 /*
  * Problem description; plain data, copied by lbm_create.
  * nz == 1 selects 2D (lattices must be D2Q*), nz > 1 selects 3D (D3Q*).
- * Supported lattice sets (f, g, s): (D2Q9, D2Q9, D2Q5), (D2Q9, D2Q9, D2Q9), (D3Q19, D3Q7, D3Q7).
+ * Supported lattice sets (f, g, s): (D2Q9, D2Q9, D2Q5), (D2Q9, D2Q9, D2Q9), (D3Q19, D3Q7, D3Q7), (D3Q15, D3Q7, D3Q7).
  * bc_*[axis][side]: axis 0,1,2 = x,y,z; side 0 = low face, 1 = high face.  A periodic face must be
  * periodic on both sides and for all three distributions (except next to a ghost layer, see halo).
  * Walls sit half a cell outside the first/last node (node i is at (i + 1/2) dx).

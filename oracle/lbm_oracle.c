@@ -98,6 +98,18 @@ static int make_lattice(int id, lattice_t *L)
         set_e(L, 15, 0, 1, 1, 1.0 / 36.0); set_e(L, 16, 0, -1, 1, 1.0 / 36.0);
         set_e(L, 17, 0, 1, -1, 1.0 / 36.0); set_e(L, 18, 0, -1, -1, 1.0 / 36.0);
         break;
+    case ORA_D3Q15:
+        /* e7 = (1,1,1), e8 = (-1,1,1), "...", e14 = (1,-1,-1); the elided ones are taken counter-clockwise
+         * around z on each level, which ends on the printed e14 (reading G10).  w0 = 2/9, w1..6 = 1/9, w7..14 = 1/72. */
+        L->Q = 15; L->e2 = 1.0 / 3.0;
+        set_e(L, 0, 0, 0, 0, 2.0 / 9.0);
+        set_e(L, 1, 1, 0, 0, 1.0 / 9.0); set_e(L, 2, 0, 1, 0, 1.0 / 9.0); set_e(L, 3, 0, 0, 1, 1.0 / 9.0);
+        set_e(L, 4, -1, 0, 0, 1.0 / 9.0); set_e(L, 5, 0, -1, 0, 1.0 / 9.0); set_e(L, 6, 0, 0, -1, 1.0 / 9.0);
+        set_e(L, 7, 1, 1, 1, 1.0 / 72.0); set_e(L, 8, -1, 1, 1, 1.0 / 72.0);
+        set_e(L, 9, -1, -1, 1, 1.0 / 72.0); set_e(L, 10, 1, -1, 1, 1.0 / 72.0);
+        set_e(L, 11, 1, 1, -1, 1.0 / 72.0); set_e(L, 12, -1, 1, -1, 1.0 / 72.0);
+        set_e(L, 13, -1, -1, -1, 1.0 / 72.0); set_e(L, 14, 1, -1, -1, 1.0 / 72.0);
+        break;
     default:
         return -1;
     }
@@ -132,7 +144,7 @@ int oracle_num_threads(void)
 #endif
 }
 
-static int lattice_is_3d(int id) { return id == ORA_D3Q7 || id == ORA_D3Q19; }
+static int lattice_is_3d(int id) { return id == ORA_D3Q7 || id == ORA_D3Q19 || id == ORA_D3Q15; }
 
 static long idx(const oracle_ctx *c, int x, int y, int z)
 {

@@ -30,7 +30,7 @@ extern "C" {
 #endif
 
 /* lattice ids (D2Q5 is not in the paper, reading S1) */
-enum { ORA_D2Q5 = 0, ORA_D2Q9 = 1, ORA_D3Q7 = 2, ORA_D3Q19 = 3 };
+enum { ORA_D2Q5 = 0, ORA_D2Q9 = 1, ORA_D3Q7 = 2, ORA_D3Q19 = 3, ORA_D3Q15 = 4 };
 /* boundary kinds of the Navier-Stokes distribution f, per face */
 enum { ORA_F_PERIODIC = 0, ORA_F_WALL = 1 /* half bounce-back */,
        ORA_F_OPEN = 2 /* pressure anti-bounce-back, reading S12 */ };

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SRC_DIR = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblbm_b200.so")
 SOURCES = ["lbm.cu", "halo.cu", "inst_2d995_f64.cu", "inst_2d995_f32.cu", "inst_2d999_f64.cu", "inst_2d999_f32.cu",
-           "inst_3d_f64.cu", "inst_3d_f32.cu"]
+           "inst_3d_f64.cu", "inst_3d_f32.cu", "inst_3d15_f64.cu", "inst_3d15_f32.cu"]
 DEPS = SOURCES + ["ctx.h", "impl.cuh", "kernels.cuh", "k_phi.cuh", "k_main.cuh", "k_main_tma.cuh", "k_main_phitma.cuh", "k_main_fused.cuh", "lattices.cuh",
                   os.path.join("..", "..", "include", "lbm.h")]
 NVCC_COMPILE = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xptxas", "-v",

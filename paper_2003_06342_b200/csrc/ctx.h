@@ -21,7 +21,7 @@ extern int g_last_cuda_error;
         if (e_ != cudaSuccess) { lbm::g_last_cuda_error = (int)e_; return LBM_E_CUDA; } \
     } while (0)
 
-enum LatSet { SET_NONE = 0, SET_2D_995, SET_2D_999, SET_3D_1977 };
+enum LatSet { SET_NONE = 0, SET_2D_995, SET_2D_999, SET_3D_1977, SET_3D_1577 };
 
 struct Layout {
     long long N;
@@ -42,6 +42,8 @@ struct ImplOps {
 
 // defined in inst_*.cu (compiled in parallel); nx selects the tile shape
 const ImplOps *ops_2d995_f64(int nx);
+const ImplOps *ops_3d15_f64(int nx);
+const ImplOps *ops_3d15_f32(int nx);
 const ImplOps *ops_2d995_f32(int nx);
 const ImplOps *ops_2d999_f64(int nx);
 const ImplOps *ops_2d999_f32(int nx);

@@ -77,6 +77,11 @@ bool make_plan(const lbm_ctx *c, int what, int side, bool ghost, HaloPlan &pl) {
         add_pops<D3Q7>(pl, c, c->L.off_g[c->cur], axis, dir, layer, es);
         add_pops<D3Q7>(pl, c, c->L.off_s[c->cur], axis, dir, layer, es);
         break;
+    case SET_3D_1577:
+        add_pops<D3Q15>(pl, c, c->L.off_f[c->cur], axis, dir, layer, es);
+        add_pops<D3Q7>(pl, c, c->L.off_g[c->cur], axis, dir, layer, es);
+        add_pops<D3Q7>(pl, c, c->L.off_s[c->cur], axis, dir, layer, es);
+        break;
     default: return false;
     }
     return pl.count > 0 && pl.count <= HALO_MAX_REGIONS;

@@ -13,8 +13,8 @@ namespace lbm {
 // Tiles of nodes per CTA (one node per thread).  A warp is one x-row.  Wide tiles (long contiguous x-runs: fewer partially
 // used sectors on the x-shifted pulls) are 3.5% faster on config 4 and are used when the row is long enough; narrow tiles
 // keep small grids busy.  Wide tiles only when the ragged last tile wastes at most 4% of the threads (192 = 128 + 64
-// would idle 25%).
-inline bool wide_tile_pays(int nx) { return nx >= 128 && ((nx + 127) / 128 * 128 - nx) * 25 <= nx; }
+// would idle 25%; a 192-wide tile on nx = 192 measured 9% SLOWER than the narrow tile).
+inline bool wide_tile_pays(int nx, int bx = 128) { return nx >= bx && ((nx + bx - 1) / bx * bx - nx) * 25 <= nx; }
 
 // K_phi and the utility kernels always run 256-thread tiles (PhiTile).  K_main on wide tiles runs 128-thread CTAs, one
 // x-row each (finer CTA turnover at the same number of warps: +3% fp64 3D, +7% fp64 2D, +7% fp32 2D), except in fp32 3D

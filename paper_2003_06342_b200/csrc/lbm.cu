@@ -27,15 +27,16 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 int lattice_q(int id) {
-    switch (id) { case LBM_D2Q5: return 5; case LBM_D2Q9: return 9; case LBM_D3Q7: return 7; case LBM_D3Q19: return 19; }
+    switch (id) { case LBM_D2Q5: return 5; case LBM_D2Q9: return 9; case LBM_D3Q7: return 7; case LBM_D3Q19: return 19; case LBM_D3Q15: return 15; }
     return 0;
 }
-bool lattice_3d(int id) { return id == LBM_D3Q7 || id == LBM_D3Q19; }
+bool lattice_3d(int id) { return id == LBM_D3Q7 || id == LBM_D3Q19 || id == LBM_D3Q15; }
 
 LatSet lattice_set(const lbm_params *p) {
     if (p->lat_f == LBM_D2Q9 && p->lat_g == LBM_D2Q9 && p->lat_s == LBM_D2Q5) return SET_2D_995;
     if (p->lat_f == LBM_D2Q9 && p->lat_g == LBM_D2Q9 && p->lat_s == LBM_D2Q9) return SET_2D_999;
     if (p->lat_f == LBM_D3Q19 && p->lat_g == LBM_D3Q7 && p->lat_s == LBM_D3Q7) return SET_3D_1977;
+    if (p->lat_f == LBM_D3Q15 && p->lat_g == LBM_D3Q7 && p->lat_s == LBM_D3Q7) return SET_3D_1577;
     return SET_NONE;
 }
 
@@ -282,6 +283,7 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         case SET_2D_995: c->ops = d ? ops_2d995_f64(p->nx) : ops_2d995_f32(p->nx); break;
         case SET_2D_999: c->ops = d ? ops_2d999_f64(p->nx) : ops_2d999_f32(p->nx); break;
         case SET_3D_1977: c->ops = d ? ops_3d_f64(p->nx) : ops_3d_f32(p->nx); break;
+        case SET_3D_1577: c->ops = d ? ops_3d15_f64(p->nx) : ops_3d15_f32(p->nx); break;
         default: delete c; return LBM_E_UNSUPPORTED;
         }
     }

@@ -180,7 +180,7 @@ def bytes_per_lu(P, itemsize=8, macros=False):
 
     K_phi: Q_g + 1 reads, 1 write.  K_main: Q_f + Q_g + Q_s + 3 reads (phi^{n+1}, phi^n, Pdot),
     Q_f + Q_g + Q_s + 1 writes (+5 or +4 when u, p, T are written)."""
-    q = {"D2Q5": 5, "D2Q9": 9, "D3Q7": 7, "D3Q19": 19}
+    q = {"D2Q5": 5, "D2Q9": 9, "D3Q7": 7, "D3Q19": 19, "D3Q15": 15}
     Q = q[P["lat_f"]] + q[P["lat_g"]] + q[P["lat_s"]]
     vals = (q[P["lat_g"]] + 1 + 1) + (Q + 3) + (Q + 1)
     if macros:

@@ -17,6 +17,7 @@ _SHELL_W = {
     "D2Q9": (2, {0: 4 / 9, 1: 1 / 9, 2: 1 / 36}),
     "D3Q7": (3, {0: 1 / 4, 1: 1 / 8}),
     "D3Q19": (3, {0: 1 / 3, 1: 1 / 18, 2: 1 / 36}),
+    "D3Q15": (3, {0: 2 / 9, 1: 1 / 9, 3: 1 / 72}),
 }
 
 

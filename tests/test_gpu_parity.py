@@ -250,6 +250,47 @@ def test_tma_variant(gpu, oracle_mod, monkeypatch):
     _run_parity(gpu, oracle_mod, P, _random_state(P, 33), [1, 12], label="tma 2d periodic")
 
 
+# ---------------------------------------------------------------------------- D3Q15 Navier-Stokes lattice
+def _d3q15_cases():
+    P1 = wl.base_params(136, 10, 7, lat_f="D3Q15", grav=[1e-4, -1e-4, -2e-4], force=[1e-5, 0.0, 2e-5])   # wide tiles, ragged
+    P2 = wl.base_params(40, 9, 12, lat_f="D3Q15", grav=[0.0, 0.0, -1e-4])                                # narrow tiles, z walls
+    P2["bc_f"][2] = ["wall", "wall"]; P2["bc_g"][2] = ["zeroflux", "zeroflux"]; P2["bc_s"][2] = ["dirichlet", "dirichlet"]
+    P2["bc_T"][2] = [1.0, 0.0]
+    P3 = wl.base_params(12, 9, 8, lat_f="D3Q15")                 # walls on all axes: corner links leave through two faces
+    for a in range(3):
+        P3["bc_f"][a] = ["wall", "open" if a == 0 else "wall"]; P3["bc_g"][a] = ["dirichlet", "zeroflux"]
+        P3["bc_s"][a] = ["dirichlet", "zeroflux"]; P3["bc_phi"][a] = [0.9, 0.0]; P3["bc_T"][a] = [0.2, 0.0]
+    return P1, P2, P3
+
+
+def test_d3q15_lattice_set(gpu, oracle_mod):
+    P1, P2, P3 = _d3q15_cases()
+    _run_parity(gpu, oracle_mod, P1, _random_state(P1, 71), [1, 2, 15], label="D3Q15 periodic")
+    _run_parity(gpu, oracle_mod, P2, _random_state(P2, 72), [1, 15], label="D3Q15 z walls")
+    _run_parity(gpu, oracle_mod, P3, _random_state(P3, 73), [1, 3], label="D3Q15 box")
+    Pc, I = wl.config4_film3d(nx=48, ny=40, nz=64, h0=12.0, amp=2.0, lat_f="D3Q15")
+    _run_parity(gpu, oracle_mod, Pc, (I["phi"], I["T"]), [1, 100], pops=False, label="D3Q15 config4 48x40x64")
+
+
+@pytest.mark.parametrize("env", [("LBM_PHI", "ldg"), ("LBM_VARIANT", "tma"), ("LBM_VARIANT", "fused")])
+def test_d3q15_variants(gpu, oracle_mod, monkeypatch, env):
+    monkeypatch.setenv(*env)
+    P1, P2, _ = _d3q15_cases()
+    _run_parity(gpu, oracle_mod, P1, _random_state(P1, 74), [1, 8], label="D3Q15 periodic %s" % env[1])
+    _run_parity(gpu, oracle_mod, P2, _random_state(P2, 75), [1, 8], label="D3Q15 z walls %s" % env[1])
+
+
+def test_d3q15_fp32(gpu, oracle_mod):
+    P1, _, _ = _d3q15_cases()
+    init = _random_state(P1, 76)
+    o = oracle_mod.Oracle(P1); o.init(*init); o.step(10)
+    sim = gpu.LBM(P1, 32); sim.init(*init); sim.step(10)
+    for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
+        scale = max(np.abs(b).max(), 1e-3)
+        assert np.abs(a - b).max() <= REL32 * scale, (name, np.abs(a - b).max(), scale)
+    sim.destroy(); o.close()
+
+
 # ---------------------------------------------------------------------------- the five configs (bounded horizons)
 def test_config1_droplet_1000_steps(gpu, oracle_mod):
     P, I = wl.config1_droplet()

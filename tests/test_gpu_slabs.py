@@ -85,6 +85,11 @@ def test_periodic_box_3d(gpu, oracle_mod):
     _check(gpu, oracle_mod, P, _random_state(P, 61), [1, 2, 5], [1, 6])
 
 
+def test_d3q15_slabs(gpu, oracle_mod):
+    P, st = wl.config4_film3d(40, 24, 14, h0=5.0, amp=1.5, lat_f="D3Q15")
+    _check(gpu, oracle_mod, P, (st["phi"], st["T"], None, None), [3], [1, 6], exact=False)
+
+
 def test_film_2d_cut_along_y(gpu, oracle_mod):
     P, st = wl.config3_film2d(40, 30, h0=8.0, amp=2.0)
     _check(gpu, oracle_mod, P, (st["phi"], st["T"], None, None), [2, 4], [1, 12], exact=False)

@@ -112,12 +112,21 @@ def test_2d_prescribed_velocity(oracle_mod):
     _compare(oracle_mod, P, 10, 19)
 
 
+def test_3d_d3q15_navier_stokes_lattice(oracle_mod):
+    P = wl.base_params(6, 7, 8, lat_f="D3Q15", grav=[1e-4, -2e-4, 5e-5])
+    _compare(oracle_mod, P, 10, 20)
+    P = wl.base_params(8, 6, 7, lat_f="D3Q15", grav=[0.0, 0.0, -1e-4])
+    P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
+    P["bc_T"][2] = [1.0, 0.0]
+    _compare(oracle_mod, P, 8, 21)
+
+
 def test_3d_flags_off(oracle_mod):
     P = wl.base_params(6, 8, 6, phase_change=False, latent_heat=False)
     _compare(oracle_mod, P, 10, 18)
 
 
-@pytest.mark.parametrize("name", ["D2Q5", "D2Q9", "D3Q7", "D3Q19"])
+@pytest.mark.parametrize("name", ["D2Q5", "D2Q9", "D3Q7", "D3Q19", "D3Q15"])
 def test_lattice_tables(oracle_mod, name):
     """Weights sum to 1, first moment 0, second moment e2 * identity, opposite pairs present; the typed
     tables of the oracle equal the generated shells of the NumPy model as sets."""
@@ -131,4 +140,11 @@ def test_lattice_tables(oracle_mod, name):
     e_n, w_n, e2_n = make_lattice(name)
     assert abs(e2 - e2_n) < 1e-15
     assert {tuple(v) + (round(ww, 12),) for v, ww in zip(e, w)} == {tuple(v) + (round(ww, 12),) for v, ww in zip(e_n, w_n)}
-    assert abs(e2 - {"D2Q5": 1 / 3, "D2Q9": 1 / 3, "D3Q7": 1 / 4, "D3Q19": 1 / 3}[name]) < 1e-15
+    assert abs(e2 - {"D2Q5": 1 / 3, "D2Q9": 1 / 3, "D3Q7": 1 / 4, "D3Q19": 1 / 3, "D3Q15": 1 / 3}[name]) < 1e-15
+    if name in ("D2Q9", "D3Q19", "D3Q15"):     # Navier-Stokes lattices: isotropic fourth moment e2^2 (dd + dd + dd)
+        m4 = np.einsum("i,ia,ib,ic,id->abcd", w, *(e.astype(float),) * 4)
+        d = np.eye(3)
+        iso = e2 * e2 * (np.einsum("ab,cd->abcd", d, d) + np.einsum("ac,bd->abcd", d, d) + np.einsum("ad,bc->abcd", d, d))
+        assert np.abs(m4[:dim, :dim, :dim, :dim] - iso[:dim, :dim, :dim, :dim]).max() < 1e-15
+    if name == "D3Q15":                         # the two direction vectors the paper prints
+        assert tuple(e[7]) == (1, 1, 1) and tuple(e[8]) == (-1, 1, 1) and tuple(e[14]) == (1, -1, -1)

@@ -239,19 +239,21 @@ def test_layered_poiseuille_viscosity_contrast(oracle_mod):
     assert abs(printed[0]) > 0.3 * exact.max()          # the printed branch labels do not even vanish at the wall
 
 
-def test_laplace_pressure_jump_3d_sphere(oracle_mod):
+@pytest.mark.parametrize("lat_f,n,R,steps,lo,hi", [("D3Q19", 32, 9.0, 1200, 0.92, 0.99), ("D3Q15", 24, 7.0, 900, 0.88, 0.99)])
+def test_laplace_pressure_jump_3d_sphere(oracle_mod, lat_f, n, R, steps, lo, hi):
     """3D analogue of P4 for the coupling terms the paper did not run in 3D: a spherical liquid drop at
     rest obeys p_in - p_out = 2 sigma / R (mean curvature 2/R; Eq.39 is the 2D form sigma/R).  Pins F_s = mu_phi grad phi,
-    mu_phi and the D3Q19 directional-derivative stencils (Eq.13, 14, 35, 36) with D3Q19 + D3Q7 + D3Q7 lattices."""
-    n, R, W = 32, 9.0, 4.0
-    P = wl.base_params(n, n, n, W=W, nu_l=0.2, nu_g=0.2, phase_change=False, latent_heat=False)
+    mu_phi and the directional-derivative stencils (Eq.13, 14, 35, 36) on the NS lattice: D3Q19 (measured 0.952) and
+    D3Q15, whose stencil runs along the cube diagonals (measured 0.968 at R = 7)."""
+    W = 4.0
+    P = wl.base_params(n, n, n, W=W, nu_l=0.2, nu_g=0.2, phase_change=False, latent_heat=False, lat_f=lat_f)
     c = np.arange(n) + 0.5
     z, y, x = np.meshgrid(c, c, c, indexing="ij")
     r = np.sqrt((x - n / 2) ** 2 + (y - n / 2) ** 2 + (z - n / 2) ** 2)
     phi0 = 0.5 * (1 - np.tanh(2 * (R - r) / W))
     o = oracle_mod.Oracle(P)
     o.init(phi0)
-    o.step(1200)
+    o.step(steps)
     acc = []
     for _ in range(6):
         o.step(50)
@@ -260,7 +262,7 @@ def test_laplace_pressure_jump_3d_sphere(oracle_mod):
     phi, u, _, _ = o.read_macro()
     o.close()
     ratio = np.mean(acc) / (2 * P["sigma"] / R)
-    assert 0.92 < ratio < 0.99, ratio                  # 0.952 measured; sigma/R (the 2D law) would read 0.476
+    assert lo < ratio < hi, ratio                      # sigma/R (the 2D law) would read half of it
     assert np.abs(u).max() < 5e-6
     assert abs(phi.sum() - phi0.sum()) / phi0.sum() < 1e-12
 
