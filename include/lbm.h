@@ -123,7 +123,10 @@ size_t lbm_workspace_bytes(const lbm_params *p);
  * (owned by the library; release with lbm_destroy). */
 int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_stream, lbm_ctx **out);
 
-/* Set the state of time level 0 from HOST arrays (element type = precision).  h_phi is required; h_T, h_u,
+/* Pointer arguments named h_* below are HOST pointers or, equally, DEVICE pointers of the context's device: the copies use
+ * unified addressing (cudaMemcpyDefault), so a caller that keeps its fields on the GPU passes them directly.
+ *
+ * Set the state of time level 0 from HOST arrays (element type = precision).  h_phi is required; h_T, h_u,
  * h_p may be NULL (T = T_sat, u = 0, p = 0).  Sets dphi/dt = 0, the production field from the initial macros
  * (Eq.18) and the populations to bar-equilibrium theta_eq - dt/2 S (Eq.24; DESIGN.md reading
  * S9), then collides once so that the stored state is post-collision at level 0.  Resets the step counter.

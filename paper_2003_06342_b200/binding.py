@@ -134,7 +134,8 @@ def lbm_workspace_bytes(P: dict, precision: int = 64) -> int:
 
 
 def _host_ptr(a, dtype, shape, name):
-    """Pointer to a host array: numpy array or CPU torch tensor (pinned or not), contiguous, right dtype/shape."""
+    """Pointer to a numpy array or a torch tensor (CPU, pinned or not, or CUDA: the library copies with unified
+    addressing), contiguous, right dtype/shape."""
     if a is None:
         return None, None
     if isinstance(a, np.ndarray):
@@ -144,13 +145,13 @@ def _host_ptr(a, dtype, shape, name):
         return b.ctypes.data, b
     import torch
     if isinstance(a, torch.Tensor):
-        if a.device.type != "cpu" or not a.is_contiguous() or tuple(a.shape) != tuple(shape):
-            raise ValueError("%s: need a contiguous CPU tensor of shape %s" % (name, shape))
+        if not a.is_contiguous() or tuple(a.shape) != tuple(shape):
+            raise ValueError("%s: need a contiguous tensor of shape %s" % (name, shape))
         want = torch.float64 if dtype == np.float64 else torch.float32
         if a.dtype != want:
             raise ValueError("%s: dtype %s, expected %s" % (name, a.dtype, want))
         return a.data_ptr(), a
-    raise TypeError("%s: numpy array or CPU torch tensor expected" % name)
+    raise TypeError("%s: numpy array or torch tensor expected" % name)
 
 
 class LBM:

@@ -111,17 +111,17 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         const size_t N = (size_t)c->L.N, es = sizeof(real);
         const DevParams<real> &P = dev_params<real>(c);
         real *scratch = wsp<real>(c, c->L.off_scratch);
-        CK(cudaMemcpyAsync(scratch, h_phi, N * es, cudaMemcpyHostToDevice, c->stream));
+        CK(cudaMemcpyAsync(scratch, h_phi, N * es, cudaMemcpyDefault, c->stream));
         real *dT = wsp<real>(c, c->L.off_T), *du = wsp<real>(c, c->L.off_u), *dp = wsp<real>(c, c->L.off_p);
-        if (h_T) CK(cudaMemcpyAsync(dT, h_T, N * es, cudaMemcpyHostToDevice, c->stream));
+        if (h_T) CK(cudaMemcpyAsync(dT, h_T, N * es, cudaMemcpyDefault, c->stream));
         else {
             k_fill<real><<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(dT, (long long)N, (real)c->P.T_sat);
             c->launches++;
             CK(cudaGetLastError());
         }
-        if (h_u) CK(cudaMemcpyAsync(du, h_u, 3 * N * es, cudaMemcpyHostToDevice, c->stream));
+        if (h_u) CK(cudaMemcpyAsync(du, h_u, 3 * N * es, cudaMemcpyDefault, c->stream));
         else CK(cudaMemsetAsync(du, 0, 3 * N * es, c->stream));
-        if (h_p) CK(cudaMemcpyAsync(dp, h_p, N * es, cudaMemcpyHostToDevice, c->stream));
+        if (h_p) CK(cudaMemcpyAsync(dp, h_p, N * es, cudaMemcpyDefault, c->stream));
         else CK(cudaMemsetAsync(dp, 0, N * es, c->stream));
         for (int b = 0; b < 2; ++b)
             CK(cudaMemsetAsync(wsp<real>(c, c->L.off_phi[b]), 0, c->L.phi_pad_elems * es, c->stream));
@@ -261,11 +261,11 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
                 dev_params<real>(c), wsp<real>(c, c->L.off_phi[c->curphi]), scratch);
             c->launches++;
             CK(cudaGetLastError());
-            CK(cudaMemcpyAsync(h_phi, scratch, N * es, cudaMemcpyDeviceToHost, c->stream));
+            CK(cudaMemcpyAsync(h_phi, scratch, N * es, cudaMemcpyDefault, c->stream));
         }
-        if (h_u) CK(cudaMemcpyAsync(h_u, wsp<real>(c, c->L.off_u), 3 * N * es, cudaMemcpyDeviceToHost, c->stream));
-        if (h_p) CK(cudaMemcpyAsync(h_p, wsp<real>(c, c->L.off_p), N * es, cudaMemcpyDeviceToHost, c->stream));
-        if (h_T) CK(cudaMemcpyAsync(h_T, wsp<real>(c, c->L.off_T), N * es, cudaMemcpyDeviceToHost, c->stream));
+        if (h_u) CK(cudaMemcpyAsync(h_u, wsp<real>(c, c->L.off_u), 3 * N * es, cudaMemcpyDefault, c->stream));
+        if (h_p) CK(cudaMemcpyAsync(h_p, wsp<real>(c, c->L.off_p), N * es, cudaMemcpyDefault, c->stream));
+        if (h_T) CK(cudaMemcpyAsync(h_T, wsp<real>(c, c->L.off_T), N * es, cudaMemcpyDefault, c->stream));
         CK(cudaStreamSynchronize(c->stream));
         return LBM_OK;
     }
@@ -273,7 +273,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     template <class L> static int read_pops_one(lbm_ctx *c, int which, int stage, const size_t (&off)[2], void *h) {
         const size_t N = (size_t)c->L.N, bytes = (size_t)L::Q * N * sizeof(real);
         if (stage == LBM_STAGE_POSTCOLLISION) {
-            CK(cudaMemcpyAsync(h, wsp<real>(c, off[c->cur]), bytes, cudaMemcpyDeviceToHost, c->stream));
+            CK(cudaMemcpyAsync(h, wsp<real>(c, off[c->cur]), bytes, cudaMemcpyDefault, c->stream));
             CK(cudaStreamSynchronize(c->stream));
             return LBM_OK;
         }
@@ -284,7 +284,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
             dev_params<real>(c), wsp<real>(c, off[1 - c->cur]), tmp, which);
         c->launches++;
         cudaError_t e = cudaGetLastError();
-        if (e == cudaSuccess) e = cudaMemcpyAsync(h, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h, tmp, bytes, cudaMemcpyDefault, c->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
         cudaFree(tmp);
         CK(e);

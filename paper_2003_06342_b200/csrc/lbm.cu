@@ -317,7 +317,7 @@ int lbm_set_velocity(lbm_ctx *c, const void *h_u) {
     if (!c || !h_u || !(c->P.flags & LBM_FLAG_PRESCRIBED_U)) return LBM_E_INVALID;
     if (!c->inited) return LBM_E_STATE;
     const size_t es = c->P.precision == 64 ? 8 : 4;
-    CK(cudaMemcpyAsync(c->ws + c->L.off_u, h_u, 3 * (size_t)c->L.N * es, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->ws + c->L.off_u, h_u, 3 * (size_t)c->L.N * es, cudaMemcpyDefault, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return LBM_OK;
 }

@@ -452,6 +452,23 @@ def test_api_states_and_degenerate_calls(gpu, oracle_mod):
     sim.destroy(); sim.destroy(); o.close()                  # destroy is idempotent
 
 
+def test_device_resident_fields(gpu, oracle_mod):
+    """lbm_init / lbm_set_velocity / lbm_read_macro take DEVICE pointers as well (unified addressing)."""
+    import torch
+    P = wl.base_params(40, 10, 7, grav=[1e-4, 0.0, -2e-4])
+    init = _random_state(P, 47)
+    o = oracle_mod.Oracle(P); o.init(*init); o.step(4)
+    sim = gpu.LBM(P, 64)
+    sim.init(*[torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in init])
+    sim.step(4)
+    out = (torch.empty(sim.shape, dtype=torch.float64, device="cuda"), torch.empty((3,) + sim.shape, dtype=torch.float64, device="cuda"),
+           torch.empty(sim.shape, dtype=torch.float64, device="cuda"), torch.empty(sim.shape, dtype=torch.float64, device="cuda"))
+    sim.read_macro(out=out)
+    for a, b, name in zip(out, o.read_macro(), ("phi", "u", "p", "T")):
+        assert np.abs(a.cpu().numpy() - b).max() <= TOL64, name
+    sim.destroy(); o.close()
+
+
 def test_fp32_populations_and_defaults(gpu, oracle_mod):
     P = wl.base_params(33, 17, 1, lat_s="D2Q9")
     init = _random_state(P, 42)
