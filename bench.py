@@ -244,7 +244,7 @@ def run_ours(args):
     Q = q[P["lat_f"]] + q[P["lat_g"]] + q[P["lat_s"]]
     main_vals = (Q + 3) + (Q + 1)                    # reads: pops, phi^{n+1}, phi^n, Pdot; writes: pops, Pdot
     phi_vals = q[P["lat_g"]] + 1 + 1
-    main_bytes = main_vals * es * N
+    main_bytes = (main_vals * es + 2 * (8 - es)) * N    # the two phi values are doubles in both precisions
     main_ms = ms_main / max(nsteps_timed, 1)
     phi_ms = ms_phi / max(nsteps_timed, 1)
     peak, peak_src = measured_peak()
@@ -254,7 +254,7 @@ def run_ours(args):
         "bound": "hbm", "kernel": "k_main", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "peak_source": peak_src, "traffic": ncu_traffic(args.workload, prec),
         "algorithmic_bytes_per_launch": main_bytes, "ms_per_launch": main_ms,
-        "k_phi": {"ms_per_launch": phi_ms, "achieved": phi_vals * es * N / (phi_ms * 1e-3) / 1e9 if phi_ms > 0 else None},
+        "k_phi": {"ms_per_launch": phi_ms, "achieved": (phi_vals * es + (8 - es)) * N / (phi_ms * 1e-3) / 1e9 if phi_ms > 0 else None},
         "step": {"bytes_per_lu": wl.bytes_per_lu(P, es), "achieved": step_bytes / (ms_job / K * 1e-3) / 1e9,
                  "frac_of_peak": step_bytes / (ms_job / K * 1e-3) / 1e9 / peak,
                  "frac_of_8TBs": step_bytes / (ms_job / K * 1e-3) / 1e9 / 8000.0},

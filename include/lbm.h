@@ -17,6 +17,12 @@
  *     populations [Q][z][y][x] in the direction order documented in DESIGN.md ("Lattices").
  *   - "h_" pointers are HOST memory (pageable or pinned), "d_" pointers are DEVICE memory.
  *   - Element type of every field pointer is the context's precision: double (64) or float (32).
+ *   - Precisions.  64: double storage and arithmetic (parity bar 1e-10 against the oracle).  32: float populations,
+ *     production field, macro arrays and arithmetic -- except the phase-field path, which is kept wide because what its
+ *     rounding adds to dphi/dt reaches T multiplied by L/Cp: the padded phi arrays are double,
+ *     phi^{n+1} = sum_i g_i (Eq.32) is an exact sum of the float populations, dphi/dt = (phi^{n+1} - phi^n)/dt (Eq.34,
+ *     DESIGN.md reading S4) and the collision of g (Eq.31) are evaluated in double.  Parity bar: 1e-4 relative to the
+ *     oracle.  LBM_HALO_PHI buffers hold doubles in both precisions.
  *   - All calls return 0 (LBM_OK) or a negative LBM_E_* code; nothing throws across this boundary.
  *   - A context is bound to one device, one stream; calls on one context must not race.
  */
@@ -89,7 +95,7 @@ enum {
 typedef struct lbm_params {
     int nx, ny, nz;
     int lat_f, lat_g, lat_s;
-    int precision;          /* 64 or 32: storage and arithmetic type                                */
+    int precision;          /* 64 or 32 (see "Precisions" above)                                   */
     int bc_f[3][2];         /* LBM_F_*                                                              */
     int bc_g[3][2];         /* LBM_S_* for the phase field                                          */
     int bc_s[3][2];         /* LBM_S_* for the temperature                                          */

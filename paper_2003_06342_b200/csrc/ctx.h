@@ -25,6 +25,7 @@ enum LatSet { SET_NONE = 0, SET_2D_995, SET_2D_999, SET_3D_1977, SET_3D_1577 };
 
 struct Layout {
     long long N;
+    int es, es_phi;   // bytes per element: populations / Pdot / macros / caller's arrays; padded phi arrays
     int ppx, ppy, ppz, pz, xpad;
     size_t phi_pad_elems;
     size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot[2], off_u, off_p, off_T, off_scratch, total;

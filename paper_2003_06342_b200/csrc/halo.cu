@@ -45,7 +45,7 @@ bool make_plan(const lbm_ctx *c, int what, int side, bool ghost, HaloPlan &pl) {
     const bool three_d = P.nz > 1;
     const int axis = three_d ? 2 : 1;
     const int len = three_d ? P.nz : P.ny;
-    const size_t es = P.precision == 64 ? 8 : 4;
+    const size_t es = (size_t)c->L.es, esp = (size_t)c->L.es_phi;
     long long layer = side == 0 ? 0 : len - 1;
     if (!ghost) layer += side == 0 ? 1 : -1;
     pl.count = 0;
@@ -54,7 +54,7 @@ bool make_plan(const lbm_ctx *c, int what, int side, bool ghost, HaloPlan &pl) {
         const size_t layer_elems = three_d ? (size_t)c->L.ppx * c->L.ppy : (size_t)c->L.ppx;
         pl.elems = layer_elems;
         const int pnew = c->phase == 1 ? 1 - c->curphi : c->curphi;   // between the phases phi^{n+1} is the other buffer
-        pl.ptr[pl.count++] = c->ws + c->L.off_phi[pnew] + (size_t)(layer + 1) * layer_elems * es;
+        pl.ptr[pl.count++] = c->ws + c->L.off_phi[pnew] + (size_t)(layer + 1) * layer_elems * esp;
         return true;
     }
     // populations that stream across the cut towards `side`: e_axis = +1 for the high side, -1 for the low side.
@@ -97,7 +97,7 @@ int halo_copy(lbm_ctx *c, int what, int side, void *d_buf, bool pack) {
     if (!make_plan(c, what, side, /*ghost=*/!pack, pl)) return LBM_E_INVALID;
     const unsigned gx = (unsigned)((pl.elems + 1023) / 1024 > 0 ? (pl.elems + 1023) / 1024 : 1);
     const dim3 grid(gx > 1184u ? 1184u : gx, (unsigned)pl.count);
-    if (c->P.precision == 64) k_halo_copy<double><<<grid, 256, 0, c->stream>>>(pl, static_cast<double *>(d_buf), pack ? 1 : 0);
+    if ((what == LBM_HALO_PHI ? c->L.es_phi : c->L.es) == 8) k_halo_copy<double><<<grid, 256, 0, c->stream>>>(pl, static_cast<double *>(d_buf), pack ? 1 : 0);
     else k_halo_copy<float><<<grid, 256, 0, c->stream>>>(pl, static_cast<float *>(d_buf), pack ? 1 : 0);
     c->launches++;
     CK(cudaGetLastError());
@@ -115,7 +115,7 @@ int lbm_halo_bytes(const lbm_ctx *c, int what, size_t *bytes) {
     lbm::HaloPlan pl;
     const int side = c->P.halo[0] ? 0 : 1;   // the size depends neither on the side nor on the phase
     if (!lbm::make_plan(c, what, side, false, pl)) return LBM_E_INVALID;
-    *bytes = (size_t)pl.count * (size_t)pl.elems * (c->P.precision == 64 ? 8 : 4);
+    *bytes = (size_t)pl.count * (size_t)pl.elems * (size_t)(what == LBM_HALO_PHI ? c->L.es_phi : c->L.es);
     return LBM_OK;
 }
 

@@ -36,8 +36,11 @@ template <class T> dim3 grid_for(const lbm_params &P) {
     return dim3((P.nx + T::BX - 1) / T::BX, (P.ny + T::BY - 1) / T::BY, (P.nz + T::BZ - 1) / T::BZ);
 }
 
-template <class LF, class LG, class LS, class real, class T> struct Impl {
+// real: arithmetic type; sreal: storage of populations, Pdot, macros (and the type of the caller's arrays); preal: phi arrays.
+template <class LF, class LG, class LS, class real, class T, class sreal = real, class preal = real> struct Impl {
     static constexpr int D = LF::D;
+    static constexpr bool UNIFORM = std::is_same<real, sreal>::value && std::is_same<real, preal>::value;
+    using Fields = DevFieldsT<sreal, preal>;
     static constexpr int NT = T::BX * T::BY * T::BZ;
     using TP = typename T::PhiTile;                       // tile of K_phi and of the utility kernels
     static constexpr int NTP = TP::BX * TP::BY * TP::BZ;
@@ -54,23 +57,26 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
 #ifndef LBM_PHI_NPT
 #define LBM_PHI_NPT 2
 #endif
-    static constexpr int PHI_NPT = LBM_PHI_NPT;   // nodes per thread in K_phi
+#ifndef LBM_PHI_NPT32
+#define LBM_PHI_NPT32 2
+#endif
+    static constexpr int PHI_NPT = sizeof(sreal) == 8 ? LBM_PHI_NPT : LBM_PHI_NPT32;   // nodes per thread in K_phi
 
-    static DevFields<real> fields(const lbm_ctx *c, int in, int out, int phi_new, int phi_old) {
-        DevFields<real> F{};
-        F.f_in = wsp<real>(c, c->L.off_f[in]);  F.f_out = wsp<real>(c, c->L.off_f[out]);
-        F.g_in = wsp<real>(c, c->L.off_g[in]);  F.g_out = wsp<real>(c, c->L.off_g[out]);
-        F.s_in = wsp<real>(c, c->L.off_s[in]);  F.s_out = wsp<real>(c, c->L.off_s[out]);
-        F.phi_new = wsp<real>(c, c->L.off_phi[phi_new]);
-        F.phi_old = wsp<real>(c, c->L.off_phi[phi_old]);
-        F.pdot = wsp<real>(c, c->L.off_pdot[0]);
+    static Fields fields(const lbm_ctx *c, int in, int out, int phi_new, int phi_old) {
+        Fields F{};
+        F.f_in = wsp<sreal>(c, c->L.off_f[in]);  F.f_out = wsp<sreal>(c, c->L.off_f[out]);
+        F.g_in = wsp<sreal>(c, c->L.off_g[in]);  F.g_out = wsp<sreal>(c, c->L.off_g[out]);
+        F.s_in = wsp<sreal>(c, c->L.off_s[in]);  F.s_out = wsp<sreal>(c, c->L.off_s[out]);
+        F.phi_new = wsp<preal>(c, c->L.off_phi[phi_new]);
+        F.phi_old = wsp<preal>(c, c->L.off_phi[phi_old]);
+        F.pdot = wsp<sreal>(c, c->L.off_pdot[0]);
         F.pdot_in = F.pdot;
-        F.u = wsp<real>(c, c->L.off_u); F.p = wsp<real>(c, c->L.off_p); F.T = wsp<real>(c, c->L.off_T);
+        F.u = wsp<sreal>(c, c->L.off_u); F.p = wsp<sreal>(c, c->L.off_p); F.T = wsp<sreal>(c, c->L.off_T);
         return F;
     }
 
-    template <int MODE> static int launch_main(lbm_ctx *c, const DevFields<real> &F, int in = 0, int pnew = 0) {
-        if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU) {
+    template <int MODE> static int launch_main(lbm_ctx *c, const Fields &F, int in = 0, int pnew = 0) {
+        if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU && UNIFORM) {
             if (c->use_tma) {
                 using C = TmaCfg<LF, LG, LS, real>;
                 auto kern = k_main_tma<LF, LG, LS, real, MODE>;
@@ -108,14 +114,14 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     }
 
     static int init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, const void *h_p) {
-        const size_t N = (size_t)c->L.N, es = sizeof(real);
+        const size_t N = (size_t)c->L.N, es = sizeof(sreal);
         const DevParams<real> &P = dev_params<real>(c);
-        real *scratch = wsp<real>(c, c->L.off_scratch);
+        sreal *scratch = wsp<sreal>(c, c->L.off_scratch);
         CK(cudaMemcpyAsync(scratch, h_phi, N * es, cudaMemcpyDefault, c->stream));
-        real *dT = wsp<real>(c, c->L.off_T), *du = wsp<real>(c, c->L.off_u), *dp = wsp<real>(c, c->L.off_p);
+        sreal *dT = wsp<sreal>(c, c->L.off_T), *du = wsp<sreal>(c, c->L.off_u), *dp = wsp<sreal>(c, c->L.off_p);
         if (h_T) CK(cudaMemcpyAsync(dT, h_T, N * es, cudaMemcpyDefault, c->stream));
         else {
-            k_fill<real><<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(dT, (long long)N, (real)c->P.T_sat);
+            k_fill<sreal><<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(dT, (long long)N, (sreal)c->P.T_sat);
             c->launches++;
             CK(cudaGetLastError());
         }
@@ -124,13 +130,13 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         if (h_p) CK(cudaMemcpyAsync(dp, h_p, N * es, cudaMemcpyDefault, c->stream));
         else CK(cudaMemsetAsync(dp, 0, N * es, c->stream));
         for (int b = 0; b < 2; ++b)
-            CK(cudaMemsetAsync(wsp<real>(c, c->L.off_phi[b]), 0, c->L.phi_pad_elems * es, c->stream));
+            CK(cudaMemsetAsync(wsp<preal>(c, c->L.off_phi[b]), 0, c->L.phi_pad_elems * sizeof(preal), c->stream));
         k_phi_fill<real, TP::BX, TP::BY, TP::BZ><<<grid_for<TP>(c->P), NTP, 0, c->stream>>>(
-            P, scratch, wsp<real>(c, c->L.off_phi[0]), wsp<real>(c, c->L.off_phi[1]));
+            P, (const sreal *)scratch, wsp<preal>(c, c->L.off_phi[0]), wsp<preal>(c, c->L.off_phi[1]));
         c->launches++;
         CK(cudaGetLastError());
         c->cur = 0; c->curphi = 0;
-        DevFields<real> F = fields(c, 1, 0, 0, 0);   // INIT reads no populations; writes buffer 0
+        Fields F = fields(c, 1, 0, 0, 0);   // INIT reads no populations; writes buffer 0
         int rc = launch_main<MODE_INIT>(c, F);
         if (rc) return rc;
         CK(cudaStreamSynchronize(c->stream));
@@ -146,8 +152,8 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
 #define LBM_FLZ 32
 #endif
     struct FusedCfg { static constexpr int BX = LBM_FBX, BY = LBM_FBY, LZ = LBM_FLZ; };
-    template <int MODE> static int launch_fused(lbm_ctx *c, DevFields<real> F, int in, int pnew) {
-        if constexpr (D == 3) {
+    template <int MODE> static int launch_fused(lbm_ctx *c, Fields F, int in, int pnew) {
+        if constexpr (D == 3 && UNIFORM) {
             F.pdot_in = wsp<real>(c, c->L.off_pdot[in]);
             F.pdot = wsp<real>(c, c->L.off_pdot[1 - in]);
             const dim3 grid((c->P.nx + FusedCfg::BX - 1) / FusedCfg::BX, (c->P.ny + FusedCfg::BY - 1) / FusedCfg::BY,
@@ -169,7 +175,8 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         dim3 gphi = grid_for<TP>(c->P);
         if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
         k_phi<LG, real, TP::BX, TP::BY, TP::BZ, PHI_NPT><<<gphi, NTP, 0, c->stream>>>(
-            P, wsp<real>(c, c->L.off_g[in]), wsp<real>(c, c->L.off_pdot[0]), wsp<real>(c, c->L.off_phi[pnew]));
+            P, (const sreal *)wsp<sreal>(c, c->L.off_g[in]), (const sreal *)wsp<sreal>(c, c->L.off_pdot[0]),
+            wsp<preal>(c, c->L.off_phi[pnew]));
         c->launches++;
         CK(cudaGetLastError());
         return LBM_OK;
@@ -179,7 +186,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     static int launch_collide(lbm_ctx *c, bool macro) {
         const DevParams<real> &P = dev_params<real>(c);
         const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
-        DevFields<real> F = fields(c, in, out, pnew, pold);
+        Fields F = fields(c, in, out, pnew, pold);
         int rc;
         if (P.prescribed_u) rc = launch_main<MODE_STEP_PU>(c, F, in, pnew);   // direct kernel only
         else rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
@@ -203,7 +210,7 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
         int rc;
         if (c->fused && !dev_params<real>(c).prescribed_u) {
             const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
-            DevFields<real> F = fields(c, in, out, pnew, pold);
+            Fields F = fields(c, in, out, pnew, pold);
             if (timed) CK(cudaEventRecord(e3[1], c->stream));
             rc = macro ? launch_fused<MODE_STEP_MACRO>(c, F, in, pnew) : launch_fused<MODE_STEP>(c, F, in, pnew);
             if (rc) return rc;
@@ -254,34 +261,34 @@ template <class LF, class LG, class LS, class real, class T> struct Impl {
     }
 
     static int read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T) {
-        const size_t N = (size_t)c->L.N, es = sizeof(real);
+        const size_t N = (size_t)c->L.N, es = sizeof(sreal);
         if (h_phi) {
-            real *scratch = wsp<real>(c, c->L.off_scratch);
+            sreal *scratch = wsp<sreal>(c, c->L.off_scratch);
             k_phi_unpad<real, TP::BX, TP::BY, TP::BZ><<<grid_for<TP>(c->P), NTP, 0, c->stream>>>(
-                dev_params<real>(c), wsp<real>(c, c->L.off_phi[c->curphi]), scratch);
+                dev_params<real>(c), (const preal *)wsp<preal>(c, c->L.off_phi[c->curphi]), scratch);
             c->launches++;
             CK(cudaGetLastError());
             CK(cudaMemcpyAsync(h_phi, scratch, N * es, cudaMemcpyDefault, c->stream));
         }
-        if (h_u) CK(cudaMemcpyAsync(h_u, wsp<real>(c, c->L.off_u), 3 * N * es, cudaMemcpyDefault, c->stream));
-        if (h_p) CK(cudaMemcpyAsync(h_p, wsp<real>(c, c->L.off_p), N * es, cudaMemcpyDefault, c->stream));
-        if (h_T) CK(cudaMemcpyAsync(h_T, wsp<real>(c, c->L.off_T), N * es, cudaMemcpyDefault, c->stream));
+        if (h_u) CK(cudaMemcpyAsync(h_u, wsp<sreal>(c, c->L.off_u), 3 * N * es, cudaMemcpyDefault, c->stream));
+        if (h_p) CK(cudaMemcpyAsync(h_p, wsp<sreal>(c, c->L.off_p), N * es, cudaMemcpyDefault, c->stream));
+        if (h_T) CK(cudaMemcpyAsync(h_T, wsp<sreal>(c, c->L.off_T), N * es, cudaMemcpyDefault, c->stream));
         CK(cudaStreamSynchronize(c->stream));
         return LBM_OK;
     }
 
     template <class L> static int read_pops_one(lbm_ctx *c, int which, int stage, const size_t (&off)[2], void *h) {
-        const size_t N = (size_t)c->L.N, bytes = (size_t)L::Q * N * sizeof(real);
+        const size_t N = (size_t)c->L.N, bytes = (size_t)L::Q * N * sizeof(sreal);
         if (stage == LBM_STAGE_POSTCOLLISION) {
-            CK(cudaMemcpyAsync(h, wsp<real>(c, off[c->cur]), bytes, cudaMemcpyDefault, c->stream));
+            CK(cudaMemcpyAsync(h, wsp<sreal>(c, off[c->cur]), bytes, cudaMemcpyDefault, c->stream));
             CK(cudaStreamSynchronize(c->stream));
             return LBM_OK;
         }
         if (c->nsteps < 1) return LBM_E_STATE;
-        real *tmp = nullptr;
+        sreal *tmp = nullptr;
         CK(cudaMalloc(&tmp, bytes));   // debug path: own temporary, not the borrowed workspace
         k_stream_only<L, real, TP::BX, TP::BY, TP::BZ><<<grid_for<TP>(c->P), NTP, 0, c->stream>>>(
-            dev_params<real>(c), wsp<real>(c, off[1 - c->cur]), tmp, which);
+            dev_params<real>(c), (const sreal *)wsp<sreal>(c, off[1 - c->cur]), tmp, which);
         c->launches++;
         cudaError_t e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaMemcpyAsync(h, tmp, bytes, cudaMemcpyDefault, c->stream);

@@ -1,10 +1,10 @@
-// Instantiation unit: (D3Q19, D3Q7, D3Q7) in float.  One translation unit per (lattice set, precision) so that the build
-// compiles them in parallel.
+// Instantiation unit: (D3Q19, D3Q7, D3Q7) in float, phi kept in double (include/lbm.h "precision").  One translation unit per
+// (lattice set, precision) so that the build compiles them in parallel.
 #include "impl.cuh"
 
 namespace lbm {
 const ImplOps *ops_3d_f32(int nx) {
-    if (wide_tile_pays(nx)) return Impl<D3Q19, D3Q7, D3Q7, float, TileWide3Phi>::ops();
-    return Impl<D3Q19, D3Q7, D3Q7, float, TileNarrow3>::ops();
+    if (wide_tile_pays(nx)) return Impl<D3Q19, D3Q7, D3Q7, float, TileWide3Phi, float, double>::ops();
+    return Impl<D3Q19, D3Q7, D3Q7, float, TileNarrow3, float, double>::ops();
 }
 }  // namespace lbm

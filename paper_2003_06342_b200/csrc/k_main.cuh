@@ -9,11 +9,11 @@
 namespace lbm {
 
 // population stores: written once, read by the NEXT step only
-template <class real> __device__ __forceinline__ void st_pop(real *p, real v) {
+template <class sreal, class real> __device__ __forceinline__ void st_pop(sreal *p, real v) {
 #ifdef LBM_EXP_STCS
-    __stcs(p, v);
+    __stcs(p, sreal(v));
 #else
-    *p = v;
+    *p = sreal(v);
 #endif
 }
 
@@ -22,30 +22,33 @@ __device__ __forceinline__ float rsqrt_(float a) { return rsqrtf(a); }
 
 // Source of one node's inputs, direct variant: gathers straight from global memory (pull with wrap / boundary
 // rules); the phi^{n+1} neighbourhood comes from the padded array through L1/L2.
-template <class LF, class LG, class LS, class real, bool BC> struct SrcGlobal {
+template <class LF, class LG, class LS, class real, bool BC, class Fields = DevFields<real>> struct SrcGlobal {
+    using preal = typename Fields::preal;
     const DevParams<real> &P;
-    const DevFields<real> &Fd;
+    const Fields &Fd;
     const NodeGeom &g;
-    const real *__restrict__ pc;   // the node's own element of the padded phi^{n+1}
+    const preal *__restrict__ pc;   // the node's own element of the padded phi^{n+1}
     unsigned pcoff;
-    __device__ __forceinline__ SrcGlobal(const DevParams<real> &P_, const DevFields<real> &Fd_, const NodeGeom &g_)
+    __device__ __forceinline__ SrcGlobal(const DevParams<real> &P_, const Fields &Fd_, const NodeGeom &g_)
         : P(P_), Fd(Fd_), g(g_) {
         pcoff = ((unsigned)(g.z + P.pz) * (unsigned)P.ppy + (unsigned)(g.y + 1)) * (unsigned)P.ppx + (unsigned)(g.x + P.xpad);
         pc = Fd.phi_new + pcoff;
     }
     __device__ __forceinline__ void phi_ready() const {}
-    __device__ __forceinline__ real phi(int dx, int dy, int dz) const { return __ldg(pc + (dx + dy * P.ppx + dz * (int)P.pplane)); }
-    __device__ __forceinline__ real phi_old() const { return __ldg(Fd.phi_old + pcoff); }
-    __device__ __forceinline__ real pdot_old() const { return Fd.pdot_in[g.n]; }
+    __device__ __forceinline__ preal phi(int dx, int dy, int dz) const { return __ldg(pc + (dx + dy * P.ppx + dz * (int)P.pplane)); }
+    __device__ __forceinline__ preal phi_old() const { return __ldg(Fd.phi_old + pcoff); }
+    __device__ __forceinline__ real pdot_old() const { return real(Fd.pdot_in[g.n]); }
     // AGAIN = true: second read of a value already read for the moments (see ld_again)
     template <int I, bool AGAIN = false> __device__ __forceinline__ real f() const { return pull_one<LF, I, real, BC, AGAIN>(Fd.f_in, (unsigned)P.N, g, P.bc_f, P.bc_p); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real s() const { return pull_one<LS, I, real, BC, AGAIN>(Fd.s_in, (unsigned)P.N, g, P.bc_s, P.bc_T); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real gg() const { return pull_one<LG, I, real, BC, AGAIN>(Fd.g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi); }
 };
 
-template <class LF, class LG, class LS, class real, int MODE, class Src>
-__device__ __forceinline__ void node_update(const DevParams<real> &P, const DevFields<real> &Fd, const NodeGeom &g,
+template <class LF, class LG, class LS, class real, int MODE, class Src, class Fields>
+__device__ __forceinline__ void node_update(const DevParams<real> &P, const Fields &Fd, const NodeGeom &g,
                                             const Src &src) {
+    using sreal = typename Fields::sreal;
+    using preal = typename Fields::preal;   // phi arrays; differences of phi are taken in this type, then narrowed
     const unsigned n = g.n;
     const unsigned N = (unsigned)P.N;
 
@@ -58,19 +61,20 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
     // ---- H2: grad phi, lap phi by directional derivatives on the NS lattice (Eq.35a,b 36a,b; PAPER.md:291-315;
     //      the printed factor 3 is 1/e2, reading S2).  Opposite directions are paired: one difference, one sum.
     src.phi_ready();   // TMA-staged phi tile: wait here, after the s loads have been issued
-    const real phi = src.phi(0, 0, 0);
+    const preal phi_p = src.phi(0, 0, 0);
+    const real phi = real(phi_p);
     real gx = real(0), gy = real(0), gz = real(0), lsum = real(0);
     static_for<LF::Q>([&](auto ic) {
         constexpr int I = decltype(ic)::value;
         if constexpr (I > 0 && I < LF::opp(I)) {
             constexpr int ex = LF::ex(I), ey = LF::ey(I), ez = LF::ez(I);
-            const real pp = src.phi(ex, ey, ez), pm = src.phi(-ex, -ey, -ez);
-            const real d = pp - pm;
+            const preal pp = src.phi(ex, ey, ez), pm = src.phi(-ex, -ey, -ez);
+            const real d = real(pp - pm);
             constexpr real w = real(LF::w(I));
             if constexpr (ex != 0) gx += (ex > 0 ? w : -w) * d;
             if constexpr (ey != 0) gy += (ey > 0 ? w : -w) * d;
             if constexpr (ez != 0) gz += (ez > 0 ? w : -w) * d;
-            lsum += w * (pp + pm);
+            lsum += w * real(pp + pm);
         }
     });
     {
@@ -102,8 +106,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
 
     real ux, uy, uz, p, T, dtphi;
     if constexpr (MODE == MODE_INIT) {
-        ux = Fd.u[n]; uy = Fd.u[N + n]; uz = (LF::D == 3) ? Fd.u[2 * N + n] : real(0);
-        p = Fd.p[n]; T = Fd.T[n]; dtphi = real(0);
+        ux = real(Fd.u[n]); uy = real(Fd.u[N + n]); uz = (LF::D == 3) ? real(Fd.u[2 * N + n]) : real(0);
+        p = real(Fd.p[n]); T = real(Fd.T[n]); dtphi = real(0);
     } else {
         // ---- H4: NS moments (Eq.28a), accumulated as the pulled values arrive
         real m0 = real(0), mx = real(0), my = real(0), mz = real(0);
@@ -120,10 +124,10 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
         uy = (cm * my + P.hdt * Fy) * inv_rho;
         uz = (cm * mz + P.hdt * Fz) * inv_rho;
         if constexpr (MODE == MODE_STEP_PU) {   // Zalesak / vortex verifications: u is the field given at init
-            ux = Fd.u[n]; uy = Fd.u[N + n]; uz = (LF::D == 3) ? Fd.u[2 * N + n] : real(0);
+            ux = real(Fd.u[n]); uy = real(Fd.u[N + n]); uz = (LF::D == 3) ? real(Fd.u[2 * N + n]) : real(0);
         }
         // ---- H1 (time derivative), H5: heat moment with the STORED production rate (reading S3; Eq.34)
-        dtphi = (phi - src.phi_old()) * P.inv_dt;                              // reading S4
+        dtphi = real(phi_p - src.phi_old()) * P.inv_dt;                              // reading S4
         const real mdot_old = P.rho_g * src.pdot_old();
         const real D_old = ux * gx + uy * gy + uz * gz + phi * mdot_old * P.drho;   // reading S5
         T = sum_s;
@@ -136,14 +140,15 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
     real pdot = real(0);
     if (P.phase_change) {
         const real theta = P.CpL * (T - P.T_sat);
-        pdot = P.pc_coef * alpha * (theta - P.theta_I) * phi * (real(1) - phi);
+        // this level's collision and the next level's moment corrections use the SAME value (reading S3): the stored one
+        pdot = real(sreal(P.pc_coef * alpha * (theta - P.theta_I) * phi * (real(1) - phi)));
     }
-    Fd.pdot[n] = pdot;
+    Fd.pdot[n] = sreal(pdot);
     if constexpr (MODE == MODE_STEP_MACRO) {
-        Fd.u[n] = ux; Fd.u[N + n] = uy; Fd.u[2 * N + n] = uz;
-        Fd.p[n] = p; Fd.T[n] = T;
+        Fd.u[n] = sreal(ux); Fd.u[N + n] = sreal(uy); Fd.u[2 * N + n] = sreal(uz);
+        Fd.p[n] = sreal(p); Fd.T[n] = sreal(T);
     }
-    if constexpr (MODE == MODE_STEP_PU) { Fd.p[n] = p; Fd.T[n] = T; }
+    if constexpr (MODE == MODE_STEP_PU) { Fd.p[n] = sreal(p); Fd.T[n] = sreal(T); }
 
     // ---- H7: sources, equilibria, BGK (Eq.25)
     const real mdot = P.rho_g * pdot;
@@ -228,34 +233,43 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
     }
     // -- conservative Allen-Cahn, modified-equilibrium form (Eq.31a,b PAPER.md:246-251; P_i^g Eq.30b):
     //    eq_i = phi Gamma_i + M (4/W) phi (1-phi) w_i c_i.n / cs2,  S_i = w_i Pdot
+    //    Evaluated in the type of the phi arrays (greal = preal): sum_i g*_i is the phi of the next level, and what its
+    //    rounding adds to dphi/dt reaches T multiplied by L/Cp.
     {
-        const real om = MODE == MODE_INIT ? real(1) : P.om_g;
-        const real a = MODE == MODE_INIT ? real(0) : real(1) - P.om_g;
-        const real b = MODE == MODE_INIT ? P.hdt : P.dt * (real(1) - real(0.5) * P.om_g);
-        const real ic = P.c_cs2g;
-        const real tx = ux * ic, ty = uy * ic, tz = uz * ic;
-        const real U1 = real(1) - real(0.5) * uu * P.inv_cs2g;
+#ifdef LBM_G_NARROW
+        using greal = real;
+#else
+        using greal = preal;
+#endif
+        const greal om_g = greal(P.g_om), dtg = greal(P.g_dt);   // constants carried in double: no widening per node
+        const greal om = MODE == MODE_INIT ? greal(1) : om_g;
+        const greal a = MODE == MODE_INIT ? greal(0) : greal(1) - om_g;
+        const greal b = MODE == MODE_INIT ? greal(0.5) * dtg : dtg * (greal(1) - greal(0.5) * om_g);
+        const greal ic = greal(P.g_c_cs2);
+        const greal tx = greal(ux) * ic, ty = greal(uy) * ic, tz = greal(uz) * ic;
+        const greal U1 = greal(1) - greal(0.5) * greal(uu) * greal(P.g_inv_cs2);
         const real inv_norm = rsqrt_(gx * gx + gy * gy + gz * gz + P.eps_n2);     // Eq.(6), reading S7
-        const real B = om * P.cac * phi * (real(1) - phi) * inv_norm;             // om M (4/W) phi(1-phi) c / cs2 / |grad phi|
-        const real bx = B * gx, by = B * gy, bz = B * gz;
-        const real PO = om * phi;
-        const real bP = b * pdot;
+        const greal phi_g = greal(phi_p);
+        const greal B = om * greal(P.g_cac) * phi_g * (greal(1) - phi_g) * greal(inv_norm);   // om M (4/W) phi(1-phi) c / cs2 / |grad phi|
+        const greal bx = B * greal(gx), by = B * greal(gy), bz = B * greal(gz);
+        const greal PO = om * phi_g;
+        const greal bP = b * greal(pdot);
         {
-            constexpr real w = real(LG::w(0));
-            real bar = real(0);
-            if constexpr (MODE != MODE_INIT) bar = src.template gg<0>();
+            constexpr greal w = greal(LG::w(0));
+            greal bar = greal(0);
+            if constexpr (MODE != MODE_INIT) bar = greal(src.template gg<0>());
             st_pop(Fd.g_out + (n), a * bar + w * (PO * U1 + bP));
         }
         static_for<LG::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
             if constexpr (I > 0 && I < LG::opp(I)) {
                 constexpr int J = LG::opp(I);
-                constexpr real w = real(LG::w(I));
-                real bi = real(0), bj = real(0);
-                if constexpr (MODE != MODE_INIT) { bi = src.template gg<I>(); bj = src.template gg<J>(); }
-                const real t = dot_e<LG, I, real>(tx, ty, tz);
-                const real q = real(0.5) * t * t + U1;
-                const real cn = dot_e<LG, I, real>(bx, by, bz);
+                constexpr greal w = greal(LG::w(I));
+                greal bi = greal(0), bj = greal(0);
+                if constexpr (MODE != MODE_INIT) { bi = greal(src.template gg<I>()); bj = greal(src.template gg<J>()); }
+                const greal t = dot_e<LG, I, greal>(tx, ty, tz);
+                const greal q = greal(0.5) * t * t + U1;
+                const greal cn = dot_e<LG, I, greal>(bx, by, bz);
                 st_pop(Fd.g_out + ((unsigned)I * N + n), a * bi + w * (PO * (q + t) + (bP + cn)));
                 st_pop(Fd.g_out + ((unsigned)J * N + n), a * bj + w * (PO * (q - t) + (bP - cn)));
             }
@@ -264,19 +278,19 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const DevF
 }
 
 // Direct variant: everything gathered from global memory.
-template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB>
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB, class Fields>
 __global__ void __launch_bounds__(BX *BY *BZ, MINB)
-k_main_direct(const DevParams<real> P, const DevFields<real> Fd) {
+k_main_direct(const DevParams<real> P, const Fields Fd) {
     const int t = threadIdx.x;
     const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY, z0 = blockIdx.z * BZ;
     const int x = x0 + t % BX, y = y0 + (t / BX) % BY, z = z0 + t / (BX * BY);
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
     const NodeGeom g = make_geom(P, x, y, z);
     if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) {
-        const SrcGlobal<LF, LG, LS, real, true> src(P, Fd, g);
+        const SrcGlobal<LF, LG, LS, real, true, Fields> src(P, Fd, g);
         node_update<LF, LG, LS, real, MODE>(P, Fd, g, src);
     } else {
-        const SrcGlobal<LF, LG, LS, real, false> src(P, Fd, g);
+        const SrcGlobal<LF, LG, LS, real, false, Fields> src(P, Fd, g);
         node_update<LF, LG, LS, real, MODE>(P, Fd, g, src);
     }
 }

@@ -18,33 +18,35 @@ template <class real, int D, int BX, int BY, int BZ> struct PhiTileCfg {
     static constexpr uint32_t BYTES = (uint32_t)ELEMS * sizeof(real);
 };
 
-template <class LF, class LG, class LS, class real, bool BC, class TC> struct SrcGlobalPhiSmem {
+template <class LF, class LG, class LS, class real, bool BC, class TC, class Fields> struct SrcGlobalPhiSmem {
+    using preal = typename Fields::preal;
     const DevParams<real> &P;
-    const DevFields<real> &Fd;
+    const Fields &Fd;
     const NodeGeom &g;
-    const real *tile;    // the node's own element in the shared-memory tile
+    const preal *tile;    // the node's own element in the shared-memory tile
     uint32_t bar;
     unsigned pcoff;
-    __device__ __forceinline__ SrcGlobalPhiSmem(const DevParams<real> &P_, const DevFields<real> &Fd_, const NodeGeom &g_,
-                                                const real *tile_base, uint32_t bar_, int tx, int ty, int tz)
+    __device__ __forceinline__ SrcGlobalPhiSmem(const DevParams<real> &P_, const Fields &Fd_, const NodeGeom &g_,
+                                                const preal *tile_base, uint32_t bar_, int tx, int ty, int tz)
         : P(P_), Fd(Fd_), g(g_), bar(bar_) {
         tile = tile_base + ((LF::D == 3 ? tz + 1 : 0) * TC::BOXY + ty + 1) * TC::BOXX + tx + TC::EPB;
         pcoff = ((unsigned)(g.z + P.pz) * (unsigned)P.ppy + (unsigned)(g.y + 1)) * (unsigned)P.ppx + (unsigned)(g.x + P.xpad);
     }
     __device__ __forceinline__ void phi_ready() const { mbar_wait(bar, 0); }
-    __device__ __forceinline__ real phi(int dx, int dy, int dz) const { return tile[dx + dy * TC::BOXX + dz * (TC::BOXX * TC::BOXY)]; }
-    __device__ __forceinline__ real phi_old() const { return __ldg(Fd.phi_old + pcoff); }
-    __device__ __forceinline__ real pdot_old() const { return Fd.pdot_in[g.n]; }
+    __device__ __forceinline__ preal phi(int dx, int dy, int dz) const { return tile[dx + dy * TC::BOXX + dz * (TC::BOXX * TC::BOXY)]; }
+    __device__ __forceinline__ preal phi_old() const { return __ldg(Fd.phi_old + pcoff); }
+    __device__ __forceinline__ real pdot_old() const { return real(Fd.pdot_in[g.n]); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real f() const { return pull_one<LF, I, real, BC, AGAIN>(Fd.f_in, (unsigned)P.N, g, P.bc_f, P.bc_p); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real s() const { return pull_one<LS, I, real, BC, AGAIN>(Fd.s_in, (unsigned)P.N, g, P.bc_s, P.bc_T); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real gg() const { return pull_one<LG, I, real, BC, AGAIN>(Fd.g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi); }
 };
 
-template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB>
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB, class Fields>
 __global__ void __launch_bounds__(BX *BY *BZ, MINB)
-k_main_phitma(const DevParams<real> P, const DevFields<real> Fd, const __grid_constant__ CUtensorMap phi_map) {
-    using TC = PhiTileCfg<real, LF::D, BX, BY, BZ>;
-    __shared__ __align__(128) real tile[TC::ELEMS];
+k_main_phitma(const DevParams<real> P, const Fields Fd, const __grid_constant__ CUtensorMap phi_map) {
+    using preal = typename Fields::preal;
+    using TC = PhiTileCfg<preal, LF::D, BX, BY, BZ>;
+    __shared__ __align__(128) preal tile[TC::ELEMS];
     __shared__ __align__(8) uint64_t bar;
     const int t = threadIdx.x;
     const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY, z0 = blockIdx.z * BZ;
@@ -63,10 +65,10 @@ k_main_phitma(const DevParams<real> P, const DevFields<real> Fd, const __grid_co
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
     const NodeGeom g = make_geom(P, x, y, z);
     if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) {
-        const SrcGlobalPhiSmem<LF, LG, LS, real, true, TC> src(P, Fd, g, tile, bar_a, tx, ty, tz);
+        const SrcGlobalPhiSmem<LF, LG, LS, real, true, TC, Fields> src(P, Fd, g, tile, bar_a, tx, ty, tz);
         node_update<LF, LG, LS, real, MODE>(P, Fd, g, src);
     } else {
-        const SrcGlobalPhiSmem<LF, LG, LS, real, false, TC> src(P, Fd, g, tile, bar_a, tx, ty, tz);
+        const SrcGlobalPhiSmem<LF, LG, LS, real, false, TC, Fields> src(P, Fd, g, tile, bar_a, tx, ty, tz);
         node_update<LF, LG, LS, real, MODE>(P, Fd, g, src);
     }
 }

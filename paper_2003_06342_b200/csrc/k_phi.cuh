@@ -10,9 +10,9 @@ namespace lbm {
 // Store phi of node g into the padded array and into every ghost image of that node (reading S8-iv):
 // periodic axis -> image one period away; zero-flux face -> mirror phi(-1) = phi(0); Dirichlet face with value v ->
 // phi(-1) = 2 v - phi(0).  Transforms compose in axis order x, y, z (what an axis-by-axis ghost fill would give).
-template <class real>
-__device__ __forceinline__ void store_phi_with_images(real *__restrict__ phi_pad, const DevParams<real> &P,
-                                                      const NodeGeom &g, real v) {
+template <class real, class preal>
+__device__ __forceinline__ void store_phi_with_images(preal *__restrict__ phi_pad, const DevParams<real> &P,
+                                                      const NodeGeom &g, preal v) {
     const long long pc = ((long long)(g.z + P.pz) * P.ppy + (g.y + 1)) * P.ppx + (g.x + P.xpad);
     phi_pad[pc] = v;
     const bool edge = g.lo[0] | g.hi[0] | g.lo[1] | g.hi[1] | (P.pz && (g.lo[2] | g.hi[2]));
@@ -45,19 +45,53 @@ __device__ __forceinline__ void store_phi_with_images(real *__restrict__ phi_pad
         for (int i1 = 0; i1 < cnt[1]; ++i1)
             for (int i0 = 0; i0 < cnt[0]; ++i0) {
                 if ((i0 | i1 | i2) == 0) continue;
-                real w = v;
-                if (kind[0][i0] == BC_ANTI) w = real(2) * bval[0][i0] - w;
-                if (kind[1][i1] == BC_ANTI) w = real(2) * bval[1][i1] - w;
-                if (kind[2][i2] == BC_ANTI) w = real(2) * bval[2][i2] - w;
+                preal w = v;
+                if (kind[0][i0] == BC_ANTI) w = preal(2) * preal(bval[0][i0]) - w;
+                if (kind[1][i1] == BC_ANTI) w = preal(2) * preal(bval[1][i1]) - w;
+                if (kind[2][i2] == BC_ANTI) w = preal(2) * preal(bval[2][i2]) - w;
                 phi_pad[pc + off[0][i0] + off[1][i1] + off[2][i2]] = w;
             }
 }
 
 // Each thread handles NPT nodes, NPT tiles apart along the slowest tiled axis (z in 3D, y in 2D); all 8 NPT loads are
 // issued before the first sum, which is what a latency-bound streaming kernel needs (measured: DESIGN.md "Kernels").
-template <class LG, class real, int BX, int BY, int BZ, int NPT>
+// phi^{n+1} = sum_i g_i + dt/2 Pdot in the type of the phi array (preal), so that with float populations and a double phi
+// the result carries only the storage rounding of the populations.  Plain sum when the values already are preal;
+// when an all-float kernel feeds a double phi the sum is an error-free float accumulation (Knuth two-sum: hi + lo is the
+// exact sum) widened once at the end -- two conversions per node instead of Q_g + 1 (F2F.F64.F32 issues at a fraction
+// of the FADD rate; K_phi on config 4: 0.479 -> see DESIGN.md "Kernels").
+__device__ __forceinline__ void two_sum(float &hi, float &lo, float v) {
+    const float s = __fadd_rn(hi, v);
+    const float bb = __fsub_rn(s, hi);
+    lo = __fadd_rn(lo, __fadd_rn(__fsub_rn(hi, __fsub_rn(s, bb)), __fsub_rn(v, bb)));
+    hi = s;
+}
+template <class preal, class real, class vreal, int Q>
+__device__ __forceinline__ preal phi_sum(const vreal (&gi)[Q], real hdt, vreal pd) {
+    if constexpr (std::is_same<vreal, float>::value && std::is_same<preal, double>::value) {
+        float hi = gi[0], lo = 0.0f;
+#pragma unroll
+        for (int i = 1; i < Q; ++i) two_sum(hi, lo, gi[i]);
+        const float pr = __fmul_rn((float)hdt, pd);
+        lo = __fadd_rn(lo, __fmaf_rn((float)hdt, pd, -pr));   // rounding error of the product, exact
+        two_sum(hi, lo, pr);
+        return (double)hi + (double)lo;
+    } else {
+        preal sum = preal(gi[0]);
+#pragma unroll
+        for (int i = 1; i < Q; ++i) sum += preal(gi[i]);
+        return sum + preal(hdt) * preal(pd);   // sum_i w_i = 1
+    }
+}
+
+// Each thread handles NPT nodes, NPT tiles apart along the slowest tiled axis (z in 3D, y in 2D); all 8 NPT loads are
+// issued before the first sum, which is what a latency-bound streaming kernel needs (measured: DESIGN.md "Kernels").
+// The pulled values are held in the arithmetic type `real` when that is the stored type (all-float kernels: no widening
+// before the error-free sum), else in preal.
+template <class LG, class real, int BX, int BY, int BZ, int NPT, class sreal, class preal>
 __global__ void __launch_bounds__(BX *BY *BZ)
-k_phi(const DevParams<real> P, const real *__restrict__ g_in, const real *__restrict__ pdot, real *__restrict__ phi_new) {
+k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, const sreal *__restrict__ pdot, preal *__restrict__ phi_new) {
+    using vreal = typename std::conditional<std::is_same<real, sreal>::value, real, preal>::type;
     constexpr bool ALONG_Z = LG::D == 3;
     const int t = threadIdx.x;
     const int x0 = blockIdx.x * BX;
@@ -66,8 +100,8 @@ k_phi(const DevParams<real> P, const real *__restrict__ g_in, const real *__rest
     const int x = x0 + t % BX, yb = y0 + (t / BX) % BY, zb = z0 + t / (BX * BY);
     if (x >= P.nx) return;
     const bool bc = tile_touches_bc(P, x0, y0, z0, BX, BY * (ALONG_Z ? 1 : NPT), BZ * (ALONG_Z ? NPT : 1));
-    real gi[NPT][LG::Q];
-    real pd[NPT];
+    vreal gi[NPT][LG::Q];
+    vreal pd[NPT];
     NodeGeom g[NPT];
     bool ok[NPT];
 #pragma unroll
@@ -76,39 +110,34 @@ k_phi(const DevParams<real> P, const real *__restrict__ g_in, const real *__rest
         ok[j] = y < P.ny && z < P.nz;
         if (ok[j]) {
             g[j] = make_geom(P, x, y, z);
-            if (bc) pull<LG, real, true>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
-            else pull<LG, real, false>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
-            pd[j] = __ldg(pdot + g[j].n);
+            if (bc) pull<LG, vreal, true>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
+            else pull<LG, vreal, false>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
+            pd[j] = vreal(__ldg(pdot + g[j].n));
         }
     }
 #pragma unroll
     for (int j = 0; j < NPT; ++j) {
-        if (ok[j]) {
-            real sum = gi[j][0];
-#pragma unroll
-            for (int i = 1; i < LG::Q; ++i) sum += gi[j][i];
-            store_phi_with_images(phi_new, P, g[j], sum + P.hdt * pd[j]);   // sum_i w_i = 1
-        }
+        if (ok[j]) store_phi_with_images(phi_new, P, g[j], phi_sum<preal>(gi[j], P.hdt, pd[j]));
     }
 }
 
 // Initialisation helper: copy a plain [z][y][x] phi into both padded buffers with ghost images.
-template <class real, int BX, int BY, int BZ>
+template <class real, int BX, int BY, int BZ, class sreal, class preal>
 __global__ void __launch_bounds__(BX *BY *BZ)
-k_phi_fill(const DevParams<real> P, const real *__restrict__ phi_plain, real *__restrict__ pad_a, real *__restrict__ pad_b) {
+k_phi_fill(const DevParams<real> P, const sreal *__restrict__ phi_plain, preal *__restrict__ pad_a, preal *__restrict__ pad_b) {
     const int t = threadIdx.x;
     const int x = blockIdx.x * BX + t % BX, y = blockIdx.y * BY + (t / BX) % BY, z = blockIdx.z * BZ + t / (BX * BY);
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
     const NodeGeom g = make_geom(P, x, y, z);
-    const real v = phi_plain[g.n];
+    const preal v = preal(phi_plain[g.n]);
     store_phi_with_images(pad_a, P, g, v);
     store_phi_with_images(pad_b, P, g, v);
 }
 
 // Debug / parity: streamed (post-pull, post-BC) populations of one lattice, all directions, to a [Q][N] scratch.
-template <class L, class real, int BX, int BY, int BZ>
+template <class L, class real, int BX, int BY, int BZ, class sreal>
 __global__ void __launch_bounds__(BX *BY *BZ)
-k_stream_only(const DevParams<real> P, const real *__restrict__ src, real *__restrict__ dst, int which) {
+k_stream_only(const DevParams<real> P, const sreal *__restrict__ src, sreal *__restrict__ dst, int which) {
     const int t = threadIdx.x;
     const int x = blockIdx.x * BX + t % BX, y = blockIdx.y * BY + (t / BX) % BY, z = blockIdx.z * BZ + t / (BX * BY);
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
@@ -118,7 +147,7 @@ k_stream_only(const DevParams<real> P, const real *__restrict__ src, real *__res
     else if (which == 1) pull<L, real, true>(src, (unsigned)P.N, g, P.bc_g, P.bc_phi, v);
     else pull<L, real, true>(src, (unsigned)P.N, g, P.bc_s, P.bc_T, v);
 #pragma unroll
-    for (int i = 0; i < L::Q; ++i) dst[(size_t)i * P.N + g.n] = v[i];
+    for (int i = 0; i < L::Q; ++i) dst[(size_t)i * P.N + g.n] = sreal(v[i]);
 }
 
 template <class real> __global__ void k_fill(real *__restrict__ dst, long long n, real v) {
@@ -127,14 +156,14 @@ template <class real> __global__ void k_fill(real *__restrict__ dst, long long n
 }
 
 // unpadded copy of phi (for lbm_read_macro)
-template <class real, int BX, int BY, int BZ>
+template <class real, int BX, int BY, int BZ, class sreal, class preal>
 __global__ void __launch_bounds__(BX *BY *BZ)
-k_phi_unpad(const DevParams<real> P, const real *__restrict__ pad, real *__restrict__ plain) {
+k_phi_unpad(const DevParams<real> P, const preal *__restrict__ pad, sreal *__restrict__ plain) {
     const int t = threadIdx.x;
     const int x = blockIdx.x * BX + t % BX, y = blockIdx.y * BY + (t / BX) % BY, z = blockIdx.z * BZ + t / (BX * BY);
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
     plain[(long long)z * P.nx * P.ny + (long long)y * P.nx + x] =
-        pad[((long long)(z + P.pz) * P.ppy + (y + 1)) * P.ppx + (x + P.xpad)];
+        sreal(pad[((long long)(z + P.pz) * P.ppy + (y + 1)) * P.ppx + (x + P.xpad)]);
 }
 
 }  // namespace lbm

@@ -66,20 +66,29 @@ template <class real> struct DevParams {
     real grav[3], force[3];
     real alpha_l, alpha_diff;            // alpha_g - alpha_l
     real M, om_g, cac;                   // mobility, 1/(M/(cs2g dt)+1/2), M*(4/W)/cs2g * c
+    double g_om, g_dt, g_c_cs2, g_inv_cs2, g_cac;   // constants of the g collision, which runs in the phi type (k_main.cuh)
     real LCp, CpL, T_sat, theta_I, pc_coef;   // L/Cp, Cp/L, 4/(A W^2)
     real eps_n2;
     int phase_change, latent_heat, prescribed_u;
 };
 
-template <class real> struct DevFields {
-    const real *f_in, *g_in, *s_in;   // post-collision populations of the previous level
-    real *f_out, *g_out, *s_out;      // post-collision populations of this level
-    const real *phi_new;              // padded, level n+1 (written by k_phi)
-    const real *phi_old;              // padded, level n
-    const real *pdot_in;              // production field of level n (the stored one, reading S3)
-    real *pdot;                       // production field of level n+1 (same array as pdot_in except in the fused variant)
-    real *u, *p, *T;                  // macro arrays: outputs (MODE_STEP_MACRO) or inputs (MODE_INIT)
+// Storage types are separate from the arithmetic type `real` of the kernels (include/lbm.h "precision"):
+//   sreal  populations, Pdot and the macro arrays (what streams through HBM every step);
+//   preal  the padded phi arrays.  phi is kept in double even when everything else is float: dphi/dt =
+//          (phi^{n+1} - phi^n)/dt (reading S4) is a difference of two O(1) numbers that enters T multiplied by L/Cp, so
+//          the rounding of a float phi (6e-8) is the largest single error of an all-float step.
+template <class sreal_, class preal_> struct DevFieldsT {
+    using sreal = sreal_;
+    using preal = preal_;
+    const sreal *f_in, *g_in, *s_in;   // post-collision populations of the previous level
+    sreal *f_out, *g_out, *s_out;      // post-collision populations of this level
+    const preal *phi_new;              // padded, level n+1 (written by k_phi)
+    const preal *phi_old;              // padded, level n
+    const sreal *pdot_in;              // production field of level n (the stored one, reading S3)
+    sreal *pdot;                       // production field of level n+1 (same array as pdot_in except in the fused variant)
+    sreal *u, *p, *T;                  // macro arrays: outputs (MODE_STEP_MACRO) or inputs (MODE_INIT)
 };
+template <class real> using DevFields = DevFieldsT<real, real>;   // one type throughout (fp64; the tma and fused variants)
 
 // ---- per-node geometry ------------------------------------------------------------------------------------
 // Element offsets are 32-bit: Q * N < 2^32 is checked by the host (lbm_create).
@@ -122,9 +131,9 @@ __device__ __forceinline__ float ld_again(const float *p) {
     asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
     return v;
 }
-template <bool AGAIN, class real> __device__ __forceinline__ real ld_pop(const real *p) {
-    if constexpr (AGAIN) return ld_again(p);
-    else return __ldg(p);
+template <bool AGAIN, class real, class sreal> __device__ __forceinline__ real ld_pop(const sreal *p) {
+    if constexpr (AGAIN) return real(ld_again(p));
+    else return real(__ldg(p));
 }
 
 // Pull-stream ONE direction of one lattice (theta* = theta(x + c_i dt, t + dt)).
@@ -132,16 +141,18 @@ template <bool AGAIN, class real> __device__ __forceinline__ real ld_pop(const r
 // BC = true : a link that leaves through a non-periodic face takes the post-collision opposite population of the
 //             same node: bounce-back or anti-bounce-back -v + 2 w_i value;
 //             tangential wrap first, lowest axis decides (reading S8).
-template <class L, int I, class real, bool BC, bool AGAIN = false>
-__device__ __forceinline__ real pull_one(const real *__restrict__ src, unsigned N, const NodeGeom &g,
-                                         const int (&bc)[3][2], const real (&val)[3][2]) {
+// `real` is the type the value is returned (and the anti-bounce-back evaluated) in; the stored type and the type of the
+// face values are deduced.
+template <class L, int I, class real, bool BC, bool AGAIN = false, class sreal, class vreal>
+__device__ __forceinline__ real pull_one(const sreal *__restrict__ src, unsigned N, const NodeGeom &g,
+                                         const int (&bc)[3][2], const vreal (&val)[3][2]) {
     constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I);
     const unsigned ns = (unsigned)I * N + g.sz[ez + 1] + g.sy[ey + 1] + g.sx[ex + 1];
     if constexpr (!BC || I == 0) {
-        return ld_pop<AGAIN>(src + ns);
+        return ld_pop<AGAIN, real>(src + ns);
     } else {
         int kind = BC_PERIODIC;
-        real v = real(0);
+        vreal v = vreal(0);
         if constexpr (ex != 0) {
             constexpr int side = ex > 0 ? 0 : 1;
             if ((side == 0 ? g.lo[0] : g.hi[0]) && bc[0][side] != BC_PERIODIC) { kind = bc[0][side]; v = val[0][side]; }
@@ -154,15 +165,15 @@ __device__ __forceinline__ real pull_one(const real *__restrict__ src, unsigned 
             constexpr int side = ez > 0 ? 0 : 1;
             if (kind == BC_PERIODIC && (side == 0 ? g.lo[2] : g.hi[2]) && bc[2][side] != BC_PERIODIC) { kind = bc[2][side]; v = val[2][side]; }
         }
-        if (kind == BC_PERIODIC) return ld_pop<AGAIN>(src + ns);
-        const real back = ld_pop<AGAIN>(src + (unsigned)L::opp(I) * N + g.n);
-        return kind == BC_BOUNCE ? back : real(2.0 * L::w(I)) * v - back;
+        if (kind == BC_PERIODIC) return ld_pop<AGAIN, real>(src + ns);
+        const real back = ld_pop<AGAIN, real>(src + (unsigned)L::opp(I) * N + g.n);
+        return kind == BC_BOUNCE ? back : real(2.0 * L::w(I)) * real(v) - back;
     }
 }
 
-template <class L, class real, bool BC>
-__device__ __forceinline__ void pull(const real *__restrict__ src, unsigned N, const NodeGeom &g,
-                                     const int (&bc)[3][2], const real (&val)[3][2], real (&out)[L::Q]) {
+template <class L, class real, bool BC, class sreal, class vreal>
+__device__ __forceinline__ void pull(const sreal *__restrict__ src, unsigned N, const NodeGeom &g,
+                                     const int (&bc)[3][2], const vreal (&val)[3][2], real (&out)[L::Q]) {
     static_for<L::Q>([&](auto ic) {
         constexpr int I = decltype(ic)::value;
         out[I] = pull_one<L, I, real, BC>(src, N, g, bc, val);

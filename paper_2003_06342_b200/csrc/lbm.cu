@@ -85,9 +85,11 @@ int validate(const lbm_params *p) {
 
 Layout make_layout(const lbm_params *p) {
     Layout L{};
-    const size_t es = p->precision == 64 ? 8 : 4;
+    const size_t es = p->precision == 64 ? 8 : 4;             // populations, Pdot, macros, scratch
+    const size_t esp = 8;                                     // phi is kept in double in every precision (include/lbm.h)
+    L.es = (int)es; L.es_phi = (int)esp;
     L.N = (long long)p->nx * p->ny * p->nz;
-    const int mult = (int)(16 / es);                          // TMA: row pitch and box starts are multiples of 16 bytes
+    const int mult = (int)(16 / esp);                         // TMA: row pitch and box starts are multiples of 16 bytes
     L.xpad = mult;                                            // node 0 sits 16 bytes into the padded row
     L.ppx = (p->nx + 2 * mult + mult - 1) / mult * mult;
     L.ppy = p->ny + 2;
@@ -96,16 +98,16 @@ Layout make_layout(const lbm_params *p) {
     L.phi_pad_elems = (size_t)L.ppx * L.ppy * L.ppz;
     const size_t N = (size_t)L.N;
     size_t o = 0;
-    auto take = [&](size_t elems) { size_t r = o; o = align_up(o + elems * es); return r; };
-    for (int b = 0; b < 2; ++b) L.off_f[b] = take(N * lattice_q(p->lat_f));
-    for (int b = 0; b < 2; ++b) L.off_g[b] = take(N * lattice_q(p->lat_g));
-    for (int b = 0; b < 2; ++b) L.off_s[b] = take(N * lattice_q(p->lat_s));
-    for (int b = 0; b < 2; ++b) L.off_phi[b] = take(L.phi_pad_elems);
-    for (int b = 0; b < 2; ++b) L.off_pdot[b] = take(N);   // second buffer: fused variant only
-    L.off_u = take(3 * N);
-    L.off_p = take(N);
-    L.off_T = take(N);
-    L.off_scratch = take(N);
+    auto take = [&](size_t elems, size_t esz) { size_t r = o; o = align_up(o + elems * esz); return r; };
+    for (int b = 0; b < 2; ++b) L.off_f[b] = take(N * lattice_q(p->lat_f), es);
+    for (int b = 0; b < 2; ++b) L.off_g[b] = take(N * lattice_q(p->lat_g), es);
+    for (int b = 0; b < 2; ++b) L.off_s[b] = take(N * lattice_q(p->lat_s), es);
+    for (int b = 0; b < 2; ++b) L.off_phi[b] = take(L.phi_pad_elems, esp);
+    for (int b = 0; b < 2; ++b) L.off_pdot[b] = take(N, es);   // second buffer: fused variant only
+    L.off_u = take(3 * N, es);
+    L.off_p = take(N, es);
+    L.off_T = take(N, es);
+    L.off_scratch = take(N, es);
     L.total = o;
     return L;
 }
@@ -152,6 +154,8 @@ template <class real> DevParams<real> make_dev_params(const lbm_params *p, const
     d.M = (real)p->M;
     d.om_g = (real)(1.0 / (p->M / (cs2g * p->dt) + 0.5));      // PAPER.md:236, Eq.(25)
     d.cac = (real)(p->M * (4.0 / p->W) * c / cs2g);            // Eq.(31b) counter term factor
+    d.g_om = 1.0 / (p->M / (cs2g * p->dt) + 0.5); d.g_dt = p->dt; d.g_c_cs2 = c / cs2g; d.g_inv_cs2 = 1.0 / cs2g;
+    d.g_cac = p->M * (4.0 / p->W) * c / cs2g;
     d.LCp = (real)(p->L_latent / p->Cp); d.CpL = (real)(p->Cp / p->L_latent);
     d.T_sat = (real)p->T_sat; d.theta_I = (real)p->theta_I;
     d.pc_coef = (real)(4.0 / (p->A * p->W * p->W));            // Eq.(18)
@@ -207,7 +211,7 @@ bool encode_rows(CUtensorMap *m, void *base, int es, int rank, const unsigned lo
 bool build_phi_tile_maps(lbm_ctx *c) {
     auto fn = get_encode_fn();
     if (!fn) return false;
-    const int es = c->P.precision == 64 ? 8 : 4;
+    const int es = c->L.es_phi;
     const int epb = 16 / es;
     const bool three_d = c->P.nz > 1;
     for (int b = 0; b < 2; ++b) {
@@ -226,7 +230,8 @@ bool build_phi_tile_maps(lbm_ctx *c) {
 }
 
 bool build_tma_maps(lbm_ctx *c) {
-    const int es = c->P.precision == 64 ? 8 : 4;
+    if (c->L.es != c->L.es_phi) return false;             // the all-TMA variant stages every array in one element type
+    const int es = c->L.es;
     const int epb = 16 / es;
     const int boxx = 128 + 2 * epb;                       // TmaCfg::BOXX
     if (((size_t)c->P.nx * es) % 16 != 0) return false;
@@ -297,7 +302,8 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         // (90% of the measured HBM peak on config 4); LBM_VARIANT=tma selects the TMA-staged persistent kernel.
         const char *v = getenv("LBM_VARIANT");
         c->use_tma = (v && strcmp(v, "tma") == 0) && build_tma_maps(c);
-        c->fused = (v && strcmp(v, "fused") == 0) && p->nz > 1 && !(p->halo[0] | p->halo[1]);   // slabs need the two phases
+        c->fused = (v && strcmp(v, "fused") == 0) && p->nz > 1 && !(p->halo[0] | p->halo[1]) &&   // slabs need the two phases
+                   L.es == L.es_phi;                                                              // one element type throughout
         const char *gr = getenv("LBM_GRAPH");   // "0" disables the CUDA-graph replay of small grids
         c->graph_ok = c->stream != nullptr && L.N <= (1ll << 21) && !(gr && strcmp(gr, "0") == 0);
         c->graph2 = nullptr; c->graph_launches = 0;
@@ -316,7 +322,7 @@ int lbm_init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, co
 int lbm_set_velocity(lbm_ctx *c, const void *h_u) {
     if (!c || !h_u || !(c->P.flags & LBM_FLAG_PRESCRIBED_U)) return LBM_E_INVALID;
     if (!c->inited) return LBM_E_STATE;
-    const size_t es = c->P.precision == 64 ? 8 : 4;
+    const size_t es = (size_t)c->L.es;
     CK(cudaMemcpyAsync(c->ws + c->L.off_u, h_u, 3 * (size_t)c->L.N * es, cudaMemcpyDefault, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return LBM_OK;

@@ -485,21 +485,36 @@ def test_fp32_populations_and_defaults(gpu, oracle_mod):
 
 
 # ---------------------------------------------------------------------------- fp32 variant
+def _rel_errs(sim, o):
+    return {name: _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30)
+            for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T"))}
+
+
 def test_fp32_variant_config5_reduced(gpu, oracle_mod):
+    """north_star: relative difference <= 1e-4 in the fp32 variant, all fields, at the config-5 horizon N = 220.
+    The phase-field path of the float kernels is wide (include/lbm.h "Precisions"): measured T 4.3e-6 / 1.2e-5 / 2.4e-5
+    at N = 20 / 50 / 220 (an all-float step gave 3.2e-5 / 1.2e-4 / 2.3e-4), phi 7.7e-6, u 2.6e-6, p 2.1e-6 at N = 220."""
     P, I = wl.config5_droplets(n=40, nspheres=6, rmin=4.0, rmax=8.0)
     o = oracle_mod.Oracle(P); o.init(I["phi"], I["T"])
     sim = gpu.LBM(P, 32); sim.init(I["phi"].astype(np.float32), I["T"].astype(np.float32))
-    # phi, u, p meet 1e-4 at the full horizon N = 220.  T meets it up to N = 20 only: dphi/dt = (phi^{n+1} - phi^n)/dt
-    # cancels to ~1e-7 absolute in fp32 and enters T multiplied by L/Cp = 10, and the model amplifies it (1.2e-4 at
-    # N = 50, 2.3e-4 at N = 220, measured) -- DESIGN.md "fp32 variant".
-    o.step(20); sim.step(20)
-    for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
-        rel = _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30)
-        assert rel <= REL32, (name, 20, rel)
-    o.step(200); sim.step(200)
-    for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
-        rel = _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30)
-        assert rel <= (5 * REL32 if name == "T" else REL32), (name, 220, rel)
+    done = 0
+    for h in (20, 220):
+        o.step(h - done); sim.step(h - done); done = h
+        errs = _rel_errs(sim, o)
+        assert all(v <= REL32 for v in errs.values()), (h, errs)
+    assert errs["T"] <= 0.5 * REL32, errs      # the margin the wide phase-field path buys (all-float: 2.3e-4)
+    sim.destroy(); o.close()
+
+
+def test_fp32_variant_walls_and_phase_change(gpu, oracle_mod):
+    """fp32 on the film-boiling set-up (z walls, Dirichlet T, gravity, phase change): 1e-4 inside the horizon of the
+    workload (the film amplifies round-off, fp64 horizon N <= 100 on this grid)."""
+    P, I = wl.config4_film3d(nx=40, ny=24, nz=32, h0=10.0, amp=2.0)
+    o = oracle_mod.Oracle(P); o.init(I["phi"], I["T"])
+    sim = gpu.LBM(P, 32); sim.init(I["phi"].astype(np.float32), I["T"].astype(np.float32))
+    o.step(50); sim.step(50)
+    errs = _rel_errs(sim, o)
+    assert all(v <= REL32 for v in errs.values()), errs
     sim.destroy(); o.close()
 
 
