@@ -236,11 +236,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     //    Evaluated in the type of the phi arrays (greal = preal): sum_i g*_i is the phi of the next level, and what its
     //    rounding adds to dphi/dt reaches T multiplied by L/Cp.
     {
-#ifdef LBM_G_NARROW
-        using greal = real;
-#else
         using greal = preal;
-#endif
         const greal om_g = greal(P.g_om), dtg = greal(P.g_dt);   // constants carried in double: no widening per node
         const greal om = MODE == MODE_INIT ? greal(1) : om_g;
         const greal a = MODE == MODE_INIT ? greal(0) : greal(1) - om_g;

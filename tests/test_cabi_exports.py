@@ -45,7 +45,9 @@ def test_workspace_bytes_accounting(lib):
     lower = (2 * 33 + 8) * n * 8 + 2 * 258 * 258 * 514 * 8
     assert lower <= b64 <= lower * 1.001
     b32 = binding.lbm_workspace_bytes(P, 32)
-    assert abs(b32 / b64 - 0.5) < 1e-3
+    # float populations, Pdot, macros, scratch; the two padded phi arrays stay double (include/lbm.h "Precisions")
+    lower32 = (2 * 33 + 8) * n * 4 + 2 * 258 * 258 * 514 * 8
+    assert lower32 <= b32 <= lower32 * 1.001
     assert b64 < 180e9
 
 

@@ -386,6 +386,46 @@ def test_config5_full_size_384_periodic_replica(gpu, oracle_mod):
         assert err <= TOL64, (name, err)
 
 
+def test_config5_128_full_horizon_both_precisions(gpu, oracle_mod):
+    """BASELINE.json configs[4] at 128^3 and its full horizon N = 220 (20 warm-up + 200 timed steps), in the launch
+    configuration bench.py times (wide tiles), fp64 <= 1e-10 and fp32 <= 1e-4 relative on every field.
+    A 64^3 droplet field replicated 2x2x2 in the periodic box evolves as the replicated 64^3 solution of the oracle."""
+    Ps, Is = wl.config5_droplets(n=64, nspheres=8, rmin=6.0, rmax=12.0)
+    P = dict(Ps, nx=128, ny=128, nz=128)
+    phi = np.tile(Is["phi"], (2, 2, 2)); T = np.tile(Is["T"], (2, 2, 2))
+    o = oracle_mod.Oracle(Ps); o.init(Is["phi"], Is["T"]); o.step(220)
+    ref = o.read_macro(); o.close()
+    for prec in (64, 32):
+        dt = np.float64 if prec == 64 else np.float32
+        sim = gpu.LBM(P, prec); sim.init(phi.astype(dt), T.astype(dt)); sim.step(220)
+        got = sim.read_macro(); sim.destroy()
+        for a, r, name in zip(got, ref, ("phi", "u", "p", "T")):
+            full = np.tile(r, (1, 2, 2, 2) if a.ndim == 4 else (2, 2, 2))
+            err = _maxabs(a, full)
+            if prec == 64:
+                assert err <= TOL64, (name, err)
+            else:
+                assert err / float(np.abs(full).max()) <= REL32, (name, err / float(np.abs(full).max()))
+
+
+def test_config4_full_size_fp32(gpu, oracle_mod):
+    """The fp32 kernels on the full 256x256x512 film-boiling grid (bench.py --precision 32): 64x64 pattern replicated 4x4,
+    relative error <= 1e-4 on every field after 10 steps against the replicated 64x64x512 oracle solution."""
+    Ps, Is = wl.config4_film3d(nx=64, ny=64, nz=512)
+    P, _ = wl.config4_film3d(nx=8, ny=8, nz=8)
+    P.update(nx=256, ny=256, nz=512)
+    sim = gpu.LBM(P, 32)
+    sim.init(np.tile(Is["phi"], (1, 4, 4)).astype(np.float32), np.tile(Is["T"], (1, 4, 4)).astype(np.float32))
+    sim.step(10)
+    got = sim.read_macro(); sim.destroy()
+    o = oracle_mod.Oracle(Ps); o.init(Is["phi"], Is["T"]); o.step(10)
+    ref = o.read_macro(); o.close()
+    for a, r, name in zip(got, ref, ("phi", "u", "p", "T")):
+        full = np.tile(r, (1, 1, 4, 4) if a.ndim == 4 else (1, 4, 4))
+        rel = _maxabs(a, full) / float(np.abs(full).max())
+        assert rel <= REL32, (name, rel)
+
+
 def test_config3_full_size_periodic_replica(gpu, oracle_mod):
     """Config 3 at full size (512 x 1024, 2D film boiling): 128-periodic pattern in x replicated 4 times."""
     Ps, Is = wl.config3_film2d(nx=128, ny=1024, h0=64.0, amp=4.0)
