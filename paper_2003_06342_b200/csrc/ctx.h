@@ -73,6 +73,8 @@ struct lbm_ctx {
     CUtensorMap map_f[2], map_g[2], map_s[2], map_phi[2], map_pdot;
     // gather kernel with the phi halo tile staged by TMA: one box per CTA
     bool phi_tma;
+    // ... and the pulled populations, phi^n, Pdot staged by per-thread cp.async (k_main_smem.cuh)
+    bool pops_smem;
     // fused variant: K_phi folded into K_main (3D only), Pdot double-buffered
     bool fused;
     // CUDA graph of two consecutive plain steps, for launch-bound (small) grids

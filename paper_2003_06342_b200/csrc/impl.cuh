@@ -5,6 +5,7 @@
 #include "k_main.cuh"
 #include "k_main_fused.cuh"
 #include "k_main_phitma.cuh"
+#include "k_main_smem.cuh"
 #include "k_main_tma.cuh"
 #include "k_phi.cuh"
 
@@ -98,6 +99,25 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
             }
         }
         if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU) {
+            if (c->phi_tma && c->pops_smem) {
+                using C = SmemCfg<LF, LG, LS, sreal, preal, T::BX, T::BY, T::BZ>;
+                auto kern = k_main_smem<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB, Fields>;
+                static bool attr_set = false;
+                if (!attr_set) {
+                    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::BYTES));
+                    // shared-memory carve-out: just enough for MINB resident CTAs (+1 KB each that the driver reserves), the rest
+                    // stays L1 -- the shifted pulls of neighbouring warps share sectors there (measured on config 4, K_main ms:
+                    // 60 KB of L1: 2.89, 92 KB: 2.82, and 3.75 with the maximum carve-out)
+                    const char *co = getenv("LBM_CARVEOUT");   // tuning only
+                    const int pct = (co && *co) ? atoi(co) : (int)((MINB * (C::BYTES + 1024) * 100 + 233471) / 233472);
+                    CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, pct > 100 ? 100 : pct));
+                    attr_set = true;
+                }
+                kern<<<grid_for<T>(c->P), NT, C::BYTES, c->stream>>>(dev_params<real>(c), F, c->map_phi_tile[pnew]);
+                c->launches++;
+                CK(cudaGetLastError());
+                return LBM_OK;
+            }
             if (c->phi_tma) {
                 k_main_phitma<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB>
                     <<<grid_for<T>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F, c->map_phi_tile[pnew]);

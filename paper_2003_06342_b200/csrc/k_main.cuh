@@ -34,6 +34,8 @@ template <class LF, class LG, class LS, class real, bool BC, class Fields = DevF
         pcoff = ((unsigned)(g.z + P.pz) * (unsigned)P.ppy + (unsigned)(g.y + 1)) * (unsigned)P.ppx + (unsigned)(g.x + P.xpad);
         pc = Fd.phi_new + pcoff;
     }
+    __device__ __forceinline__ void pops_ready() const {}
+    __device__ __forceinline__ void f_ready() const {}
     __device__ __forceinline__ void phi_ready() const {}
     __device__ __forceinline__ preal phi(int dx, int dy, int dz) const { return __ldg(pc + (dx + dy * P.ppx + dz * (int)P.pplane)); }
     __device__ __forceinline__ preal phi_old() const { return __ldg(Fd.phi_old + pcoff); }
@@ -53,6 +55,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     const unsigned N = (unsigned)P.N;
 
     // ---- H5 (first half): zeroth moment of s.  Loaded first so that these loads are in flight during the stencil.
+    src.pops_ready();   // staged variants: the node's asynchronous copies have landed
     real sum_s = real(0);
     if constexpr (MODE != MODE_INIT) {
         static_for<LS::Q>([&](auto ic) { sum_s += src.template s<decltype(ic)::value>(); });
@@ -111,6 +114,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     } else {
         // ---- H4: NS moments (Eq.28a), accumulated as the pulled values arrive
         real m0 = real(0), mx = real(0), my = real(0), mz = real(0);
+        src.f_ready();   // staged variants: the second group of copies (f, g) has landed
         static_for<LF::Q>([&](auto ic) {
             constexpr int I = decltype(ic)::value;
             const real fi = src.template f<I>();

@@ -75,6 +75,8 @@ template <class LF, class LG, class LS, class real, bool BC, int PX, int PY> str
         : P(P_), Fd(Fd_), g(g_), ring(ring_), slot(slot_), off((ty + 1) * PX + tx + 1) {
         pcoff = ((unsigned)(g.z + P.pz) * (unsigned)P.ppy + (unsigned)(g.y + 1)) * (unsigned)P.ppx + (unsigned)(g.x + P.xpad);
     }
+    __device__ __forceinline__ void pops_ready() const {}
+    __device__ __forceinline__ void f_ready() const {}
     __device__ __forceinline__ void phi_ready() const {}
     __device__ __forceinline__ real phi(int dx, int dy, int dz) const {
         return ring[((slot + dz) & 3) * (PX * PY) + off + dx + dy * PX];

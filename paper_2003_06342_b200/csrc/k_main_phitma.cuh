@@ -32,6 +32,8 @@ template <class LF, class LG, class LS, class real, bool BC, class TC, class Fie
         tile = tile_base + ((LF::D == 3 ? tz + 1 : 0) * TC::BOXY + ty + 1) * TC::BOXX + tx + TC::EPB;
         pcoff = ((unsigned)(g.z + P.pz) * (unsigned)P.ppy + (unsigned)(g.y + 1)) * (unsigned)P.ppx + (unsigned)(g.x + P.xpad);
     }
+    __device__ __forceinline__ void pops_ready() const {}
+    __device__ __forceinline__ void f_ready() const {}
     __device__ __forceinline__ void phi_ready() const { mbar_wait(bar, 0); }
     __device__ __forceinline__ preal phi(int dx, int dy, int dz) const { return tile[dx + dy * TC::BOXX + dz * (TC::BOXX * TC::BOXY)]; }
     __device__ __forceinline__ preal phi_old() const { return __ldg(Fd.phi_old + pcoff); }

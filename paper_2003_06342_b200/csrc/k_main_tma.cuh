@@ -92,6 +92,8 @@ template <class LF, class LG, class LS, class real> struct SrcTma {
     __device__ __forceinline__ SrcTma(const DevParams<real> &P_, const DevFields<real> &Fd_, const NodeGeom &g_,
                                       const real *st_, int tx_, int ry_)
         : P(P_), Fd(Fd_), g(g_), st(st_), tx(tx_), ry(ry_) {}
+    __device__ __forceinline__ void pops_ready() const {}
+    __device__ __forceinline__ void f_ready() const {}
     __device__ __forceinline__ void phi_ready() const {}
     __device__ __forceinline__ real phi(int dx, int dy, int dz) const {
         const int row = C::ROW_PHI + (C::D == 3 ? (dz + 1) : 0) * (C::TY + 2) + ry + 1 + dy;

@@ -309,6 +309,12 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         c->graph2 = nullptr; c->graph_launches = 0;
         const char *ph = getenv("LBM_PHI");   // phi halo tile of the gather kernel: "tma" (shared memory) or "ldg"
         c->phi_tma = !c->use_tma && !c->fused && !(ph && strcmp(ph, "ldg") == 0) && build_phi_tile_maps(c);   // default: TMA
+        // pulled populations of the gather kernel: staged in shared memory by cp.async (k_main_smem.cuh) where that measured
+        // faster -- fp64 (+3..9% on every large grid) and fp32 in 2D (+8%); fp32 3D stays on the register gather (-1..5%).
+        // LBM_POPS=smem | ldg overrides.
+        const char *pp = getenv("LBM_POPS");
+        const bool smem_default = p->precision == 64 || p->nz == 1;
+        c->pops_smem = c->phi_tma && (pp ? strcmp(pp, "smem") == 0 : smem_default);
     }
     *out = c;
     return LBM_OK;
@@ -388,7 +394,7 @@ int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *ste
 
 long long lbm_step_count(const lbm_ctx *c) { return c ? c->nsteps : -1; }
 long long lbm_launch_count(const lbm_ctx *c) { return c ? c->launches : -1; }
-const char *lbm_variant(const lbm_ctx *c) { return c ? (c->fused ? "fused" : c->use_tma ? "tma" : (c->phi_tma ? "gather+phi-tma" : "direct")) : ""; }
+const char *lbm_variant(const lbm_ctx *c) { return c ? (c->fused ? "fused" : c->use_tma ? "tma" : (c->phi_tma ? (c->pops_smem ? "gather+smem" : "gather+phi-tma") : "direct")) : ""; }
 int lbm_last_cuda_error(void) { return g_last_cuda_error; }
 
 const char *lbm_strerror(int code) {

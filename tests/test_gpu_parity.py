@@ -175,22 +175,42 @@ def test_minimal_grids(gpu, oracle_mod):
 
 
 # ---------------------------------------------------------------------------- K_main variants
-def test_default_variant_stages_phi_by_tma_and_ldg_variant_agrees(gpu, oracle_mod, monkeypatch):
-    """Default K_main: gather kernel whose phi halo tile arrives by one TMA box per CTA; LBM_PHI=ldg reads phi through
-    L1 instead.  Both must match the oracle (the other tests in this file run the default)."""
-    P = wl.base_params(40, 10, 7, grav=[1e-4, 0.0, -2e-4])
-    sim = gpu.LBM(P, 64)
-    assert sim.variant == "gather+phi-tma"
-    sim.destroy()
-    monkeypatch.setenv("LBM_PHI", "ldg")
-    sim = gpu.LBM(P, 64)
-    assert sim.variant == "direct"
-    sim.destroy()
-    _run_parity(gpu, oracle_mod, P, _random_state(P, 34), [1, 12], label="ldg 3d periodic")
-    P = wl.base_params(40, 20, 1, grav=[0.0, -1e-4, 0.0])
-    P["bc_f"][1] = ["wall", "wall"]; P["bc_g"][1] = ["zeroflux", "dirichlet"]; P["bc_s"][1] = ["dirichlet", "zeroflux"]
-    P["bc_phi"][1] = [0.0, 1.0]; P["bc_T"][1] = [0.7, 0.0]
-    _run_parity(gpu, oracle_mod, P, _random_state(P, 35), [1, 12], label="ldg 2d walls")
+def test_k_main_variants_by_staging(gpu, oracle_mod, monkeypatch):
+    """K_main by what it stages in shared memory.  Default in fp64 (and fp32 2D): "gather+smem", phi halo tile by one TMA box
+    per CTA and the node's populations, phi^n, Pdot by per-thread cp.async (k_main_smem.cuh); fp32 3D: "gather+phi-tma"
+    (populations gathered into registers).  LBM_POPS=ldg / LBM_PHI=ldg select the plainer kernels.  Every one must match the
+    oracle on periodic and walled, 2D and 3D, narrow- and wide-tile grids (the other tests in this file run the defaults)."""
+    P3 = wl.base_params(40, 10, 7, grav=[1e-4, 0.0, -2e-4])                     # narrow tiles, ragged
+    P3w = wl.base_params(256, 6, 5, grav=[1e-4, 0.0, -2e-4], force=[0.0, 1e-5, 0.0])   # wide tiles, two per row
+    P2 = wl.base_params(40, 20, 1, grav=[0.0, -1e-4, 0.0])
+    P2["bc_f"][1] = ["wall", "wall"]; P2["bc_g"][1] = ["zeroflux", "dirichlet"]; P2["bc_s"][1] = ["dirichlet", "zeroflux"]
+    P2["bc_phi"][1] = [0.0, 1.0]; P2["bc_T"][1] = [0.7, 0.0]
+    P2w = wl.base_params(256, 12, 1, grav=[1e-4, -1e-4, 0.0], lat_s="D2Q9")   # wide tiles, three D2Q9 lattices
+    P3z = wl.base_params(128, 6, 9, grav=[0.0, 0.0, -1e-4])                       # z walls under wide tiles
+    P3z["bc_f"][2] = ["wall", "wall"]; P3z["bc_g"][2] = ["zeroflux", "zeroflux"]; P3z["bc_s"][2] = ["dirichlet", "dirichlet"]
+    P3z["bc_T"][2] = [1.0, 0.0]
+    cases = ((P3, 34), (P3w, 44), (P2, 35), (P2w, 45), (P3z, 46))
+    for env, want64, want32_3d in (({}, "gather+smem", "gather+phi-tma"), ({"LBM_POPS": "ldg"}, "gather+phi-tma", "gather+phi-tma"),
+                                   ({"LBM_POPS": "smem"}, "gather+smem", "gather+smem"), ({"LBM_PHI": "ldg"}, "direct", "direct")):
+        for k in ("LBM_POPS", "LBM_PHI"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        sim = gpu.LBM(P3, 64); assert sim.variant == want64, (env, sim.variant); sim.destroy()
+        sim = gpu.LBM(P3, 32); assert sim.variant == want32_3d, (env, sim.variant); sim.destroy()
+        for P, seed in cases:
+            _run_parity(gpu, oracle_mod, P, _random_state(P, seed), [1, 12], label="%s %dx%dx%d" % (env, P["nx"], P["ny"], P["nz"]))
+    # fp32 with the staged kernel (3D opt-in, 2D default): inside the fp32 bar
+    monkeypatch.delenv("LBM_PHI", raising=False)
+    monkeypatch.setenv("LBM_POPS", "smem")
+    for P, seed in ((P3w, 44), (P2w, 45)):
+        init = _random_state(P, seed)
+        o = oracle_mod.Oracle(P); o.init(*init); o.step(12)
+        sim = gpu.LBM(P, 32); sim.init(*[a.astype(np.float32) for a in init]); sim.step(12)
+        assert sim.variant == "gather+smem"
+        for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
+            assert _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30) <= REL32, name
+        sim.destroy(); o.close()
 
 
 def test_cuda_graph_replay_on_side_stream(gpu, oracle_mod):
