@@ -1,7 +1,7 @@
 // K_main, gather variant with EVERY input of the node staged in shared memory: the phi^{n+1} halo tile by one TMA box per CTA
-// (as k_main_phitma.cuh) and the 33 (3D) / 23 (2D) pulled populations, phi^n and Pdot by per-thread asynchronous copies
+// (as k_main_phitma.cuh) and the pulled f and s populations (26 in 3D; g only with LBM_SMEM_STAGE_G), phi^n and Pdot by per-thread asynchronous copies
 // (cp.async -> LDGSTS) into the thread's own column of a [value][thread] array.  All of a thread's loads are in flight at once
-// without occupying registers (Little's law: 16 warps x 35 x 8 B = 143 KB in flight per SM), and the second read of every
+// without occupying registers (Little's law: 16 warps x 32 lanes x 28 x 8 B = 115 KB in flight per SM), and the second read of every
 // population at collision time is a shared-memory load instead of an L2 round trip (the 200 KB L1 does not hold the
 // 16 x 18 KB working set of the gather kernel: its measured L1 hit rate is 5%).  Tiles that touch a non-periodic face take
 // the gather path of k_main_phitma.cuh (boundary rules select other addresses); the choice is tile-uniform.
