@@ -47,12 +47,14 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     static constexpr int NTP = TP::BX * TP::BY * TP::BZ;
     // Threads per SM the register allocation is bounded for (__launch_bounds__ minimum CTAs = threads / NT), measured:
     //   fp64 3D: 512 (128 registers, no spill on the interior path); more spills cost more than the warps bring
-    //   fp64 2D, 128-thread CTAs: 896 with the D2Q5 heat lattice (72 registers), 640 with D2Q9 (96); 256-thread tiles 768
+    //   fp64 2D, 128-thread CTAs: 640 (96 registers; K_main with staged populations on 4096x3072, D2Q5 heat lattice:
+    //            512 / 640 / 768 / 896 / 1024 threads: 0.785 / 0.752 / 0.754 / 0.792 / 0.854 ms; three D2Q9: 640 best);
+    //            256-thread tiles 768
     //   fp32   : 1024 (64 registers; +25% over 512 although a few values spill); 2D 128-thread CTAs 1280 (48 registers)
 #ifndef LBM_THREADS3D
 #define LBM_THREADS3D 512
 #endif
-    static constexpr int THREADS64 = D == 3 ? LBM_THREADS3D : (NT == 128 ? (LS::Q == 5 ? 896 : 640) : 768);
+    static constexpr int THREADS64 = D == 3 ? LBM_THREADS3D : (NT == 128 ? 640 : 768);
     static constexpr int THREADS32 = (D == 2 && NT == 128) ? 1280 : 1024;
     static constexpr int MINB = (sizeof(real) == 8 ? THREADS64 : THREADS32) / NT;
 #ifndef LBM_PHI_NPT

@@ -1,7 +1,8 @@
 // K_main (steps H2..H7): one thread per lattice node.  Citations are PAPER.md:<line>; readings (G*/S*) are listed in
 // DESIGN.md.  Populations are NOT held in registers across the step: the moments are accumulated while the pulled
-// values stream in, and every population is read again (L1 hit, or shared memory in the TMA variant) at the point
-// where it is collided.  That keeps the live state at ~50 doubles and lets two 256-thread CTAs share an SM.
+// values stream in, and every population is read again at the point where it is collided -- from the thread's
+// shared-memory column in the default kernel (k_main_smem.cuh), through L1/L2 in the register-gather kernels.  That keeps
+// the live state at ~50 doubles: 128 registers, four 128-thread CTAs per SM.
 #pragma once
 
 #include "kernels.cuh"

@@ -298,8 +298,9 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
     c->pd = make_dev_params<double>(p, L);
     c->pf = make_dev_params<float>(p, L);
     c->num_sms = prop.multiProcessorCount;
-    {   // K_main variant, chosen by measurement: the gather kernel at 2 CTAs/SM is the default
-        // (90% of the measured HBM peak on config 4); LBM_VARIANT=tma selects the TMA-staged persistent kernel.
+    {   // K_main variant, chosen by measurement: the gather kernel with the phi tile by TMA and the
+        // populations staged by cp.async is the default; LBM_VARIANT=tma selects the all-TMA persistent kernel, =fused the
+        // single-kernel step.
         const char *v = getenv("LBM_VARIANT");
         c->use_tma = (v && strcmp(v, "tma") == 0) && build_tma_maps(c);
         c->fused = (v && strcmp(v, "fused") == 0) && p->nz > 1 && !(p->halo[0] | p->halo[1]) &&   // slabs need the two phases
