@@ -50,12 +50,13 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     //   fp64 2D, 128-thread CTAs: 640 (96 registers; K_main with staged populations on 4096x3072, D2Q5 heat lattice:
     //            512 / 640 / 768 / 896 / 1024 threads: 0.785 / 0.752 / 0.754 / 0.792 / 0.854 ms; three D2Q9: 640 best);
     //            256-thread tiles 768
-    //   fp32   : 1024 (64 registers; +25% over 512 although a few values spill); 2D 128-thread CTAs 1280 (48 registers)
+    //   fp32   : 1024 (64 registers; +25% over 512 although a few values spill); 2D with staged populations on 4096x3072,
+    //            768 / 1024 / 1280 / 1536 threads: 0.481 / 0.470 / 0.506 / 0.570 ms (three D2Q9: 0.541 / 0.533 / 0.604 / 0.778)
 #ifndef LBM_THREADS3D
 #define LBM_THREADS3D 512
 #endif
     static constexpr int THREADS64 = D == 3 ? LBM_THREADS3D : (NT == 128 ? 640 : 768);
-    static constexpr int THREADS32 = (D == 2 && NT == 128) ? 1280 : 1024;
+    static constexpr int THREADS32 = 1024;
     static constexpr int MINB = (sizeof(real) == 8 ? THREADS64 : THREADS32) / NT;
 #ifndef LBM_PHI_NPT
 #define LBM_PHI_NPT 2
