@@ -181,7 +181,9 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
             F.pdot = wsp<real>(c, c->L.off_pdot[1 - in]);
             const dim3 grid((c->P.nx + FusedCfg::BX - 1) / FusedCfg::BX, (c->P.ny + FusedCfg::BY - 1) / FusedCfg::BY,
                             (c->P.nz + FusedCfg::LZ - 1) / FusedCfg::LZ);
-            k_main_fused<LF, LG, LS, real, MODE, FusedCfg::BX, FusedCfg::BY, FusedCfg::LZ, MINB>
+            // register bound: the same threads per SM as K_main, in CTAs of BX x BY threads
+            constexpr int FMINB = (sizeof(real) == 8 ? THREADS64 : THREADS32) / (FusedCfg::BX * FusedCfg::BY);
+            k_main_fused<LF, LG, LS, real, MODE, FusedCfg::BX, FusedCfg::BY, FusedCfg::LZ, FMINB>
                 <<<grid, FusedCfg::BX * FusedCfg::BY, 0, c->stream>>>(dev_params<real>(c), F, wsp<real>(c, c->L.off_phi[pnew]));
             c->launches++;
             CK(cudaGetLastError());
