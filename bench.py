@@ -243,7 +243,7 @@ def run_ours(args):
     q = {"D2Q5": 5, "D2Q9": 9, "D3Q7": 7, "D3Q19": 19, "D3Q15": 15}
     Q = q[P["lat_f"]] + q[P["lat_g"]] + q[P["lat_s"]]
     main_vals = (Q + 3) + (Q + 1)                    # reads: pops, phi^{n+1}, phi^n, Pdot; writes: pops, Pdot
-    phi_vals = q[P["lat_g"]] + 1 + 1
+    phi_vals = q[P["lat_g"]] + 1                    # reads: g; write: phi (dt/2 Pdot rides in the stored rest population)
     main_bytes = (main_vals * es + 2 * (8 - es)) * N    # the two phi values are doubles in both precisions
     main_ms = ms_main / max(nsteps_timed, 1)
     phi_ms = ms_phi / max(nsteps_timed, 1)

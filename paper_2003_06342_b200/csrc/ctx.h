@@ -70,7 +70,7 @@ struct lbm_ctx {
     // TMA variant of K_main: tensor maps of both buffers of every input array
     bool use_tma;
     int num_sms;
-    CUtensorMap map_f[2], map_g[2], map_s[2], map_phi[2], map_pdot;
+    CUtensorMap map_f[2], map_g[2], map_s[2], map_phi[2], map_pdot[2];
     // gather kernel with the phi halo tile staged by TMA: one box per CTA
     bool phi_tma;
     // ... and the pulled populations, phi^n, Pdot staged by per-thread cp.async (k_main_smem.cuh)

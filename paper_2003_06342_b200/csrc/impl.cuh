@@ -73,8 +73,10 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         F.s_in = wsp<sreal>(c, c->L.off_s[in]);  F.s_out = wsp<sreal>(c, c->L.off_s[out]);
         F.phi_new = wsp<preal>(c, c->L.off_phi[phi_new]);
         F.phi_old = wsp<preal>(c, c->L.off_phi[phi_old]);
-        F.pdot = wsp<sreal>(c, c->L.off_pdot[0]);
-        F.pdot_in = F.pdot;
+        // the production field lives with its population buffer: level n in [in], level n+1 into [out] (the rest population
+        // of g in a buffer carries dt/2 Pdot of the SAME buffer, k_main.cuh)
+        F.pdot_in = wsp<sreal>(c, c->L.off_pdot[in]);
+        F.pdot = wsp<sreal>(c, c->L.off_pdot[out]);
         F.u = wsp<sreal>(c, c->L.off_u); F.p = wsp<sreal>(c, c->L.off_p); F.T = wsp<sreal>(c, c->L.off_T);
         return F;
     }
@@ -91,7 +93,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
                 }
                 TmaMaps M;
                 M.f = c->map_f[in]; M.g = c->map_g[in]; M.s = c->map_s[in];
-                M.phi_new = c->map_phi[pnew]; M.phi_old = c->map_phi[1 - pnew]; M.pdot = c->map_pdot;
+                M.phi_new = c->map_phi[pnew]; M.phi_old = c->map_phi[1 - pnew]; M.pdot = c->map_pdot[in];
                 const int nxt = (c->P.nx + C::TX - 1) / C::TX, nyt = (c->P.ny + C::TY - 1) / C::TY;
                 const long long ntiles = (long long)nxt * nyt * c->P.nz;
                 const unsigned grid = (unsigned)(ntiles < c->num_sms ? ntiles : c->num_sms);
@@ -177,8 +179,6 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     struct FusedCfg { static constexpr int BX = LBM_FBX, BY = LBM_FBY, LZ = LBM_FLZ; };
     template <int MODE> static int launch_fused(lbm_ctx *c, Fields F, int in, int pnew) {
         if constexpr (D == 3 && UNIFORM) {
-            F.pdot_in = wsp<real>(c, c->L.off_pdot[in]);
-            F.pdot = wsp<real>(c, c->L.off_pdot[1 - in]);
             const dim3 grid((c->P.nx + FusedCfg::BX - 1) / FusedCfg::BX, (c->P.ny + FusedCfg::BY - 1) / FusedCfg::BY,
                             (c->P.nz + FusedCfg::LZ - 1) / FusedCfg::LZ);
             // register bound: the same threads per SM as K_main, in CTAs of BX x BY threads
@@ -200,8 +200,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         dim3 gphi = grid_for<TP>(c->P);
         if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
         k_phi<LG, real, TP::BX, TP::BY, TP::BZ, PHI_NPT><<<gphi, NTP, 0, c->stream>>>(
-            P, (const sreal *)wsp<sreal>(c, c->L.off_g[in]), (const sreal *)wsp<sreal>(c, c->L.off_pdot[0]),
-            wsp<preal>(c, c->L.off_phi[pnew]));
+            P, (const sreal *)wsp<sreal>(c, c->L.off_g[in]), wsp<preal>(c, c->L.off_phi[pnew]));
         c->launches++;
         CK(cudaGetLastError());
         return LBM_OK;
@@ -304,8 +303,18 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
 
     template <class L> static int read_pops_one(lbm_ctx *c, int which, int stage, const size_t (&off)[2], void *h) {
         const size_t N = (size_t)c->L.N, bytes = (size_t)L::Q * N * sizeof(sreal);
+        const bool is_g = which == LBM_POPS_G;
         if (stage == LBM_STAGE_POSTCOLLISION) {
             CK(cudaMemcpyAsync(h, wsp<sreal>(c, off[c->cur]), bytes, cudaMemcpyDefault, c->stream));
+            if (is_g) {   // the stored rest population carries dt/2 Pdot of its buffer (k_main.cuh): hand out g*_0 itself
+                sreal *scratch = wsp<sreal>(c, c->L.off_scratch);
+                k_unfold_g0<real, sreal><<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(
+                    scratch, (const sreal *)wsp<sreal>(c, off[c->cur]), (const sreal *)wsp<sreal>(c, c->L.off_pdot[c->cur]),
+                    (long long)N, dev_params<real>(c).hdt);
+                c->launches++;
+                CK(cudaGetLastError());
+                CK(cudaMemcpyAsync(h, scratch, N * sizeof(sreal), cudaMemcpyDefault, c->stream));
+            }
             CK(cudaStreamSynchronize(c->stream));
             return LBM_OK;
         }
@@ -313,7 +322,8 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         sreal *tmp = nullptr;
         CK(cudaMalloc(&tmp, bytes));   // debug path: own temporary, not the borrowed workspace
         k_stream_only<L, real, TP::BX, TP::BY, TP::BZ><<<grid_for<TP>(c->P), NTP, 0, c->stream>>>(
-            dev_params<real>(c), (const sreal *)wsp<sreal>(c, off[1 - c->cur]), tmp, which);
+            dev_params<real>(c), (const sreal *)wsp<sreal>(c, off[1 - c->cur]), tmp, which,
+            is_g ? (const sreal *)wsp<sreal>(c, c->L.off_pdot[1 - c->cur]) : (const sreal *)nullptr);
         c->launches++;
         cudaError_t e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaMemcpyAsync(h, tmp, bytes, cudaMemcpyDefault, c->stream);

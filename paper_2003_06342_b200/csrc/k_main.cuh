@@ -109,6 +109,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     const real om_s = rall * (rho * df);
 
     real ux, uy, uz, p, T, dtphi;
+    real pd_old = real(0);   // production rate of the previous level: in the moment corrections and folded into the stored g_0
     if constexpr (MODE == MODE_INIT) {
         ux = real(Fd.u[n]); uy = real(Fd.u[N + n]); uz = (LF::D == 3) ? real(Fd.u[2 * N + n]) : real(0);
         p = real(Fd.p[n]); T = real(Fd.T[n]); dtphi = real(0);
@@ -133,7 +134,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
         }
         // ---- H1 (time derivative), H5: heat moment with the STORED production rate (reading S3; Eq.34)
         dtphi = real(phi_p - src.phi_old()) * P.inv_dt;                              // reading S4
-        const real mdot_old = P.rho_g * src.pdot_old();
+        pd_old = src.pdot_old();
+        const real mdot_old = P.rho_g * pd_old;
         const real D_old = ux * gx + uy * gy + uz * gz + phi * mdot_old * P.drho;   // reading S5
         T = sum_s;
         if (P.latent_heat) T -= P.hdt * P.LCp * (dtphi + D_old);
@@ -256,10 +258,14 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
         const greal PO = om * phi_g;
         const greal bP = b * greal(pdot);
         {
+            // The rest population never moves, so the term dt/2 Pdot of Eq.(32) (phi^{n+1} = sum_i g_i + dt/2 Pdot, same node,
+            // same production rate as stored below) rides in it: stored g_0' = g*_0 + dt/2 Pdot.  K_phi then needs no Pdot, and
+            // the bar value is recovered here with the production rate of the previous level.
             constexpr greal w = greal(LG::w(0));
+            const greal hdtg = greal(0.5) * dtg;
             greal bar = greal(0);
-            if constexpr (MODE != MODE_INIT) bar = greal(src.template gg<0>());
-            st_pop(Fd.g_out + (n), a * bar + w * (PO * U1 + bP));
+            if constexpr (MODE != MODE_INIT) bar = greal(src.template gg<0>()) - hdtg * greal(pd_old);
+            st_pop(Fd.g_out + (n), a * bar + w * (PO * U1 + bP) + hdtg * greal(pdot));
         }
         static_for<LG::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;

@@ -43,7 +43,6 @@ __device__ __forceinline__ real phi_new_at(const DevParams<real> &P, const real 
     real v = gi[0];
 #pragma unroll
     for (int i = 1; i < LG::Q; ++i) v += gi[i];
-    v += P.hdt * __ldg(pdot_in + g.n);
     if constexpr (BC) {
 #pragma unroll
         for (int a = 0; a < 3; ++a)
@@ -120,7 +119,7 @@ k_main_fused(const DevParams<real> P, const DevFields<real> Fd, real *__restrict
     // pulled g* values and of Pdot of every entry this thread owns into stage[k][e]; reduce() sums them in the same
     // order as phi_new_at (so both forms give the same bits) once the copies have landed.
     constexpr int NEP = (NE + 31) / 32 * 32;
-    __shared__ real stage[(LG::Q + 1) * NEP];
+    __shared__ real stage[LG::Q * NEP];
     auto plane_is_plain = [&](int z) { return !(bc_xy_phi || (P.nonper[2] && (z <= 0 || z >= P.nz - 1))); };
     auto issue = [&](int z) {
         for (int e = t; e < NE; e += NT) {
@@ -135,7 +134,6 @@ k_main_fused(const DevParams<real> P, const DevFields<real> Fd, real *__restrict
                     cp_async_elem(&stage[I * NEP + e],
                                   Fd.g_in + ((unsigned)I * (unsigned)P.N + g.sz[LG::ez(I) + 1] + g.sy[LG::ey(I) + 1] + g.sx[LG::ex(I) + 1]));
                 });
-                cp_async_elem(&stage[LG::Q * NEP + e], Fd.pdot_in + g.n);
             }
         }
         cp_async_commit();
@@ -149,7 +147,6 @@ k_main_fused(const DevParams<real> P, const DevFields<real> Fd, real *__restrict
                 v = stage[e];
 #pragma unroll
                 for (int i = 1; i < LG::Q; ++i) v += stage[i * NEP + e];
-                v += P.hdt * stage[LG::Q * NEP + e];
             }
             dst[e] = v;
         }

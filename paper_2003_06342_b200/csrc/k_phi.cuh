@@ -55,7 +55,8 @@ __device__ __forceinline__ void store_phi_with_images(preal *__restrict__ phi_pa
 
 // Each thread handles NPT nodes, NPT tiles apart along the slowest tiled axis (z in 3D, y in 2D); all 8 NPT loads are
 // issued before the first sum, which is what a latency-bound streaming kernel needs (measured: DESIGN.md "Kernels").
-// phi^{n+1} = sum_i g_i + dt/2 Pdot in the type of the phi array (preal), so that with float populations and a double phi
+// phi^{n+1} = sum_i g_i + dt/2 Pdot (Eq.32); the last term is already inside the stored rest population (k_main.cuh), so
+// this is a plain sum of the pulled values, in the type of the phi array (preal), so that with float populations and a double phi
 // the result carries only the storage rounding of the populations.  Plain sum when the values already are preal;
 // when an all-float kernel feeds a double phi the sum is an error-free float accumulation (Knuth two-sum: hi + lo is the
 // exact sum) widened once at the end -- two conversions per node instead of Q_g + 1 (F2F.F64.F32 issues at a fraction
@@ -66,21 +67,18 @@ __device__ __forceinline__ void two_sum(float &hi, float &lo, float v) {
     lo = __fadd_rn(lo, __fadd_rn(__fsub_rn(hi, __fsub_rn(s, bb)), __fsub_rn(v, bb)));
     hi = s;
 }
-template <class preal, class real, class vreal, int Q>
-__device__ __forceinline__ preal phi_sum(const vreal (&gi)[Q], real hdt, vreal pd) {
+template <class preal, class vreal, int Q>
+__device__ __forceinline__ preal phi_sum(const vreal (&gi)[Q]) {
     if constexpr (std::is_same<vreal, float>::value && std::is_same<preal, double>::value) {
         float hi = gi[0], lo = 0.0f;
 #pragma unroll
         for (int i = 1; i < Q; ++i) two_sum(hi, lo, gi[i]);
-        const float pr = __fmul_rn((float)hdt, pd);
-        lo = __fadd_rn(lo, __fmaf_rn((float)hdt, pd, -pr));   // rounding error of the product, exact
-        two_sum(hi, lo, pr);
         return (double)hi + (double)lo;
     } else {
         preal sum = preal(gi[0]);
 #pragma unroll
         for (int i = 1; i < Q; ++i) sum += preal(gi[i]);
-        return sum + preal(hdt) * preal(pd);   // sum_i w_i = 1
+        return sum;
     }
 }
 
@@ -90,7 +88,7 @@ __device__ __forceinline__ preal phi_sum(const vreal (&gi)[Q], real hdt, vreal p
 // before the error-free sum), else in preal.
 template <class LG, class real, int BX, int BY, int BZ, int NPT, class sreal, class preal>
 __global__ void __launch_bounds__(BX *BY *BZ)
-k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, const sreal *__restrict__ pdot, preal *__restrict__ phi_new) {
+k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, preal *__restrict__ phi_new) {
     using vreal = typename std::conditional<std::is_same<real, sreal>::value, real, preal>::type;
     constexpr bool ALONG_Z = LG::D == 3;
     const int t = threadIdx.x;
@@ -101,7 +99,6 @@ k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, const sreal *__re
     if (x >= P.nx) return;
     const bool bc = tile_touches_bc(P, x0, y0, z0, BX, BY * (ALONG_Z ? 1 : NPT), BZ * (ALONG_Z ? NPT : 1));
     vreal gi[NPT][LG::Q];
-    vreal pd[NPT];
     NodeGeom g[NPT];
     bool ok[NPT];
 #pragma unroll
@@ -112,12 +109,11 @@ k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, const sreal *__re
             g[j] = make_geom(P, x, y, z);
             if (bc) pull<LG, vreal, true>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
             else pull<LG, vreal, false>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
-            pd[j] = vreal(__ldg(pdot + g[j].n));
         }
     }
 #pragma unroll
     for (int j = 0; j < NPT; ++j) {
-        if (ok[j]) store_phi_with_images(phi_new, P, g[j], phi_sum<preal>(gi[j], P.hdt, pd[j]));
+        if (ok[j]) store_phi_with_images(phi_new, P, g[j], phi_sum<preal>(gi[j]));
     }
 }
 
@@ -135,9 +131,12 @@ k_phi_fill(const DevParams<real> P, const sreal *__restrict__ phi_plain, preal *
 }
 
 // Debug / parity: streamed (post-pull, post-BC) populations of one lattice, all directions, to a [Q][N] scratch.
+// `pdot_fold` (g only, else null): the production field folded into the stored rest population of `src` (k_main.cuh), taken out
+// again so that the caller sees the populations of the paper.
 template <class L, class real, int BX, int BY, int BZ, class sreal>
 __global__ void __launch_bounds__(BX *BY *BZ)
-k_stream_only(const DevParams<real> P, const sreal *__restrict__ src, sreal *__restrict__ dst, int which) {
+k_stream_only(const DevParams<real> P, const sreal *__restrict__ src, sreal *__restrict__ dst, int which,
+              const sreal *__restrict__ pdot_fold) {
     const int t = threadIdx.x;
     const int x = blockIdx.x * BX + t % BX, y = blockIdx.y * BY + (t / BX) % BY, z = blockIdx.z * BZ + t / (BX * BY);
     if (x >= P.nx || y >= P.ny || z >= P.nz) return;
@@ -146,8 +145,16 @@ k_stream_only(const DevParams<real> P, const sreal *__restrict__ src, sreal *__r
     if (which == 0) pull<L, real, true>(src, (unsigned)P.N, g, P.bc_f, P.bc_p, v);
     else if (which == 1) pull<L, real, true>(src, (unsigned)P.N, g, P.bc_g, P.bc_phi, v);
     else pull<L, real, true>(src, (unsigned)P.N, g, P.bc_s, P.bc_T, v);
+    if (pdot_fold) v[0] -= P.hdt * real(pdot_fold[g.n]);
 #pragma unroll
     for (int i = 0; i < L::Q; ++i) dst[(size_t)i * P.N + g.n] = sreal(v[i]);
+}
+
+// Debug / parity: the stored rest population of g without the folded dt/2 Pdot (k_main.cuh).
+template <class real, class sreal> __global__ void k_unfold_g0(sreal *__restrict__ dst, const sreal *__restrict__ g0,
+                                                              const sreal *__restrict__ pdot, long long n, real hdt) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = sreal(real(g0[i]) - hdt * real(pdot[i]));
 }
 
 template <class real> __global__ void k_fill(real *__restrict__ dst, long long n, real v) {

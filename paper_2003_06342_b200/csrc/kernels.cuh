@@ -6,7 +6,8 @@
 //                zero-flux mirror, Dirichlet 2v - mirror), two buffers (level n and n+1);
 //   Pdot, u, p, T  [z][y][x].
 // Kernels:
-//   k_phi   H1: pull g (+BC), phi^{n+1} = sum g + dt/2 Pdot (Eq.32), ghost images.
+//   k_phi   H1: pull g (+BC), phi^{n+1} = sum g + dt/2 Pdot (Eq.32; the Pdot term rides in the stored rest
+//           population, k_main.cuh), ghost images.
 //   k_main  H2..H7: stencils (Eq.35,36), closures, pull f,s,g (+BC), moments (Eq.28a,b, 34), production
 //           refresh (Eq.18), BGK collision of the three lattices (Eq.25), store post-collision populations.
 #pragma once
@@ -85,7 +86,7 @@ template <class sreal_, class preal_> struct DevFieldsT {
     const preal *phi_new;              // padded, level n+1 (written by k_phi)
     const preal *phi_old;              // padded, level n
     const sreal *pdot_in;              // production field of level n (the stored one, reading S3)
-    sreal *pdot;                       // production field of level n+1 (same array as pdot_in except in the fused variant)
+    sreal *pdot;                       // production field of level n+1 (the array that belongs to the output buffers)
     sreal *u, *p, *T;                  // macro arrays: outputs (MODE_STEP_MACRO) or inputs (MODE_INIT)
 };
 template <class real> using DevFields = DevFieldsT<real, real>;   // one type throughout (fp64; the tma and fused variants)

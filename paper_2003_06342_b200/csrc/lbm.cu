@@ -103,7 +103,7 @@ Layout make_layout(const lbm_params *p) {
     for (int b = 0; b < 2; ++b) L.off_g[b] = take(N * lattice_q(p->lat_g), es);
     for (int b = 0; b < 2; ++b) L.off_s[b] = take(N * lattice_q(p->lat_s), es);
     for (int b = 0; b < 2; ++b) L.off_phi[b] = take(L.phi_pad_elems, esp);
-    for (int b = 0; b < 2; ++b) L.off_pdot[b] = take(N, es);   // second buffer: fused variant only
+    for (int b = 0; b < 2; ++b) L.off_pdot[b] = take(N, es);   // one per population buffer
     L.off_u = take(3 * N, es);
     L.off_p = take(N, es);
     L.off_T = take(N, es);
@@ -248,7 +248,7 @@ bool build_tma_maps(lbm_ctx *c) {
         ok = ok && encode_rows(&c->map_phi[b], c->ws + c->L.off_phi[b], es, 3, dp, boxx);
     }
     const unsigned long long dd[3] = {nx, ny, nz};
-    ok = ok && encode_rows(&c->map_pdot, c->ws + c->L.off_pdot[0], es, 3, dd, boxx);
+    for (int b = 0; b < 2; ++b) ok = ok && encode_rows(&c->map_pdot[b], c->ws + c->L.off_pdot[b], es, 3, dd, boxx);
     return ok;
 }
 

@@ -178,12 +178,12 @@ def config5_droplets(n=128, nspheres=64, rmin=8.0, rmax=24.0, seed=5, **over):
 def bytes_per_lu(P, itemsize=8, macros=False):
     """Algorithmic HBM bytes per lattice update of the two-kernel step.
 
-    K_phi: Q_g + 1 reads, 1 write.  K_main: Q_f + Q_g + Q_s + 3 reads (phi^{n+1}, phi^n, Pdot),
+    K_phi: Q_g reads, 1 write (the dt/2 Pdot term of Eq.32 rides in the stored rest population of g).  K_main: Q_f + Q_g + Q_s + 3 reads (phi^{n+1}, phi^n, Pdot),
     Q_f + Q_g + Q_s + 1 writes (+5 or +4 when u, p, T are written).  The three phi values (one written, two read) are
     doubles in both precisions (include/lbm.h "Precisions")."""
     q = {"D2Q5": 5, "D2Q9": 9, "D3Q7": 7, "D3Q19": 19, "D3Q15": 15}
     Q = q[P["lat_f"]] + q[P["lat_g"]] + q[P["lat_s"]]
-    vals = (q[P["lat_g"]] + 1 + 1) + (Q + 3) + (Q + 1)
+    vals = (q[P["lat_g"]] + 1) + (Q + 3) + (Q + 1)
     if macros:
         vals += (3 if P["nz"] > 1 else 2) + 2
     return vals * itemsize + 3 * (8 - itemsize)
