@@ -1,12 +1,12 @@
 // K_fused (3D): the whole step H1..H7 in ONE kernel -- no K_phi, no phi^{n+1} hand-off through HBM.
 //
 // A CTA owns a column of BX x BY nodes and marches LZ planes in z.  For every plane it needs it first computes
-// phi^{n+1} = sum_i g*_i(x - e_i) [+BC] + dt/2 Pdot^n  (Eq.32) on the plane INCLUDING a one-cell halo in
+// phi^{n+1} = sum_i g*_i(x - e_i) [+BC]  (Eq.32; its dt/2 Pdot^n rides in the stored g*_0, k_main.cuh) on the plane INCLUDING a one-cell halo in
 // x and y, straight from the post-collision g* of the previous level, into a ring of four shared-memory planes
 // (z-1, z, z+1 in use, z+2 being filled).  The halo values are recomputed by the neighbouring CTAs as well: identical
 // arithmetic, identical bits, served by L2 -- the price for dropping K_phi's 9 values per node of HBM traffic
-// (step: 79 -> 70 values per lattice update).  Pdot is double-buffered because neighbours still read level n while
-// owners write level n+1.  Ghost values outside non-periodic faces are the mirror / Dirichlet images of DESIGN.md S8.
+// (step: 78 -> 70 values per lattice update).  Ghost values outside non-periodic faces are the mirror / Dirichlet images of
+// DESIGN.md S8.
 #pragma once
 
 #include <cstdint>
@@ -116,7 +116,7 @@ k_main_fused(const DevParams<real> P, const DevFields<real> Fd, real *__restrict
     };
 
     // Asynchronous form of fill_plane for planes that need no boundary rule: issue() starts the copies of the LG::Q
-    // pulled g* values and of Pdot of every entry this thread owns into stage[k][e]; reduce() sums them in the same
+    // pulled g* values of every entry this thread owns into stage[k][e]; reduce() sums them in the same
     // order as phi_new_at (so both forms give the same bits) once the copies have landed.
     constexpr int NEP = (NE + 31) / 32 * 32;
     __shared__ real stage[LG::Q * NEP];
