@@ -168,6 +168,21 @@ def test_time_dependent_prescribed_velocity(gpu, oracle_mod):
     g.destroy()
 
 
+def test_physical_units_dx_dt_not_one(gpu, oracle_mod):
+    """dx = 0.5, dt = 0.2: the host-computed constants (c, c_s^2, reciprocals, relaxation rates) against the oracle's."""
+    P = wl.base_params(70, 24, 1, dx=0.5, dt=0.2, grav=[1e-3, -2e-3, 0.0], force=[2e-4, 1e-4, 0.0], W=2.0)
+    P["bc_f"][1] = ["wall", "wall"]; P["bc_g"][1] = ["zeroflux", "zeroflux"]; P["bc_s"][1] = ["dirichlet", "dirichlet"]
+    P["bc_T"][1] = [0.7, 0.0]
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 93), [1, 12], label="2d dx dt")
+    P = wl.base_params(136, 9, 7, dx=0.5, dt=0.2, grav=[1e-3, 0.0, -2e-3], W=2.0)
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 94), [1, 12], label="3d dx dt")
+    P = wl.base_params(256, 6, 5, dx=1.25e-3, dt=7.5e-5, lat_s="D3Q7", W=5e-3, sigma=5e-3, M=1.7e-3, nu_l=3e-3, nu_g=5e-4,
+                       alpha_l=2.5e-4, alpha_g=2.5e-3, rho_l=1.658, grav=[0.0, 0.0, -4.0], L_latent=1.0, Cp=1.0, eps_n=1e-2)
+    st = _random_state(P, 95)
+    st = (st[0], 0.025 * st[1], 10.0 * st[2], 100.0 * st[3])      # T of the order of the paper's theta_w, u in units of c = 16.7
+    _run_parity(gpu, oracle_mod, P, st, [1, 12], label="3d paper units (Table 2, PAPER.md:506)")
+
+
 def test_minimal_grids(gpu, oracle_mod):
     for dims in ((2, 2, 1), (3, 2, 2), (2, 5, 3)):
         P = wl.base_params(*dims)
@@ -587,3 +602,31 @@ def test_fp32_variant_2d(gpu, oracle_mod):
     assert _maxabs(g[0], r[0]) / np.abs(r[0]).max() <= REL32
     assert _maxabs(g[3], r[3]) <= REL32      # T = T_sat = 0 here: absolute
     sim.destroy(); o.close()
+
+
+# ---------------------------------------------------------------------------- the paper's film-boiling run (physical units)
+def test_paper_film_boiling_bubble_detaches(gpu):
+    """Section 5 of the paper with its Table 2 parameters in its own units on a one-wavelength window
+    (512 x 512 nodes, lambda = 0.64 > lambda_c = 0.2738): the crest of the film grows, a bubble detaches from it ("node",
+    PAPER.md:535) and rises; T stays within a few percent of [theta_sat, theta_w], phi within [0, 1].  Measured on the full
+    1024^2 domain: first detached bubbles at t* = t/t_s of about 29 (profiles/r1_full_horizon.md)."""
+    from paper_2003_06342_b200 import run_configs as rc
+    P, I = wl.paper_film_boiling(nx=512, ny=512)
+    sim = gpu.LBM(P, 64)
+    sim.init(I["phi"], I["T"])
+    vol0 = float(I["phi"].sum())
+    seen, top = 0, []
+    for k in range(12):
+        sim.step(5000)
+        phi, u, p, T = sim.read_macro()
+        assert np.isfinite(phi).all() and np.isfinite(T).all() and np.isfinite(u).all(), sim.step_count
+        assert phi.min() > -0.01 and phi.max() < 1.01, (sim.step_count, phi.min(), phi.max())
+        assert T.min() > -0.05 and T.max() < 0.03, (sim.step_count, T.min(), T.max())      # theta_w = 0.025
+        n, t, _ = rc.detached_bubbles(phi[0])
+        seen = max(seen, n)
+        if n:
+            top.append(t)
+    sim.destroy()
+    assert seen >= 1, "no bubble detached in 60 000 steps"
+    assert len(top) >= 2 and top[-1] > top[0], top                                       # it rises
+    assert float(phi.sum()) > vol0                                                        # net evaporation at the heated wall

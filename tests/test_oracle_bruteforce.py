@@ -54,6 +54,16 @@ def test_2d_periodic(oracle_mod):
     _compare(oracle_mod, P, 12, 11)
 
 
+def test_physical_units_dx_dt_not_one(oracle_mod):
+    """dx = 0.5, dt = 0.2 (c = 2.5): every place where c, c_s^2 = e^2 c^2, 1/dx, 1/dx^2 or dt enters (PAPER.md:190, 208, 236, 272,
+    Eq.35-36) must agree between the two transcriptions; the paper's own runs are in physical units."""
+    P = wl.base_params(8, 8, 1, dx=0.5, dt=0.2, grav=[1e-3, -2e-3, 0.0], force=[2e-4, 1e-4, 0.0], W=2.0)
+    P["bc_f"][1] = ["wall", "wall"]; P["bc_g"][1] = ["zeroflux", "dirichlet"]; P["bc_s"][1] = ["dirichlet", "zeroflux"]
+    P["bc_phi"][1] = [0.0, 1.0]; P["bc_T"][1] = [0.7, 0.0]
+    _compare(oracle_mod, P, 12, 91)
+    _compare(oracle_mod, wl.base_params(8, 8, 8, dx=0.5, dt=0.2, grav=[1e-3, 0.0, -2e-3], W=2.0), 12, 92)
+
+
 def test_2d_periodic_d2q9_heat(oracle_mod):
     P = wl.base_params(8, 8, 1, lat_s="D2Q9", theta_I=0.05)
     _compare(oracle_mod, P, 12, 12)
