@@ -1,6 +1,6 @@
 """Run the BASELINE.json configurations at their FULL step counts on the GPU and report physical observables.
 
-    python -m paper_2003_06342_b200.run_configs [--configs 1,2,3,4,paper] [--precision 64] [--samples 10]
+    python -m paper_2003_06342_b200.run_configs [--configs 1,2,3,4,paper,paper_large,paper_large_ja01] [--precision 64] [--samples 10]
 
 One JSON line per configuration: the observables the paper discusses for that test (PAPER.md:446 Laplace law, PAPER.md:473
 Stefan interface position, PAPER.md:535 bubbles growing and rising from the heated wall) sampled along the run, plus
@@ -139,10 +139,10 @@ def run_config4(prec, samples):
     return _run_film(4, P, I, 5000, prec, samples, 0)
 
 
-def run_paper_film(prec, samples, steps=200000):
+def run_paper_film(prec, samples, steps=200000, label="paper", **kw):
     """The paper's film-boiling run (Table 2, 1024^2); the paper ran 5.33e5 steps, a bubble cycle shows much earlier."""
-    P, I = wl.paper_film_boiling()
-    r = _run_film("paper", P, I, steps, prec, samples, 0)
+    P, I = wl.paper_film_boiling(**kw)
+    r = _run_film(label, P, I, steps, prec, samples, 0)
     for s in r["samples"]:
         s["t_star"] = s["step"] * P["dt"] / I["t_s"]          # dimensionless time of PAPER.md:535
         for k in ("h_mean", "h_max", "h_min", "bubble_top"):
@@ -157,7 +157,18 @@ def run_paper_film(prec, samples, steps=200000):
     return r
 
 
-RUNNERS = {1: run_config1, 2: run_config2, 3: run_config3, 4: run_config4, "paper": run_paper_film}
+def run_paper_large(prec, samples, theta_w=0.025):
+    """The paper's 8-GPU run: 4096 x 3072, sixteen modes (Eq.44), 5.33e5 steps, on one GPU."""
+    r = run_paper_film(prec, samples, steps=533000, label="paper_large_Ja%g" % theta_w, nx=4096, ny=3072, modes=16, y1=0.004,
+                       theta_w=theta_w)
+    r["mlups_including_reads"] = 4096.0 * 3072.0 * 533000 / r["wall_seconds_including_reads"] / 1e6
+    r["note"] = ("PAPER.md:563: 80 minutes on 8 GPUs (713 MLUPS as printed) for these 5.33e5 steps; Ja = 0.025 releases discrete bubbles, "
+                 "Ja = 0.1 grows long vapour jets under the bubbles (h_max: the film still attached to the wall reaches far up)")
+    return r
+
+
+RUNNERS = {1: run_config1, 2: run_config2, 3: run_config3, 4: run_config4, "paper": run_paper_film,
+           "paper_large": run_paper_large, "paper_large_ja01": lambda prec, samples: run_paper_large(prec, samples, theta_w=0.1)}
 
 
 def main(argv=None):
@@ -168,7 +179,7 @@ def main(argv=None):
     args = ap.parse_args(argv)
     binding.load_library()
     for c in args.configs.split(","):
-        key = c if c == "paper" else int(c)
+        key = c if c.startswith("paper") else int(c)
         print(json.dumps(RUNNERS[key](args.precision, args.samples)), flush=True)
     return 0
 

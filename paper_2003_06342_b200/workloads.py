@@ -126,18 +126,22 @@ def config3_film2d(nx=512, ny=1024, h0=64.0, amp=4.0, seed=3, noise=1e-6, modes=
     return P, dict(phi=phi, T=T, u=None, p=None, seed=seed, name="config3_film2d_%dx%d" % (nx, ny))
 
 
-def paper_film_boiling(nx=1024, ny=1024, lam=0.64, seed=None, **over):
+def paper_film_boiling(nx=1024, ny=1024, lam=0.64, seed=None, modes=0, y1=0.015, theta_w=0.025, **over):
     """The paper's own film-boiling set-up (Section 5), in ITS physical units: Table 2 parameters, domain
     [0, 1.28]^2 on 1024^2 nodes (dx = 1.25e-3, dt = 7.5e-5), three D2Q9 lattices, interface y = y0 + y1 sin(2 pi x / lambda) with
     y0 = 0.03, y1 = 0.015, lambda = 0.64 (Eq.42), bottom wall at theta_w = 0.025, top wall at saturation with
     phi = 1, x periodic.  With L/Cp = 1 and T_sat = 0 the temperature IS theta.  Not stated in the paper and chosen
     here: the initial temperature (conduction profile across the film, as in config 3) and the phase-field condition on the
-    bottom wall (zero flux).  A smaller grid keeps dx, dt and the physical lengths (a window of the same problem)."""
+    bottom wall (zero flux).  A smaller grid keeps dx, dt and the physical lengths (a window of the same problem).
+
+    modes = 16 with nx, ny = 4096, 3072 is the paper's large run (Eq.44): y = y0 + y1 sum_i sin(2 pi x / lambda_i),
+    lambda_i uniform in [0.5, 1.5 sqrt(3)] lambda_c (seeded), at theta_w = 0.025 or 0.1 (Ja = 0.025 / 0.1).  The paper does not restate
+    y1 for that run; with sixteen modes y1 = 0.015 would put the interface below the wall, so pass a smaller y1 (the film is kept
+    thicker than 2 W everywhere)."""
     dx, dt = 1.25e-3, 7.5e-5
     P = base_params(nx, ny, 1, lat_s="D2Q9", dx=dx, dt=dt, rho_l=1.658, rho_g=1.0, nu_l=3e-3, nu_g=5e-4,
                     alpha_l=2.5e-4, alpha_g=2.5e-3, sigma=5e-3, M=1.7e-3, W=5e-3, grav=[0.0, -4.0, 0.0],
                     L_latent=1.0, Cp=1.0, T_sat=0.0, theta_I=0.0, eps_n=1e-5 / dx, **over)
-    theta_w = 0.025
     P["bc_f"][1] = ["wall", "wall"]
     P["bc_g"][1] = ["zeroflux", "dirichlet"]
     P["bc_phi"][1] = [0.0, 1.0]
@@ -145,11 +149,17 @@ def paper_film_boiling(nx=1024, ny=1024, lam=0.64, seed=None, **over):
     P["bc_T"][1] = [theta_w, 0.0]
     x = (np.arange(nx) + 0.5).reshape(1, 1, nx) * dx
     y = (np.arange(ny) + 0.5).reshape(1, ny, 1) * dx
-    h = 0.03 + 0.015 * np.sin(2.0 * np.pi * x / lam)
+    lam_s = math.sqrt(P["sigma"] / ((P["rho_l"] - P["rho_g"]) * 4.0))      # Eq.(43): 4.358e-2
+    lam_c = 2.0 * math.pi * lam_s
+    if modes > 0:
+        rng = np.random.Generator(np.random.PCG64(44 if seed is None else seed))
+        lams = rng.uniform(0.5 * lam_c, 1.5 * math.sqrt(3.0) * lam_c, size=modes)
+        h = np.maximum(0.03 + y1 * sum(np.sin(2.0 * np.pi * x / l) for l in lams), 2.0 * P["W"])
+    else:
+        h = 0.03 + y1 * np.sin(2.0 * np.pi * x / lam)
     phi = 0.5 * (1.0 - np.tanh(2.0 * (y - h) / P["W"]))
     T = theta_w * np.maximum(0.0, 1.0 - y / h)
-    lam_s = math.sqrt(P["sigma"] / ((P["rho_l"] - P["rho_g"]) * 4.0))      # Eq.(43): 4.358e-2
-    return P, dict(phi=phi, T=T, u=None, p=None, seed=seed, t_s=math.sqrt(lam_s / 4.0), lam_c=2.0 * math.pi * lam_s,
+    return P, dict(phi=phi, T=T, u=None, p=None, seed=seed, t_s=math.sqrt(lam_s / 4.0), lam_c=lam_c,
                    name="paper_film_boiling_%dx%d" % (nx, ny))
 
 
