@@ -630,3 +630,12 @@ def test_paper_film_boiling_bubble_detaches(gpu):
     assert seen >= 1, "no bubble detached in 60 000 steps"
     assert len(top) >= 2 and top[-1] > top[0], top                                       # it rises
     assert float(phi.sum()) > vol0                                                        # net evaporation at the heated wall
+
+
+def test_paper_film_boiling_parity_window(gpu, oracle_mod):
+    """The paper's film-boiling recipe in its physical units on a small window against the oracle: all distributions and
+    fields, 1e-10 ABSOLUTE although p and the f populations are of the order of rho c_s^2 = 150 here."""
+    P, I = wl.paper_film_boiling(nx=136, ny=72, lam=0.17)
+    # horizon: the liquid meets the phi = 1 top wall of the paper's set-up (PAPER.md:520) with a jump, and that transient amplifies
+    # a 1-ulp input perturbation to 1e-13 by step 20 and 5e-7 by step 100, oracle against oracle
+    _run_parity(gpu, oracle_mod, P, (I["phi"], I["T"]), [1, 20], label="paper film boiling 136x72")
