@@ -1,6 +1,6 @@
 """Run the BASELINE.json configurations at their FULL step counts on the GPU and report physical observables.
 
-    python -m paper_2003_06342_b200.run_configs [--configs 1,2,3,4,paper,paper_large,paper_large_ja01] [--precision 64] [--samples 10]
+    python -m paper_2003_06342_b200.run_configs [--configs 1,2,3,3_window,4,paper,paper_large,paper_large_ja01] [--set M=0.1] [--precision 64] [--samples 10]
 
 One JSON line per configuration: the observables the paper discusses for that test (PAPER.md:446 Laplace law, PAPER.md:473
 Stefan interface position, PAPER.md:535 bubbles growing and rising from the heated wall) sampled along the run, plus
@@ -134,6 +134,15 @@ def run_config3(prec, samples):
     return _run_film(3, P, I, 50000, prec, samples, 0)
 
 
+def run_config3_window(prec, samples, **over):
+    """Config 3 on a 128 x 256 window (film height 32) for 30 000 steps: small enough for the oracle to follow
+    (tests/test_gpu_parity.py::test_config3_window_diverges_like_the_oracle); `--set key=value` varies one parameter."""
+    P, I = wl.config3_film2d(nx=128, ny=256, h0=32.0, amp=4.0, **over)
+    r = _run_film("3_window", P, I, 30000, prec, samples, 0)
+    r["overrides"] = over
+    return r
+
+
 def run_config4(prec, samples):
     P, I = wl.config4_film3d()
     return _run_film(4, P, I, 5000, prec, samples, 0)
@@ -176,9 +185,14 @@ def main(argv=None):
     ap.add_argument("--configs", default="1,2,3,4")
     ap.add_argument("--precision", type=int, default=64, choices=(32, 64))
     ap.add_argument("--samples", type=int, default=10)
+    ap.add_argument("--set", action="append", default=[], metavar="KEY=VALUE", help="3_window only: override a physical parameter")
     args = ap.parse_args(argv)
     binding.load_library()
     for c in args.configs.split(","):
+        if c == "3_window":
+            over = {kv.split("=")[0]: float(kv.split("=")[1]) for kv in args.set}
+            print(json.dumps(run_config3_window(args.precision, args.samples, **over)), flush=True)
+            continue
         key = c if c.startswith("paper") else int(c)
         print(json.dumps(RUNNERS[key](args.precision, args.samples)), flush=True)
     return 0

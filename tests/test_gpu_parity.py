@@ -639,3 +639,23 @@ def test_paper_film_boiling_parity_window(gpu, oracle_mod):
     # horizon: the liquid meets the phi = 1 top wall of the paper's set-up with a jump, and that transient amplifies
     # a 1-ulp input perturbation to 1e-13 by step 20 and 5e-7 by step 100, oracle against oracle
     _run_parity(gpu, oracle_mod, P, (I["phi"], I["T"]), [1, 20], label="paper film boiling 136x72")
+
+
+def test_config3_window_diverges_like_the_oracle(gpu, oracle_mod):
+    """Config 3 does not survive its 50 000 steps at the BASELINE.json parameters: on a 128 x 256 window
+    the CUDA path and the oracle stay together (to the accuracy the amplified round-off allows) up to step 7000 and are both non-finite
+    by step 9000 -- the divergence belongs to the method at these parameters (mobility 0.02 at density ratio 10), not to
+    one implementation."""
+    P, I = wl.config3_film2d(nx=128, ny=256, h0=32.0, amp=4.0)
+    o = oracle_mod.Oracle(P); o.init(I["phi"], I["T"])
+    sim = gpu.LBM(P, 64); sim.init(I["phi"], I["T"])
+    o.step(7000); sim.step(7000)
+    for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
+        assert np.isfinite(a).all() and np.isfinite(b).all(), name
+        assert _maxabs(a, b) <= 0.05 * float(np.abs(b).max()), (name, _maxabs(a, b))
+    g_phi, o_phi = sim.read_macro()[0], o.read_macro()[0]
+    assert 1.01 < g_phi.max() < 1.1 and 1.01 < o_phi.max() < 1.1          # the overshoot that ends the run
+    o.step(2000); sim.step(2000)
+    assert not np.isfinite(sim.read_macro()[3]).all()
+    assert not np.isfinite(o.read_macro()[3]).all()
+    sim.destroy(); o.close()
