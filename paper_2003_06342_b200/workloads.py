@@ -163,6 +163,31 @@ def paper_film_boiling(nx=1024, ny=1024, lam=0.64, seed=None, modes=0, y1=0.015,
                    name="paper_film_boiling_%dx%d" % (nx, ny))
 
 
+def paper_film_boiling_3d(nx=256, ny=256, nz=384, y1=0.015, theta_w=0.025, **over):
+    """The paper's film-boiling set-up carried to 3D (its 3D coupling terms were "planned"): Table 2 parameters
+    in physical units (dx = 1.25e-3, dt = 7.5e-5), D3Q19 + D3Q7 + D3Q7, heated plate at z = 0, top wall at saturation with phi = 1,
+    x and y periodic, film z = y0 + y1/2 [cos(2 pi x / Lx) + cos(2 pi y / Ly)] with y0 = 0.03: one crest per box.  The box must be
+    wider than lambda_c = 0.2738 for the crest to grow (Eq.43): 256 nodes = 0.32."""
+    dx, dt = 1.25e-3, 7.5e-5
+    P = base_params(nx, ny, nz, dx=dx, dt=dt, rho_l=1.658, rho_g=1.0, nu_l=3e-3, nu_g=5e-4, alpha_l=2.5e-4, alpha_g=2.5e-3,
+                    sigma=5e-3, M=1.7e-3, W=5e-3, grav=[0.0, 0.0, -4.0], L_latent=1.0, Cp=1.0, T_sat=0.0, theta_I=0.0,
+                    eps_n=1e-5 / dx, **over)
+    P["bc_f"][2] = ["wall", "wall"]
+    P["bc_g"][2] = ["zeroflux", "dirichlet"]
+    P["bc_phi"][2] = [0.0, 1.0]
+    P["bc_s"][2] = ["dirichlet", "dirichlet"]
+    P["bc_T"][2] = [theta_w, 0.0]
+    x = (np.arange(nx) + 0.5).reshape(1, 1, nx) * dx
+    y = (np.arange(ny) + 0.5).reshape(1, ny, 1) * dx
+    z = (np.arange(nz) + 0.5).reshape(nz, 1, 1) * dx
+    h = 0.03 + 0.5 * y1 * (np.cos(2.0 * np.pi * x / (nx * dx)) + np.cos(2.0 * np.pi * y / (ny * dx)))
+    phi = 0.5 * (1.0 - np.tanh(2.0 * (z - h) / P["W"]))
+    T = theta_w * np.maximum(0.0, 1.0 - z / h)
+    lam_s = math.sqrt(P["sigma"] / ((P["rho_l"] - P["rho_g"]) * 4.0))
+    return P, dict(phi=phi, T=T, u=None, p=None, seed=None, t_s=math.sqrt(lam_s / 4.0), lam_c=2.0 * math.pi * lam_s,
+                   name="paper_film_boiling_3d_%dx%dx%d" % (nx, ny, nz))
+
+
 def config4_film3d(nx=256, ny=256, nz=512, h0=32.0, amp=3.0, seed=4, zrange=None, **over):
     """Config 4: 3D film boiling, x,y periodic, walls in z, heated bottom plate (configs[3]).
 

@@ -50,3 +50,11 @@ def test_paper_film_boiling_recipe():
     _, I3 = wl.paper_film_boiling(nx=1024, ny=64, modes=16, y1=0.004, theta_w=0.1)
     assert np.array_equal(I2["phi"], I3["phi"]) and I2["T"].max() <= 0.1
     assert ((I2["phi"][0] > 0.5).sum(axis=0) * P2["dx"]).min() >= 2 * P2["W"] - P2["dx"]
+
+
+def test_paper_film_boiling_3d_recipe():
+    P, I = wl.paper_film_boiling_3d(nx=32, ny=32, nz=48)
+    assert (P["lat_f"], P["lat_g"], P["lat_s"]) == ("D3Q19", "D3Q7", "D3Q7") and P["grav"] == [0.0, 0.0, -4.0]
+    assert I["phi"].shape == (48, 32, 32) and P["bc_phi"][2] == [0.0, 1.0] and P["bc_T"][2] == [0.025, 0.0]
+    h = (I["phi"] > 0.5).sum(axis=0) * P["dx"]
+    assert abs(h.max() - 0.045) < 2e-3 and abs(h.min() - 0.015) < 2e-3 and abs(h.mean() - 0.03) < 1e-3   # y0 +- y1, one crest per box
