@@ -1,6 +1,6 @@
 """Run the BASELINE.json configurations at their FULL step counts on the GPU and report physical observables.
 
-    python -m paper_2003_06342_b200.run_configs [--configs 1,2,3,3_window,4,paper,paper_3d,paper_large,paper_large_ja01] [--set M=0.1] [--precision 64] [--samples 10]
+    python -m paper_2003_06342_b200.run_configs [--configs 1,2,3,3_window,4,paper,paper_full,paper_3d,paper_large,paper_large_ja01] [--set M=0.1] [--precision 64] [--samples 10]
 
 One JSON line per configuration: the observables the paper discusses for that test (PAPER.md:446 Laplace law, PAPER.md:473
 Stefan interface position, PAPER.md:535 bubbles growing and rising from the heated wall) sampled along the run, plus
@@ -192,7 +192,7 @@ def run_paper_3d(prec, samples, steps=60000):
 
 
 RUNNERS = {1: run_config1, 2: run_config2, 3: run_config3, 4: run_config4, "paper": run_paper_film,
-           "paper_3d": run_paper_3d, "paper_large": run_paper_large, "paper_large_ja01": lambda prec, samples: run_paper_large(prec, samples, theta_w=0.1)}
+           "paper_full": lambda prec, samples: run_paper_film(prec, samples, steps=533000, label="paper_full"), "paper_3d": run_paper_3d, "paper_large": run_paper_large, "paper_large_ja01": lambda prec, samples: run_paper_large(prec, samples, theta_w=0.1)}
 
 
 def main(argv=None):
