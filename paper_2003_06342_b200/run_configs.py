@@ -1,6 +1,6 @@
 """Run the BASELINE.json configurations at their FULL step counts on the GPU and report physical observables.
 
-    python -m paper_2003_06342_b200.run_configs [--configs 1,2,3,3_window,4,paper,paper_full,paper_3d,paper_large,paper_large_ja01] [--set M=0.1] [--precision 64] [--samples 10]
+    python -m paper_2003_06342_b200.run_configs [--configs 1,2,3,3_window,4,stefan_paper,paper,paper_full,paper_3d,paper_large,paper_large_ja01] [--set M=0.1] [--precision 64] [--samples 10]
 
 One JSON line per configuration: the observables the paper discusses for that test (PAPER.md:446 Laplace law, PAPER.md:473
 Stefan interface position, PAPER.md:535 bubbles growing and rising from the heated wall) sampled along the run, plus
@@ -95,6 +95,43 @@ def run_config2(prec, samples):
     return dict(config=2, name=I["name"], steps=steps, samples=out,
                 note="one-phase Stefan solution x_I = 2 xi sqrt(alpha_g (t + t0)), xi = 0.220016 (SURVEY.md S12); with the Navier-Stokes "
                      "lattice on and the OPEN face the interface runs 0.3 cell ahead at 20 000 steps (DESIGN.md)")
+
+
+def run_stefan_paper(prec, samples):
+    """The paper's Stefan validation (Fig.7): 512 x 32, D2Q9 for phi and T, flow at rest (equal densities, no
+    surface tension), W = 3, M = 0.08, theta_w = -0.3, theta_inf = 0.3, t_f = 2e5 steps; interface position against
+    x_I = 2 xi sqrt(alpha_l t) (Eq.41a) with the xi the paper prints for its six cases."""
+    cases = [(0.14, 0.14, 0.0, 0.280680), (0.08, 0.08, 0.0, 0.280680), (0.03, 0.03, 0.0, 0.280680),
+             (0.14, 0.014, 0.05, 0.349635), (0.125, 0.025, 0.05, 0.343882), (0.08, 0.04, 0.05, 0.331864)]
+    nx, ny, steps = 512, 32, 200000
+    out = []
+    for alpha_l, alpha_g, theta_I, xi in cases:
+        P = wl.base_params(nx, ny, 1, lat_s="D2Q9", rho_l=1.0, rho_g=1.0, sigma=0.0, W=3.0, M=0.08, Cp=1.0, L_latent=1.0,
+                           alpha_l=alpha_l, alpha_g=alpha_g, theta_I=theta_I)
+        P["bc_f"][0] = ["wall", "wall"]
+        P["bc_g"][0] = ["dirichlet", "dirichlet"]
+        P["bc_s"][0] = ["dirichlet", "dirichlet"]
+        P["bc_phi"][0] = [0.0, 1.0]
+        P["bc_T"][0] = [-0.3, 0.3]
+        x = (np.arange(nx) + 0.5)[None, None, :]
+        phi0 = 0.5 * (1.0 + np.tanh(2.0 * x / 3.0)) + np.zeros((1, ny, 1))
+        sim = binding.LBM(P, prec)
+        sim.init(phi0.astype(sim.dtype), np.full((1, ny, nx), 0.3, dtype=sim.dtype))
+        rows = []
+        every = steps // samples
+        for k in range(samples):
+            sim.step(every)
+            phi = sim.read_macro()[0]
+            row = phi[0, 0, :]
+            j = int(np.nonzero((row[:-1] < 0.5) & (row[1:] >= 0.5))[0][0])          # liquid (phi = 0) grows from the cold wall
+            x_i = (j + 0.5) + (0.5 - float(row[j])) / (float(row[j + 1]) - float(row[j]))
+            t = sim.step_count
+            rows.append(dict(step=t, x_interface=x_i, x_analytic=2.0 * xi * math.sqrt(alpha_l * t),
+                             ratio=x_i / (2.0 * xi * math.sqrt(alpha_l * t))))
+        sim.destroy()
+        out.append(dict(alpha_l=alpha_l, alpha_g=alpha_g, theta_I=theta_I, xi=xi, samples=rows))
+    return dict(config="stefan_paper", name="paper_stefan_512x32", steps=steps, cases=out,
+                note="PAPER.md:498-500: xi = 0.280680 for theta_I = 0; 0.349635 / 0.343882 / 0.331864 for alpha_l/alpha_g = 10 / 5 / 2, theta_I = 0.05")
 
 
 def _run_film(config, P, I, steps, prec, samples, normal_axis):
@@ -192,7 +229,7 @@ def run_paper_3d(prec, samples, steps=60000):
 
 
 RUNNERS = {1: run_config1, 2: run_config2, 3: run_config3, 4: run_config4, "paper": run_paper_film,
-           "paper_full": lambda prec, samples: run_paper_film(prec, samples, steps=533000, label="paper_full"), "paper_3d": run_paper_3d, "paper_large": run_paper_large, "paper_large_ja01": lambda prec, samples: run_paper_large(prec, samples, theta_w=0.1)}
+           "stefan_paper": run_stefan_paper, "paper_full": lambda prec, samples: run_paper_film(prec, samples, steps=533000, label="paper_full"), "paper_3d": run_paper_3d, "paper_large": run_paper_large, "paper_large_ja01": lambda prec, samples: run_paper_large(prec, samples, theta_w=0.1)}
 
 
 def main(argv=None):
@@ -208,7 +245,7 @@ def main(argv=None):
             over = {kv.split("=")[0]: float(kv.split("=")[1]) for kv in args.set}
             print(json.dumps(run_config3_window(args.precision, args.samples, **over)), flush=True)
             continue
-        key = c if c.startswith("paper") else int(c)
+        key = c if (c.startswith("paper") or c.startswith("stefan")) else int(c)
         print(json.dumps(RUNNERS[key](args.precision, args.samples)), flush=True)
     return 0
 
