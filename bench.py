@@ -48,6 +48,10 @@ def make_workload(name: str, seed_offset: int = 0):
         return wl.config3_film2d(nx=nx, ny=ny, seed=3 + seed_offset, **over)
     if name.startswith("config5_"):
         return wl.config5_droplets(n=int(name.split("_")[1]), seed=5 + seed_offset)
+    if name == "paper_film_1024":     # the paper's own film-boiling run, Table 2 in physical units
+        return wl.paper_film_boiling()
+    if name == "paper_film_4096x3072":   # its 8-GPU run
+        return wl.paper_film_boiling(nx=4096, ny=3072, modes=16, y1=0.004)
     if name == "config1":
         return wl.config1_droplet(seed=1 + seed_offset)
     raise SystemExit("unknown workload %r" % name)
@@ -107,6 +111,14 @@ def measured_peak():
             return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def vs_paper(workload: str, precision: int, value: float):
+    """value / the paper's number, only where BASELINE.md holds one for this exact metric and workload: the 1024^2 film-boiling run
+    of PAPER.md:559 (80.96 MLUPS, fp64, one K80 -- another machine: context, not a target)."""
+    if workload == "paper_film_1024" and precision == 64:
+        return value / 80.96
+    return None
 
 
 def ncu_traffic(workload: str, precision: int):
@@ -271,7 +283,7 @@ def run_ours(args):
     line = {
         "metric": METRIC if prec == 64 else "MLUPS (full coupled step, fp32)", "value": value, "unit": "MLUPS",
         "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_job / K, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": vs_paper(args.workload, prec, value), "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
         "config": {"workload": args.workload, "grid": [nx, ny, nz], "lattices": [P["lat_f"], P["lat_g"], P["lat_s"]],
                    "parallelism": "replicas x%d" % world, "variant": sim.variant,
                    "l2": "state (%.1f GB) is far larger than L2; no flush needed" % (sim.workspace_bytes / 1e9)
