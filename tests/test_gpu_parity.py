@@ -108,6 +108,17 @@ def test_3d_periodic_ragged(gpu, oracle_mod):
     _run_parity(gpu, oracle_mod, P, _random_state(P, 39), [1, 8], label="3d wide tiles")
 
 
+def test_3d_mid_tiles(gpu, oracle_mod):
+    """Rows that are a multiple of 64 but not worth a 128-wide tile (192, 320; here 64 and 192) run 64 x 2 tiles in fp64 3D."""
+    P = wl.base_params(64, 7, 5, grav=[1e-4, -1e-4, -2e-4])
+    sim = gpu.LBM(P, 64); assert sim.variant == "gather+smem"; sim.destroy()
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 61), [1, 12], label="3d 64-wide periodic")
+    P = wl.base_params(192, 5, 6, grav=[0.0, 0.0, -1e-4], lat_f="D3Q15")
+    P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
+    P["bc_T"][2] = [1.0, 0.0]
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 62), [1, 12], label="3d 192-wide z walls, D3Q15")
+
+
 def test_3d_walls_z(gpu, oracle_mod):
     P = wl.base_params(34, 9, 12, grav=[0.0, 0.0, -1e-4])
     P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
