@@ -24,8 +24,8 @@ struct TileWide3Phi { static constexpr int BX = 128, BY = 2, BZ = 1; using PhiTi
 struct TileWide3 { static constexpr int BX = 128, BY = 1, BZ = 1; using PhiTile = TileWide3Phi; };
 struct TileNarrow3 { static constexpr int BX = 32, BY = 4, BZ = 2; using PhiTile = TileNarrow3; };
 struct TileMid3Phi { static constexpr int BX = 64, BY = 4, BZ = 1; using PhiTile = TileMid3Phi; };
-// rows that are a multiple of 64 where the 128-wide tile does not pay (192, 320): 64 x 2 instead of the narrow tile, fp64 3D:
-// config 5 at 192^3 9759 -> 10 019 MLUPS (bench.py), 320^3 9856 -> 10 213 (probe)
+// rows that are a multiple of 64 where the 128-wide tile does not pay (192, 320): 64 x 2 instead of the narrow tile, 3D:
+// config 5 at 192^3 9759 -> 10 019 MLUPS (bench.py), 320^3 9856 -> 10 213 (probe); fp32 3D: 192^3 15 719 -> 16 853, 320^3 16 285 -> 17 386
 struct TileMid3 { static constexpr int BX = 64, BY = 2, BZ = 1; using PhiTile = TileMid3Phi; };
 struct TileWide2 { static constexpr int BX = 128, BY = 2, BZ = 1; using PhiTile = TileWide2; };
 struct TileWide2K { static constexpr int BX = 128, BY = 1, BZ = 1; using PhiTile = TileWide2; };

@@ -117,6 +117,13 @@ def test_3d_mid_tiles(gpu, oracle_mod):
     P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
     P["bc_T"][2] = [1.0, 0.0]
     _run_parity(gpu, oracle_mod, P, _random_state(P, 62), [1, 12], label="3d 192-wide z walls, D3Q15")
+    # the same tiles in fp32
+    init = _random_state(P, 62)
+    o = oracle_mod.Oracle(P); o.init(*init); o.step(12)
+    sim = gpu.LBM(P, 32); sim.init(*[x.astype(np.float32) for x in init]); sim.step(12)
+    for x, y, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
+        assert _maxabs(x, y) / max(float(np.abs(y).max()), 1e-30) <= REL32, name
+    sim.destroy(); o.close()
 
 
 def test_3d_walls_z(gpu, oracle_mod):
