@@ -113,14 +113,6 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def vs_paper(workload: str, precision: int, value: float):
-    """value / the paper's number, only where BASELINE.md holds one for this exact metric and workload: the 1024^2 film-boiling run
-    of PAPER.md:559 (80.96 MLUPS, fp64, one K80 -- another machine: context, not a target)."""
-    if workload == "paper_film_1024" and precision == 64:
-        return value / 80.96
-    return None
-
-
 def ncu_traffic(workload: str, precision: int):
     """DRAM bytes per K_main launch from the committed ncu --set full capture, if there is one for this workload."""
     try:
@@ -207,9 +199,9 @@ def run_ours(args):
     replicas.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    e0.record()
+    e0.record(sim.stream)
     sim.step(K)
-    e1.record()
+    e1.record(sim.stream)
     torch.cuda.synchronize()
     replicas.barrier()
     t1 = time.perf_counter()
@@ -227,22 +219,22 @@ def run_ours(args):
     replicas.barrier()
     torch.cuda.synchronize()
     f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    f0.record()
+    f0.record(sim.stream)
     sim.init(h_phi, h_T)
     sim.step(K)
     sim.read_macro(out=outs)
-    f1.record()
+    f1.record(sim.stream)
     torch.cuda.synchronize()
     ms_e2e, lu_e2e = replicas.reduce_job(f0.elapsed_time(f1), float(N) * K, dev)
     e2e_value = replicas.job_throughput_mlups(ms_e2e, lu_e2e)
     # the same with the host copies around EVERY step (what a per-step host round trip would cost): 3 iterations
     s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    s0.record()
+    s0.record(sim.stream)
     for _ in range(3):
         sim.init(h_phi, h_T)
         sim.step(1)
         sim.read_macro(out=outs)
-    s1.record()
+    s1.record(sim.stream)
     torch.cuda.synchronize()
     ms_strict, lu_strict = replicas.reduce_job(s0.elapsed_time(s1), float(N) * 3, dev)
     e2e_strict = replicas.job_throughput_mlups(ms_strict, lu_strict)
@@ -283,7 +275,7 @@ def run_ours(args):
     line = {
         "metric": METRIC if prec == 64 else "MLUPS (full coupled step, fp32)", "value": value, "unit": "MLUPS",
         "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_job / K, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": vs_paper(args.workload, prec, value), "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
         "config": {"workload": args.workload, "grid": [nx, ny, nz], "lattices": [P["lat_f"], P["lat_g"], P["lat_s"]],
                    "parallelism": "replicas x%d" % world, "variant": sim.variant,
                    "l2": "state (%.1f GB) is far larger than L2; no flush needed" % (sim.workspace_bytes / 1e9)
@@ -342,9 +334,9 @@ def run_slabs(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     replicas.barrier()
     torch.cuda.synchronize()
-    e0.record()
+    e0.record(sim.stream)
     sim.step(K)
-    e1.record()
+    e1.record(sim.stream)
     torch.cuda.synchronize()
     replicas.barrier()
     ms_job, lu_job = replicas.reduce_job(e0.elapsed_time(e1), float(owned) * K, dev)

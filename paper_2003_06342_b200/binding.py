@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("LBM_LIB_PATH") or os.path.join(_HERE, "liblbm_b200.so")   # override: tuning builds only
+LIB_PATH = os.path.join(_HERE, "liblbm_b200.so")
 
 LATTICES = {"D2Q5": 0, "D2Q9": 1, "D3Q7": 2, "D3Q19": 3, "D3Q15": 4}
 LATTICE_Q = {"D2Q5": 5, "D2Q9": 9, "D3Q7": 7, "D3Q19": 19, "D3Q15": 15}
@@ -21,12 +21,16 @@ S_KINDS = {"periodic": 0, "zeroflux": 1, "dirichlet": 2}
 FLAG_PHASE_CHANGE = 1
 FLAG_LATENT_HEAT = 2
 FLAG_PRESCRIBED_U = 4
+# kernel selection (include/lbm.h): speed only, never the method
+FLAG_TWO_LAUNCHES, FLAG_POPS_GATHER, FLAG_POPS_STAGED, FLAG_PHI_LDG, FLAG_NO_GRAPH = 8, 16, 32, 64, 128
+KERNEL_FLAGS = {"two_launches": FLAG_TWO_LAUNCHES, "pops_gather": FLAG_POPS_GATHER, "pops_staged": FLAG_POPS_STAGED,
+                "phi_ldg": FLAG_PHI_LDG, "no_graph": FLAG_NO_GRAPH}
 POPS_F, POPS_G, POPS_S = 0, 1, 2
 STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1
 
 EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops",
-           "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
+           "lbm_sync", "lbm_set_sweep", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
 
@@ -77,6 +81,7 @@ def load_library():
         L.lbm_read_macro.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_sync.argtypes = [C.c_void_p]
+        L.lbm_set_sweep.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.lbm_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.lbm_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.lbm_step_count.restype = C.c_longlong
@@ -113,6 +118,8 @@ def make_params(P: dict, precision: int = 64) -> lbm_params:
         setattr(s, k, float(P[k]))
     s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0) | (
         FLAG_PRESCRIBED_U if P.get("prescribed_u", False) else 0)
+    for name in P.get("kernels", ()):        # e.g. P["kernels"] = ("two_launches",): force a plainer kernel variant
+        s.flags |= KERNEL_FLAGS[name]
     halo = P.get("halo", (0, 0))
     s.halo[0], s.halo[1] = int(halo[0]), int(halo[1])
     return s
@@ -133,12 +140,17 @@ def lbm_workspace_bytes(P: dict, precision: int = 64) -> int:
     return int(load_library().lbm_workspace_bytes(C.byref(s)))
 
 
-def _host_ptr(a, dtype, shape, name):
+def _host_ptr(a, dtype, shape, name, output=False):
     """Pointer to a numpy array or a torch tensor (CPU, pinned or not, or CUDA: the library copies with unified
-    addressing), contiguous, right dtype/shape."""
+    addressing), contiguous, right dtype/shape.  Inputs may be converted (a temporary copy); an ``output`` array is
+    written in place, so a wrong dtype, shape or layout raises instead."""
     if a is None:
         return None, None
     if isinstance(a, np.ndarray):
+        if output:
+            if a.dtype != dtype or not a.flags["C_CONTIGUOUS"] or not a.flags["WRITEABLE"] or tuple(a.shape) != tuple(shape):
+                raise ValueError("%s: output must be a writable C-contiguous %s array of shape %s" % (name, np.dtype(dtype), shape))
+            return a.ctypes.data, a
         b = np.ascontiguousarray(a, dtype=dtype)
         if tuple(b.shape) != tuple(shape):
             raise ValueError("%s: shape %s, expected %s" % (name, b.shape, shape))
@@ -175,7 +187,9 @@ class LBM:
         self.workspace_bytes = nbytes
         # device memory is allocated by torch and lent to the library (torch allocations are 512-byte aligned)
         self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
-        self._stream = stream if stream is not None else torch.cuda.current_stream()
+        # A stream of the context's own unless the caller gives one: every call below is enqueued there, and the CUDA-graph
+        # replay of small grids needs a stream that can be captured (the legacy default stream cannot).
+        self._stream = stream if stream is not None else torch.cuda.Stream()
         h = C.c_void_p()
         _check(self._L.lbm_create(C.byref(self._params), C.c_void_p(self._ws.data_ptr()), nbytes,
                                   C.c_void_p(self._stream.cuda_stream), C.byref(h)), "lbm_create")
@@ -227,7 +241,7 @@ class LBM:
         shapes = (self.shape, (3,) + self.shape, self.shape, self.shape)
         ptrs = []
         for a, shape, name in zip(out, shapes, ("phi", "u", "p", "T")):
-            ptr, _ = _host_ptr(a, self.dtype, shape, name)
+            ptr, _ = _host_ptr(a, self.dtype, shape, name, output=True)
             ptrs.append(C.c_void_p(ptr) if ptr is not None else None)
         _check(self._L.lbm_read_macro(self._h, *ptrs), "lbm_read_macro")
         return out
@@ -239,6 +253,14 @@ class LBM:
 
     def sync(self):
         _check(self._L.lbm_sync(self._h), "lbm_sync")
+
+    def set_sweep(self, rows_per_block: int = 0, lead: int = -1):
+        _check(self._L.lbm_set_sweep(self._h, int(rows_per_block), int(lead)), "lbm_set_sweep")
+
+    @property
+    def stream(self):
+        """The torch.cuda.Stream every kernel and copy of this context is enqueued on (record timing events there)."""
+        return self._stream
 
     def set_timing(self, enable: bool):
         _check(self._L.lbm_set_timing(self._h, 1 if enable else 0), "lbm_set_timing")

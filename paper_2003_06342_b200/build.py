@@ -5,6 +5,7 @@ The ptxas resource report (registers / spills per kernel) is written next to the
 """
 from __future__ import annotations
 
+import glob
 import os
 import subprocess
 import sys
@@ -14,8 +15,14 @@ SRC_DIR = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblbm_b200.so")
 SOURCES = ["lbm.cu", "halo.cu", "inst_2d995_f64.cu", "inst_2d995_f32.cu", "inst_2d999_f64.cu", "inst_2d999_f32.cu",
            "inst_3d_f64.cu", "inst_3d_f32.cu", "inst_3d15_f64.cu", "inst_3d15_f32.cu"]
-DEPS = SOURCES + ["ctx.h", "impl.cuh", "kernels.cuh", "k_phi.cuh", "k_main.cuh", "k_main_tma.cuh", "k_main_phitma.cuh", "k_main_fused.cuh", "lattices.cuh",
-                  os.path.join("..", "..", "include", "lbm.h")]
+
+
+def deps():
+    """Every file the library is built from: all of csrc/ and the public header."""
+    return sorted(glob.glob(os.path.join(SRC_DIR, "*.cu")) + glob.glob(os.path.join(SRC_DIR, "*.cuh")) +
+                  glob.glob(os.path.join(SRC_DIR, "*.h"))) + [os.path.join(HERE, "..", "include", "lbm.h")]
+
+
 NVCC_COMPILE = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xptxas", "-v",
                 "-Xcompiler", "-fPIC", "-c"]
 NVCC_LINK = ["-gencode", "arch=compute_100a,code=sm_100a", "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
@@ -25,7 +32,7 @@ def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(SRC_DIR, d)) > t for d in DEPS)
+    return any(os.path.getmtime(d) > t for d in deps())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -28,7 +28,8 @@ struct Layout {
     int es, es_phi;   // bytes per element: populations / Pdot / macros / caller's arrays; padded phi arrays
     int ppx, ppy, ppz, pz, xpad;
     size_t phi_pad_elems;
-    size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot[2], off_u, off_p, off_T, off_scratch, total;
+    size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot[2], off_u, off_p, off_T, off_scratch, off_sync, total;
+    size_t sync_bytes;   // ticket, error flag and slice counters of the single-launch step
 };
 
 // One implementation = one (lattice set, precision, tile shape); chosen once in lbm_create.
@@ -39,6 +40,7 @@ struct ImplOps {
     int (*read_macro)(lbm_ctx *, void *, void *, void *, void *);
     int (*read_pops)(lbm_ctx *, int, int, void *);
     int bx, by, bz;   // tile of nodes per CTA
+    int step_bm;      // rows of the mid axis per work item of the single-launch step (k_step.cuh); 0: tile shape not supported
 };
 
 // defined in inst_*.cu (compiled in parallel); nx selects the tile shape
@@ -67,16 +69,15 @@ struct lbm_ctx {
     long long nsteps, launches;
     lbm::DevParams<double> pd;
     lbm::DevParams<float> pf;
-    // TMA variant of K_main: tensor maps of both buffers of every input array
-    bool use_tma;
     int num_sms;
-    CUtensorMap map_f[2], map_g[2], map_s[2], map_phi[2], map_pdot[2];
-    // gather kernel with the phi halo tile staged by TMA: one box per CTA
+    // K_main variants: phi halo tile staged by TMA, one box per CTA (k_main_phitma.cuh) ...
     bool phi_tma;
     // ... and the pulled populations, phi^n, Pdot staged by per-thread cp.async (k_main_smem.cuh)
     bool pops_smem;
-    // fused variant: K_phi folded into K_main (3D only), Pdot double-buffered
-    bool fused;
+    // K_phi and K_main as work items of one launch per step (k_step.cuh)
+    bool one_launch;
+    lbm::SweepPlan sweep;
+    int attr_done[8];   // kernel attributes set on this context's device: [MODE] K_main, [4 + MODE] single-launch step
     // CUDA graph of two consecutive plain steps, for launch-bound (small) grids
     bool graph_ok;
     cudaGraphExec_t graph2;

@@ -3,11 +3,10 @@
 
 #include "ctx.h"
 #include "k_main.cuh"
-#include "k_main_fused.cuh"
 #include "k_main_phitma.cuh"
 #include "k_main_smem.cuh"
-#include "k_main_tma.cuh"
 #include "k_phi.cuh"
+#include "k_step.cuh"
 
 namespace lbm {
 
@@ -56,19 +55,13 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     //            256-thread tiles 768
     //   fp32   : 1024 (64 registers; +25% over 512 although a few values spill); 2D with staged populations on 4096x3072,
     //            768 / 1024 / 1280 / 1536 threads: 0.481 / 0.470 / 0.506 / 0.570 ms (three D2Q9: 0.541 / 0.533 / 0.604 / 0.778)
-#ifndef LBM_THREADS3D
-#define LBM_THREADS3D 512
-#endif
-    static constexpr int THREADS64 = D == 3 ? LBM_THREADS3D : (NT == 128 ? 640 : 768);
+    static constexpr int THREADS64 = D == 3 ? 512 : (NT == 128 ? 640 : 768);
     static constexpr int THREADS32 = 1024;
     static constexpr int MINB = (sizeof(real) == 8 ? THREADS64 : THREADS32) / NT;
-#ifndef LBM_PHI_NPT
-#define LBM_PHI_NPT 2
-#endif
-#ifndef LBM_PHI_NPT32
-#define LBM_PHI_NPT32 2
-#endif
-    static constexpr int PHI_NPT = sizeof(sreal) == 8 ? LBM_PHI_NPT : LBM_PHI_NPT32;   // nodes per thread in K_phi
+    static constexpr int PHI_NPT = 2;   // nodes per thread in K_phi (1: 0.427 ms, 2: 0.378, 4: 0.447 on config 4 fp64)
+    // the single-launch step (k_step.cuh) needs tiles of one layer of the slow axis
+    static constexpr bool STEP_OK = T::BZ == 1 && (D == 3 || T::BY == 1);
+    static constexpr int STEP_BM = D == 3 ? T::BY : 1;
 
     static Fields fields(const lbm_ctx *c, int in, int out, int phi_new, int phi_old) {
         Fields F{};
@@ -85,43 +78,26 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         return F;
     }
 
-    template <int MODE> static int launch_main(lbm_ctx *c, const Fields &F, int in = 0, int pnew = 0) {
-        if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU && UNIFORM) {
-            if (c->use_tma) {
-                using C = TmaCfg<LF, LG, LS, real>;
-                auto kern = k_main_tma<LF, LG, LS, real, MODE>;
-                static bool attr_set = false;
-                if (!attr_set) {
-                    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-                    attr_set = true;
-                }
-                TmaMaps M;
-                M.f = c->map_f[in]; M.g = c->map_g[in]; M.s = c->map_s[in];
-                M.phi_new = c->map_phi[pnew]; M.phi_old = c->map_phi[1 - pnew]; M.pdot = c->map_pdot[in];
-                const int nxt = (c->P.nx + C::TX - 1) / C::TX, nyt = (c->P.ny + C::TY - 1) / C::TY;
-                const long long ntiles = (long long)nxt * nyt * c->P.nz;
-                const unsigned grid = (unsigned)(ntiles < c->num_sms ? ntiles : c->num_sms);
-                kern<<<grid, C::NT, C::SMEM_BYTES, c->stream>>>(dev_params<real>(c), F, M, ntiles, nxt, nyt);
-                c->launches++;
-                CK(cudaGetLastError());
-                return LBM_OK;
-            }
-        }
+    // kernel attributes are per device: set once per context (lbm_create may run on any device of the process)
+    template <class K> static int set_smem_attrs(lbm_ctx *c, K kern, size_t bytes, int &done_flag) {
+        if (done_flag) return LBM_OK;
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+        // shared-memory carve-out: just enough for MINB resident CTAs (+1 KB each that the driver reserves), the rest
+        // stays L1 -- the shifted pulls of neighbouring warps share sectors there (measured on config 4, K_main ms:
+        // 60 KB of L1: 2.89, 92 KB: 2.82, and 3.75 with the maximum carve-out)
+        const int pct = (int)((MINB * (bytes + 1024) * 100 + 233471) / 233472);
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, pct > 100 ? 100 : pct));
+        done_flag = 1;
+        return LBM_OK;
+    }
+
+    template <int MODE> static int launch_main(lbm_ctx *c, const Fields &F, int pnew = 0) {
         if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU) {
             if (c->phi_tma && c->pops_smem) {
                 using C = SmemCfg<LF, LG, LS, sreal, preal, T::BX, T::BY, T::BZ>;
                 auto kern = k_main_smem<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB, Fields>;
-                static bool attr_set = false;
-                if (!attr_set) {
-                    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::BYTES));
-                    // shared-memory carve-out: just enough for MINB resident CTAs (+1 KB each that the driver reserves), the rest
-                    // stays L1 -- the shifted pulls of neighbouring warps share sectors there (measured on config 4, K_main ms:
-                    // 60 KB of L1: 2.89, 92 KB: 2.82, and 3.75 with the maximum carve-out)
-                    const char *co = getenv("LBM_CARVEOUT");   // tuning only
-                    const int pct = (co && *co) ? atoi(co) : (int)((MINB * (C::BYTES + 1024) * 100 + 233471) / 233472);
-                    CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, pct > 100 ? 100 : pct));
-                    attr_set = true;
-                }
+                int rc = set_smem_attrs(c, kern, C::BYTES, c->attr_done[MODE]);
+                if (rc) return rc;
                 kern<<<grid_for<T>(c->P), NT, C::BYTES, c->stream>>>(dev_params<real>(c), F, c->map_phi_tile[pnew]);
                 c->launches++;
                 CK(cudaGetLastError());
@@ -139,6 +115,36 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
             <<<grid_for<T>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F);
         c->launches++;
         CK(cudaGetLastError());
+        return LBM_OK;
+    }
+
+    // the whole step in one launch (k_step.cuh); the buffers flip
+    template <int MODE, bool POPS_SMEM, bool STAGE_G = POPS_SMEM> static int launch_step_kernel(lbm_ctx *c, const Fields &F, int pnew) {
+        if constexpr (STEP_OK) {
+            using CS = SmemCfg<LF, LG, LS, sreal, preal, T::BX, D == 3 ? T::BY : 1, 1, STAGE_G>;
+            using CP = PhiTileSmem<preal, PhiTileCfg<preal, D, T::BX, D == 3 ? T::BY : 1, 1>>;
+            constexpr size_t BYTES = POPS_SMEM ? CS::BYTES : CP::BYTES;
+            auto kern = k_step<LF, LG, LS, real, MODE, T::BX, STEP_BM, MINB, POPS_SMEM, STAGE_G, Fields>;
+            int rc = set_smem_attrs(c, kern, BYTES, c->attr_done[4 + MODE + (STAGE_G ? 0 : 2)]);
+            if (rc) return rc;
+            kern<<<c->sweep.total, NT, BYTES, c->stream>>>(dev_params<real>(c), F, wsp<preal>(c, c->L.off_phi[pnew]),
+                                                           c->map_phi_tile[pnew], c->sweep);
+            c->launches++;
+            CK(cudaGetLastError());
+            return LBM_OK;
+        } else {
+            return LBM_E_UNSUPPORTED;
+        }
+    }
+    static int launch_step(lbm_ctx *c, bool macro) {
+        const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
+        Fields F = fields(c, in, out, pnew, pold);
+        int rc;
+        if (c->pops_smem && (c->sweep.xflags & 1)) rc = macro ? launch_step_kernel<MODE_STEP_MACRO, true, false>(c, F, pnew) : launch_step_kernel<MODE_STEP, true, false>(c, F, pnew);
+        else if (c->pops_smem) rc = macro ? launch_step_kernel<MODE_STEP_MACRO, true>(c, F, pnew) : launch_step_kernel<MODE_STEP, true>(c, F, pnew);
+        else rc = macro ? launch_step_kernel<MODE_STEP_MACRO, false>(c, F, pnew) : launch_step_kernel<MODE_STEP, false>(c, F, pnew);
+        if (rc) return rc;
+        c->cur = out; c->curphi = pnew; c->nsteps++;
         return LBM_OK;
     }
 
@@ -174,29 +180,6 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         return LBM_OK;
     }
 
-    // fused variant (3D): one kernel per step, see k_main_fused.cuh
-#ifndef LBM_FBX
-#define LBM_FBX 64
-#define LBM_FBY 4
-#define LBM_FLZ 32
-#endif
-    struct FusedCfg { static constexpr int BX = LBM_FBX, BY = LBM_FBY, LZ = LBM_FLZ; };
-    template <int MODE> static int launch_fused(lbm_ctx *c, Fields F, int in, int pnew) {
-        if constexpr (D == 3 && UNIFORM) {
-            const dim3 grid((c->P.nx + FusedCfg::BX - 1) / FusedCfg::BX, (c->P.ny + FusedCfg::BY - 1) / FusedCfg::BY,
-                            (c->P.nz + FusedCfg::LZ - 1) / FusedCfg::LZ);
-            // register bound: the same threads per SM as K_main, in CTAs of BX x BY threads
-            constexpr int FMINB = (sizeof(real) == 8 ? THREADS64 : THREADS32) / (FusedCfg::BX * FusedCfg::BY);
-            k_main_fused<LF, LG, LS, real, MODE, FusedCfg::BX, FusedCfg::BY, FusedCfg::LZ, FMINB>
-                <<<grid, FusedCfg::BX * FusedCfg::BY, 0, c->stream>>>(dev_params<real>(c), F, wsp<real>(c, c->L.off_phi[pnew]));
-            c->launches++;
-            CK(cudaGetLastError());
-            return LBM_OK;
-        } else {
-            return LBM_E_UNSUPPORTED;
-        }
-    }
-
     // phase 0 of a step: K_phi (phi^{n+1} of every node, Eq.32)
     static int launch_phi(lbm_ctx *c) {
         const DevParams<real> &P = dev_params<real>(c);
@@ -216,8 +199,8 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
         Fields F = fields(c, in, out, pnew, pold);
         int rc;
-        if (P.prescribed_u) rc = launch_main<MODE_STEP_PU>(c, F, in, pnew);   // direct kernel only
-        else rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, in, pnew) : launch_main<MODE_STEP>(c, F, in, pnew);
+        if (P.prescribed_u) rc = launch_main<MODE_STEP_PU>(c, F, pnew);   // direct kernel only
+        else rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, pnew) : launch_main<MODE_STEP>(c, F, pnew);
         if (rc) return rc;
         c->cur = out; c->curphi = pnew; c->nsteps++;
         return LBM_OK;
@@ -236,13 +219,10 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
             CK(cudaEventRecord(e3[0], c->stream));
         }
         int rc;
-        if (c->fused && !dev_params<real>(c).prescribed_u) {
-            const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
-            Fields F = fields(c, in, out, pnew, pold);
+        if (c->one_launch) {
             if (timed) CK(cudaEventRecord(e3[1], c->stream));
-            rc = macro ? launch_fused<MODE_STEP_MACRO>(c, F, in, pnew) : launch_fused<MODE_STEP>(c, F, in, pnew);
+            rc = launch_step(c, macro);
             if (rc) return rc;
-            c->cur = out; c->curphi = pnew; c->nsteps++;
         } else {
             rc = launch_phi(c);
             if (rc) return rc;
@@ -345,7 +325,8 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     }
 
     static const ImplOps *ops() {
-        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::step_phase, &Impl::read_macro, &Impl::read_pops, T::BX, T::BY, T::BZ};
+        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::step_phase, &Impl::read_macro, &Impl::read_pops, T::BX, T::BY, T::BZ,
+                                  STEP_OK ? STEP_BM : 0};
         return &o;
     }
 };

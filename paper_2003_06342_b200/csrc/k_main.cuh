@@ -11,11 +11,7 @@ namespace lbm {
 
 // population stores: written once, read by the NEXT step only
 template <class sreal, class real> __device__ __forceinline__ void st_pop(sreal *p, real v) {
-#ifdef LBM_EXP_STCS
-    __stcs(p, sreal(v));
-#else
     *p = sreal(v);
-#endif
 }
 
 __device__ __forceinline__ double rsqrt_(double a) { return rsqrt(a); }

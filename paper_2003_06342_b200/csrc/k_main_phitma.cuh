@@ -3,11 +3,21 @@
 // node become shared-memory loads; the populations are gathered from global memory as in k_main_direct.
 // The padded phi array has materialised ghost layers and a 16-byte x offset (xpad), so the box
 // [x0 - EPB, x0 + BX + EPB) x [y0 - 1, y0 + BY] x [z0 - 1, z0 + BZ] always starts 16-byte aligned and never needs wrap logic.
+//
+// The tile bodies are device functions taking the tile origin and a `ready` hook that runs after the tile's independent loads
+// have been issued and before the phi box is requested: a no-op when K_phi is its own launch (the kernels below), the wait for
+// the producing K_phi items when both run in one launch (k_step.cuh).
 #pragma once
 
-#include "k_main_tma.cuh"   // PTX wrappers (mbarrier, TMA)
+#include "k_main.cuh"
+#include "ptx.cuh"
 
 namespace lbm {
+
+struct NoWait {
+    static constexpr bool WAITS = false;
+    __device__ __forceinline__ void operator()() const {}
+};
 
 template <class real, int D, int BX, int BY, int BZ> struct PhiTileCfg {
     static constexpr int EPB = 16 / (int)sizeof(real);
@@ -43,24 +53,45 @@ template <class LF, class LG, class LS, class real, bool BC, class TC, class Fie
     template <int I, bool AGAIN = false> __device__ __forceinline__ real gg() const { return pull_one<LG, I, real, BC, AGAIN>(Fd.g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi); }
 };
 
-template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB, class Fields>
-__global__ void __launch_bounds__(BX *BY *BZ, MINB)
-k_main_phitma(const DevParams<real> P, const Fields Fd, const __grid_constant__ CUtensorMap phi_map) {
+// shared memory of one CTA: the phi tile and its mbarrier
+template <class preal, class TC> struct PhiTileSmem {
+    static constexpr size_t TILE_BYTES = ((size_t)TC::BYTES + 127) / 128 * 128;
+    static constexpr size_t BYTES = TILE_BYTES + 16;
+};
+
+// one tile of BX x BY x BZ nodes with origin (x0, y0, z0); smem_raw: PhiTileSmem::BYTES bytes, 128-byte aligned
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, class Fields, class Ready>
+__device__ __forceinline__ void main_tile_phitma(const DevParams<real> &P, const Fields &Fd, const CUtensorMap *phi_map,
+                                                 unsigned char *smem_raw, int x0, int y0, int z0, const Ready &ready) {
     using preal = typename Fields::preal;
     using TC = PhiTileCfg<preal, LF::D, BX, BY, BZ>;
-    __shared__ __align__(128) preal tile[TC::ELEMS];
-    __shared__ __align__(8) uint64_t bar;
+    using SM = PhiTileSmem<preal, TC>;
+    preal *tile = reinterpret_cast<preal *>(smem_raw);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + SM::TILE_BYTES);
     const int t = threadIdx.x;
-    const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY, z0 = blockIdx.z * BZ;
     const int tx = t % BX, ty = (t / BX) % BY, tz = t / (BX * BY);
-    const uint32_t bar_a = smem_u32(&bar);
+    const uint32_t bar_a = smem_u32(bar);
     if (t == 0) {
         mbar_init(bar_a, 1);
         fence_mbar_init();
         fence_proxy_async();
-        mbar_expect_tx(bar_a, TC::BYTES);
-        // padded coordinates of node (x0 - EPB, y0 - 1, z0 - 1): (x0, y0, z0 + pz - 1)
-        tma_load_3d(smem_u32(tile), &phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
+        if constexpr (!Ready::WAITS) {
+            mbar_expect_tx(bar_a, TC::BYTES);
+            // padded coordinates of node (x0 - EPB, y0 - 1, z0 - 1): (x0, y0, z0 + pz - 1)
+            tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
+        }
+    }
+    if constexpr (Ready::WAITS) {
+        // single-launch step (k_step.cuh): warp 0 waits for the producers of phi^{n+1} in the box, then requests it
+        if (t < 32) {
+            ready();
+            __syncwarp();
+            if (t == 0) {
+                fence_proxy_async_global();   // the acquired generic-proxy writes of phi^{n+1} before the async-proxy read
+                mbar_expect_tx(bar_a, TC::BYTES);
+                tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
+            }
+        }
     }
     __syncthreads();   // the barrier is initialised before anybody waits on it
     const int x = x0 + tx, y = y0 + ty, z = z0 + tz;
@@ -73,6 +104,16 @@ k_main_phitma(const DevParams<real> P, const Fields Fd, const __grid_constant__ 
         const SrcGlobalPhiSmem<LF, LG, LS, real, false, TC, Fields> src(P, Fd, g, tile, bar_a, tx, ty, tz);
         node_update<LF, LG, LS, real, MODE>(P, Fd, g, src);
     }
+}
+
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB, class Fields>
+__global__ void __launch_bounds__(BX *BY *BZ, MINB)
+k_main_phitma(const DevParams<real> P, const Fields Fd, const __grid_constant__ CUtensorMap phi_map) {
+    using preal = typename Fields::preal;
+    using SM = PhiTileSmem<preal, PhiTileCfg<preal, LF::D, BX, BY, BZ>>;
+    __shared__ __align__(128) unsigned char smem_raw[SM::BYTES];
+    main_tile_phitma<LF, LG, LS, real, MODE, BX, BY, BZ>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, blockIdx.y * BY,
+                                                          blockIdx.z * BZ, NoWait{});
 }
 
 }  // namespace lbm

@@ -1,5 +1,5 @@
 // K_main, gather variant with EVERY input of the node staged in shared memory: the phi^{n+1} halo tile by one TMA box per CTA
-// (as k_main_phitma.cuh) and the pulled f and s populations (26 in 3D; g only with LBM_SMEM_STAGE_G), phi^n and Pdot by per-thread asynchronous copies
+// (as k_main_phitma.cuh) and the pulled f and s populations (26 in 3D), phi^n and Pdot by per-thread asynchronous copies
 // (cp.async -> LDGSTS) into the thread's own column of a [value][thread] array.  All of a thread's loads are in flight at once
 // without occupying registers (Little's law: 16 warps x 32 lanes x 28 x 8 B = 115 KB in flight per SM), and the second read of every
 // population at collision time is a shared-memory load instead of an L2 round trip (the 200 KB L1 does not hold the
@@ -7,17 +7,9 @@
 // the gather path of k_main_phitma.cuh (boundary rules select other addresses); the choice is tile-uniform.
 #pragma once
 
-#include "k_main_fused.cuh"   // cp_async_commit / cp_async_wait_all
 #include "k_main_phitma.cuh"
 
 namespace lbm {
-
-__device__ __forceinline__ void cp_async_val(uint32_t dst, const double *src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_val(uint32_t dst, const float *src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
-}
 
 // element offset of the pull source of direction I (periodic wrap only)
 template <class L, int I> __device__ __forceinline__ unsigned pull_offset(unsigned N, const NodeGeom &g) {
@@ -25,13 +17,12 @@ template <class L, int I> __device__ __forceinline__ unsigned pull_offset(unsign
 }
 
 // shared-memory carve-up of one CTA of NT threads
-template <class LF, class LG, class LS, class sreal, class preal, int BX, int BY, int BZ> struct SmemCfg {
+// STAGE_G: g is read once (at its collision), so staging it only buys the early issue -- which is what the single-launch step
+// wants (k_step.cuh: the g lines K_phi has just pulled are re-read while they are still in L2).
+template <class LF, class LG, class LS, class sreal, class preal, int BX, int BY, int BZ, bool STAGE_G_ = false> struct SmemCfg {
     using TC = PhiTileCfg<preal, LF::D, BX, BY, BZ>;
     static constexpr int NT = BX * BY * BZ;
-#ifndef LBM_SMEM_STAGE_G
-#define LBM_SMEM_STAGE_G 0
-#endif
-    static constexpr bool STAGE_G = LBM_SMEM_STAGE_G != 0;   // g is read once (at its collision): staging it only buys the early issue
+    static constexpr bool STAGE_G = STAGE_G_;
     static constexpr int QT = LF::Q + LS::Q + (STAGE_G ? LG::Q : 0);
     static constexpr int OFF_F = 0, OFF_S = LF::Q, OFF_G = LF::Q + LS::Q, OFF_PDOT = QT;   // sreal slots
     static constexpr size_t TILE_BYTES = ((size_t)TC::BYTES + 127) / 128 * 128;
@@ -84,7 +75,7 @@ template <class LF, class LG, class LS, class real, class C, class Fields> struc
         cp_async_commit();   // group 2: f (and g), first needed by the moments
     }
     // own copies only: no CTA barrier needed, nobody else reads the column
-    __device__ __forceinline__ void pops_ready() const { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+    __device__ __forceinline__ void pops_ready() const { cp_async_wait_1(); }
     __device__ __forceinline__ void f_ready() const { cp_async_wait_all(); }
     __device__ __forceinline__ void phi_ready() const { mbar_wait(bar, 0); }
     __device__ __forceinline__ preal phi(int dx, int dy, int dz) const { return tile[dx + dy * TC::BOXX + dz * (TC::BOXX * TC::BOXY)]; }
@@ -98,28 +89,42 @@ template <class LF, class LG, class LS, class real, class C, class Fields> struc
     }
 };
 
-template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB, class Fields>
-__global__ void __launch_bounds__(BX *BY *BZ, MINB)
-k_main_smem(const DevParams<real> P, const Fields Fd, const __grid_constant__ CUtensorMap phi_map) {
+// one tile of BX x BY x BZ nodes with origin (x0, y0, z0); smem_raw: SmemCfg::BYTES bytes of dynamic shared memory
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, bool STAGE_G = false, class Fields, class Ready>
+__device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const Fields &Fd, const CUtensorMap *phi_map,
+                                               unsigned char *smem_raw, int x0, int y0, int z0, const Ready &ready) {
     using sreal = typename Fields::sreal;
     using preal = typename Fields::preal;
-    using C = SmemCfg<LF, LG, LS, sreal, preal, BX, BY, BZ>;
+    using C = SmemCfg<LF, LG, LS, sreal, preal, BX, BY, BZ, STAGE_G>;
     using TC = typename C::TC;
-    extern __shared__ __align__(128) unsigned char smem_raw[];
     preal *tile = reinterpret_cast<preal *>(smem_raw);
     preal *phiold = reinterpret_cast<preal *>(smem_raw + C::TILE_BYTES);
     sreal *pops = reinterpret_cast<sreal *>(smem_raw + C::TILE_BYTES + C::PHIOLD_BYTES);
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + C::TILE_BYTES + C::PHIOLD_BYTES + C::POPS_BYTES);
     const int t = threadIdx.x;
-    const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY, z0 = blockIdx.z * BZ;
     const int tx = t % BX, ty = (t / BX) % BY, tz = t / (BX * BY);
     const uint32_t bar_a = smem_u32(bar);
     if (t == 0) {
         mbar_init(bar_a, 1);
         fence_mbar_init();
         fence_proxy_async();
-        mbar_expect_tx(bar_a, TC::BYTES);
-        tma_load_3d(smem_u32(tile), &phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
+        if constexpr (!Ready::WAITS) {
+            mbar_expect_tx(bar_a, TC::BYTES);
+            tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
+        }
+    }
+    if constexpr (Ready::WAITS) {
+        // single-launch step (k_step.cuh): warp 0 waits for the producers of phi^{n+1} in the box BEFORE it issues its own
+        // population copies (the polls would queue behind them), then requests the box; the other warps go straight on
+        if (t < 32) {
+            ready();
+            __syncwarp();
+            if (t == 0) {
+                fence_proxy_async_global();   // the acquired generic-proxy writes of phi^{n+1} before the async-proxy read
+                mbar_expect_tx(bar_a, TC::BYTES);
+                tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
+            }
+        }
     }
     const int x = x0 + tx, y = y0 + ty, z = z0 + tz;
     const bool active = x < P.nx && y < P.ny && z < P.nz;
@@ -129,7 +134,7 @@ k_main_smem(const DevParams<real> P, const Fields Fd, const __grid_constant__ CU
         g = make_geom(P, x, y, z);
         if (!bc) {
             const SrcSmem<LF, LG, LS, real, C, Fields> src(P, Fd, g, tile, phiold, pops, bar_a, t, tx, ty, tz);
-            src.prefetch();   // before the barrier below: the copies fly while the CTA assembles
+            src.prefetch();   // before the barrier below: the copies fly while the CTA assembles (and while `ready` waits)
         }
     }
     __syncthreads();   // the mbarrier is initialised before anybody waits on it
@@ -141,6 +146,14 @@ k_main_smem(const DevParams<real> P, const Fields Fd, const __grid_constant__ CU
         const SrcSmem<LF, LG, LS, real, C, Fields> src(P, Fd, g, tile, phiold, pops, bar_a, t, tx, ty, tz);
         node_update<LF, LG, LS, real, MODE>(P, Fd, g, src);
     }
+}
+
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB, class Fields>
+__global__ void __launch_bounds__(BX *BY *BZ, MINB)
+k_main_smem(const DevParams<real> P, const Fields Fd, const __grid_constant__ CUtensorMap phi_map) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    main_tile_smem<LF, LG, LS, real, MODE, BX, BY, BZ>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, blockIdx.y * BY,
+                                                        blockIdx.z * BZ, NoWait{});
 }
 
 }  // namespace lbm

@@ -210,9 +210,11 @@ class SlabGroup:
     """``nslabs`` slabs of one domain in one process, on the current device and stream."""
 
     def __init__(self, P: dict, nslabs: int, precision: int = 64):
+        import torch
         self.P = P
         self.periodic = axis_is_periodic(P)
-        self.slabs = [Slab(P, r, nslabs, precision) for r in range(nslabs)]
+        self.stream = torch.cuda.Stream()   # one stream for all slabs: pack, hand-over and unpack are ordered by it
+        self.slabs = [Slab(P, r, nslabs, precision, stream=self.stream) for r in range(nslabs)]
         self.any_halo = any(s.has_halo for s in self.slabs)
 
     def init(self, phi, T=None, u=None, p=None):
@@ -253,8 +255,10 @@ class DistSlab:
 
     def __init__(self, P: dict, rank: int, world: int, precision: int = 64, group=None):
         self.periodic = axis_is_periodic(P)
+        import torch
         self.rank, self.world, self.group = rank, world, group
-        self.slab = Slab(P, rank, world, precision)
+        # the transfers (torch.distributed) are enqueued on torch's current stream: the slab's kernels go there too
+        self.slab = Slab(P, rank, world, precision, stream=torch.cuda.current_stream())
 
     def init(self, phi, T=None, u=None, p=None, local=False):
         """GLOBAL fields, or with ``local=True`` this rank's layers including the ghost copies (Slab.layer_range)."""

@@ -111,7 +111,7 @@ def test_3d_periodic_ragged(gpu, oracle_mod):
 def test_3d_mid_tiles(gpu, oracle_mod):
     """Rows that are a multiple of 64 but not worth a 128-wide tile (192, 320; here 64 and 192) run 64 x 2 tiles in fp64 3D."""
     P = wl.base_params(64, 7, 5, grav=[1e-4, -1e-4, -2e-4])
-    sim = gpu.LBM(P, 64); assert sim.variant == "gather+smem"; sim.destroy()
+    sim = gpu.LBM(P, 64); assert sim.variant == "one-launch gather+smem"; sim.destroy()
     _run_parity(gpu, oracle_mod, P, _random_state(P, 61), [1, 12], label="3d 64-wide periodic")
     P = wl.base_params(192, 5, 6, grav=[0.0, 0.0, -1e-4], lat_f="D3Q15")
     P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
@@ -207,12 +207,18 @@ def test_minimal_grids(gpu, oracle_mod):
         _run_parity(gpu, oracle_mod, P, _random_state(P, 30), [1, 4], label="tiny %s" % (dims,))
 
 
-# ---------------------------------------------------------------------------- K_main variants
-def test_k_main_variants_by_staging(gpu, oracle_mod, monkeypatch):
-    """K_main by what it stages in shared memory.  Default in fp64 (and fp32 2D): "gather+smem", phi halo tile by one TMA box
-    per CTA and the node's populations, phi^n, Pdot by per-thread cp.async (k_main_smem.cuh); fp32 3D: "gather+phi-tma"
-    (populations gathered into registers).  LBM_POPS=ldg / LBM_PHI=ldg select the plainer kernels.  Every one must match the
-    oracle on periodic and walled, 2D and 3D, narrow- and wide-tile grids (the other tests in this file run the defaults)."""
+# ---------------------------------------------------------------------------- kernel variants (lbm_params.flags)
+def _with_kernels(P, *names):
+    Q = dict(P); Q["kernels"] = tuple(names)
+    return Q
+
+
+def test_kernel_variants(gpu, oracle_mod):
+    """The step by how it is launched and what K_main stages in shared memory (include/lbm.h "Kernel selection").
+    Defaults: one launch per step (k_step.cuh) on tiles of one layer, "gather+smem" (phi halo tile by one TMA box per CTA,
+    the node's populations, phi^n, Pdot by per-thread cp.async) in fp64 and fp32 2D, "gather+phi-tma" (populations gathered
+    into registers) in fp32 3D.  The flags force the plainer kernels.  Every one must match the oracle on periodic and
+    walled, 2D and 3D, narrow- and wide-tile grids (the other tests in this file run the defaults)."""
     P3 = wl.base_params(40, 10, 7, grav=[1e-4, 0.0, -2e-4])                     # narrow tiles, ragged
     P3w = wl.base_params(256, 6, 5, grav=[1e-4, 0.0, -2e-4], force=[0.0, 1e-5, 0.0])   # wide tiles, two per row
     P2 = wl.base_params(40, 20, 1, grav=[0.0, -1e-4, 0.0])
@@ -223,27 +229,70 @@ def test_k_main_variants_by_staging(gpu, oracle_mod, monkeypatch):
     P3z["bc_f"][2] = ["wall", "wall"]; P3z["bc_g"][2] = ["zeroflux", "zeroflux"]; P3z["bc_s"][2] = ["dirichlet", "dirichlet"]
     P3z["bc_T"][2] = [1.0, 0.0]
     cases = ((P3, 34), (P3w, 44), (P2, 35), (P2w, 45), (P3z, 46))
-    for env, want64, want32_3d in (({}, "gather+smem", "gather+phi-tma"), ({"LBM_POPS": "ldg"}, "gather+phi-tma", "gather+phi-tma"),
-                                   ({"LBM_POPS": "smem"}, "gather+smem", "gather+smem"), ({"LBM_PHI": "ldg"}, "direct", "direct")):
-        for k in ("LBM_POPS", "LBM_PHI"):
-            monkeypatch.delenv(k, raising=False)
-        for k, v in env.items():
-            monkeypatch.setenv(k, v)
-        sim = gpu.LBM(P3, 64); assert sim.variant == want64, (env, sim.variant); sim.destroy()
-        sim = gpu.LBM(P3, 32); assert sim.variant == want32_3d, (env, sim.variant); sim.destroy()
+    # (flags, variant of the wide 3D case in fp64, in fp32)
+    for names, want64, want32 in (((), "one-launch gather+smem", "one-launch gather+phi-tma"),
+                                  (("two_launches",), "gather+smem", "gather+phi-tma"),
+                                  (("pops_gather",), "one-launch gather+phi-tma", "one-launch gather+phi-tma"),
+                                  (("pops_staged",), "one-launch gather+smem", "one-launch gather+smem"),
+                                  (("two_launches", "pops_gather"), "gather+phi-tma", "gather+phi-tma"),
+                                  (("phi_ldg",), "direct", "direct")):
+        sim = gpu.LBM(_with_kernels(P3w, *names), 64); assert sim.variant == want64, (names, sim.variant); sim.destroy()
+        sim = gpu.LBM(_with_kernels(P3w, *names), 32); assert sim.variant == want32, (names, sim.variant); sim.destroy()
         for P, seed in cases:
-            _run_parity(gpu, oracle_mod, P, _random_state(P, seed), [1, 12], label="%s %dx%dx%d" % (env, P["nx"], P["ny"], P["nz"]))
+            _run_parity(gpu, oracle_mod, _with_kernels(P, *names), _random_state(P, seed), [1, 12],
+                        label="%s %dx%dx%d" % (names, P["nx"], P["ny"], P["nz"]))
+    # narrow tiles span two layers: two launches whatever the flags
+    sim = gpu.LBM(P3, 64); assert sim.variant == "gather+smem", sim.variant; sim.destroy()
     # fp32 with the staged kernel (3D opt-in, 2D default): inside the fp32 bar
-    monkeypatch.delenv("LBM_PHI", raising=False)
-    monkeypatch.setenv("LBM_POPS", "smem")
     for P, seed in ((P3w, 44), (P2w, 45)):
+        for names in (("pops_staged",), ("pops_staged", "two_launches")):
+            init = _random_state(P, seed)
+            o = oracle_mod.Oracle(P); o.init(*init); o.step(12)
+            sim = gpu.LBM(_with_kernels(P, *names), 32); sim.init(*[a.astype(np.float32) for a in init]); sim.step(12)
+            assert sim.variant.endswith("gather+smem")
+            for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
+                assert _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30) <= REL32, name
+            sim.destroy(); o.close()
+
+
+def test_one_launch_step_sweep_orders(gpu, oracle_mod):
+    """The single-launch step (k_step.cuh) must give the same result whatever the order of its work items: mid-axis blocks of
+    4..16 rows (several blocks, ragged last block, the shifted K_phi windows), leads 0..3, odd and even numbers of layers,
+    periodic and walled slow / mid axes.  Every order gives the same bits (same kernel, same arithmetic per node); the
+    two-launch step (other instantiations: the compiler contracts differently) agrees to rounding, the oracle within 1e-10."""
+    cases = []
+    P = wl.base_params(250, 37, 9, grav=[1e-4, -1e-4, -2e-4], force=[1e-5, 0.0, 2e-5])     # wide tiles, ragged x, odd nz
+    cases.append((P, 81))
+    P = wl.base_params(128, 22, 8, grav=[0.0, 0.0, -1e-4])                                  # y and z walls
+    for a in (1, 2):
+        P["bc_f"][a] = ["wall", "wall"]; P["bc_g"][a] = ["zeroflux", "dirichlet" if a == 1 else "zeroflux"]
+        P["bc_s"][a] = ["dirichlet", "dirichlet"]; P["bc_T"][a] = [1.0, 0.0]; P["bc_phi"][a] = [0.0, 1.0]
+    cases.append((P, 82))
+    P = wl.base_params(64, 26, 7, grav=[1e-4, 0.0, -2e-4])                                  # 64 x 2 tiles
+    cases.append((P, 83))
+    P = wl.base_params(256, 19, 1, grav=[1e-4, -1e-4, 0.0])                                 # 2D: the slow axis is y
+    cases.append((P, 84))
+    for P, seed in cases:
         init = _random_state(P, seed)
-        o = oracle_mod.Oracle(P); o.init(*init); o.step(12)
-        sim = gpu.LBM(P, 32); sim.init(*[a.astype(np.float32) for a in init]); sim.step(12)
-        assert sim.variant == "gather+smem"
-        for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
-            assert _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30) <= REL32, name
-        sim.destroy(); o.close()
+        o = oracle_mod.Oracle(P); o.init(*init); o.step(9)
+        ref = gpu.LBM(_with_kernels(P, "two_launches"), 64); ref.init(*init); ref.step(9)
+        want = ref.read_macro() + tuple(ref.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
+        ref.destroy()
+        first = None
+        for rows, lead in ((0, -1), (4, 0), (4, 3), (6, 1), (8, 2), (16, 1), (1000, 0)):
+            sim = gpu.LBM(P, 64)
+            assert sim.variant.startswith("one-launch")
+            sim.set_sweep(rows, lead)
+            sim.init(*init); sim.step(4); sim.step(5)
+            sim.sync()
+            got = sim.read_macro() + tuple(sim.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
+            first = first or got
+            for a, b, w in zip(got, first, want):
+                assert np.array_equal(a, b), (P["nx"], P["ny"], P["nz"], rows, lead, _maxabs(a, b))
+                assert _maxabs(a, w) <= 1e-13, (P["nx"], P["ny"], P["nz"], rows, lead, _maxabs(a, w))
+            _compare_state(gpu, sim, o, oracle_mod, TOL64, True, "one launch rows %d lead %d" % (rows, lead))
+            sim.destroy()
+        o.close()
 
 
 def test_cuda_graph_replay_on_side_stream(gpu, oracle_mod):
@@ -263,44 +312,6 @@ def test_cuda_graph_replay_on_side_stream(gpu, oracle_mod):
         _compare_state(gpu, sim, o, oracle_mod, TOL64, True, "graph replay")
         sim.destroy()
     o.close()
-
-
-def test_fused_variant(gpu, oracle_mod, monkeypatch):
-    """LBM_VARIANT=fused (3D): K_phi folded into K_main, phi planes with halo recomputed per CTA from g*."""
-    monkeypatch.setenv("LBM_VARIANT", "fused")
-    P = wl.base_params(70, 10, 37, grav=[1e-4, 0.0, -2e-4])      # ragged in x, y and in the z segments of 32
-    sim = gpu.LBM(P, 64)
-    assert sim.variant == "fused"
-    sim.destroy()
-    _run_parity(gpu, oracle_mod, P, _random_state(P, 36), [1, 2, 12], label="fused 3d periodic")
-    P = wl.base_params(34, 9, 12, grav=[0.0, 0.0, -1e-4])        # z walls, Dirichlet T
-    P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
-    P["bc_T"][2] = [1.0, 0.0]
-    _run_parity(gpu, oracle_mod, P, _random_state(P, 37), [1, 12], label="fused 3d z walls")
-    P = wl.base_params(12, 9, 8)                                 # walls on all axes, Dirichlet phi on the low faces
-    for a in range(3):
-        P["bc_f"][a] = ["wall", "wall"]; P["bc_g"][a] = ["dirichlet", "zeroflux"]; P["bc_s"][a] = ["dirichlet", "zeroflux"]
-        P["bc_phi"][a] = [0.9, 0.0]; P["bc_T"][a] = [0.2, 0.0]
-    _run_parity(gpu, oracle_mod, P, _random_state(P, 38), [1, 3], label="fused 3d box")
-    Pc, I = wl.config4_film3d(nx=48, ny=40, nz=64, h0=12.0, amp=2.0)
-    _run_parity(gpu, oracle_mod, Pc, (I["phi"], I["T"]), [1, 50], pops=False, label="fused config4 48x40x64")
-
-
-# ---------------------------------------------------------------------------- the TMA-staged variant of K_main
-def test_tma_variant(gpu, oracle_mod, monkeypatch):
-    """LBM_VARIANT=tma: persistent kernel, inputs staged through shared memory by cp.async.bulk.tensor."""
-    monkeypatch.setenv("LBM_VARIANT", "tma")
-    P = wl.base_params(264, 10, 7, grav=[1e-4, 0.0, -2e-4])       # 3 x-tiles of 128 (ragged), periodic wrap lanes
-    sim = gpu.LBM(P, 64)
-    assert sim.variant == "tma"
-    sim.destroy()
-    _run_parity(gpu, oracle_mod, P, _random_state(P, 31), [1, 2, 12], label="tma 3d periodic")
-    P = wl.base_params(136, 9, 12, grav=[0.0, 0.0, -1e-4])        # z walls: boundary tiles take the gather path
-    P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
-    P["bc_T"][2] = [1.0, 0.0]
-    _run_parity(gpu, oracle_mod, P, _random_state(P, 32), [1, 12], label="tma 3d z walls")
-    P = wl.base_params(40, 28, 1, grav=[1e-4, -2e-4, 0.0])
-    _run_parity(gpu, oracle_mod, P, _random_state(P, 33), [1, 12], label="tma 2d periodic")
 
 
 # ---------------------------------------------------------------------------- D3Q15 Navier-Stokes lattice (PAPER.md:190)
@@ -325,12 +336,11 @@ def test_d3q15_lattice_set(gpu, oracle_mod):
     _run_parity(gpu, oracle_mod, Pc, (I["phi"], I["T"]), [1, 100], pops=False, label="D3Q15 config4 48x40x64")
 
 
-@pytest.mark.parametrize("env", [("LBM_PHI", "ldg"), ("LBM_VARIANT", "tma"), ("LBM_VARIANT", "fused")])
-def test_d3q15_variants(gpu, oracle_mod, monkeypatch, env):
-    monkeypatch.setenv(*env)
+@pytest.mark.parametrize("names", [("phi_ldg",), ("two_launches",), ("pops_gather",)])
+def test_d3q15_variants(gpu, oracle_mod, names):
     P1, P2, _ = _d3q15_cases()
-    _run_parity(gpu, oracle_mod, P1, _random_state(P1, 74), [1, 8], label="D3Q15 periodic %s" % env[1])
-    _run_parity(gpu, oracle_mod, P2, _random_state(P2, 75), [1, 8], label="D3Q15 z walls %s" % env[1])
+    _run_parity(gpu, oracle_mod, _with_kernels(P1, *names), _random_state(P1, 74), [1, 8], label="D3Q15 periodic %s" % (names,))
+    _run_parity(gpu, oracle_mod, _with_kernels(P2, *names), _random_state(P2, 75), [1, 8], label="D3Q15 z walls %s" % (names,))
 
 
 def test_d3q15_fp32(gpu, oracle_mod):

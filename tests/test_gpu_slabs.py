@@ -120,12 +120,6 @@ def test_fp32_slabs(gpu, oracle_mod):
     _check(gpu, oracle_mod, P, (st["phi"], st["T"], None, None), [3], [1, 6], precision=32, oracle=False, exact=False)
 
 
-def test_tma_variant_slabs(gpu, oracle_mod, monkeypatch):
-    monkeypatch.setenv("LBM_VARIANT", "tma")
-    P, st = wl.config4_film3d(128, 6, 9, h0=4.0, amp=1.0)
-    _check(gpu, oracle_mod, P, (st["phi"], st["T"], None, None), [2], [1, 4], oracle=False, exact=False)
-
-
 def test_prescribed_velocity_slabs(gpu, oracle_mod):
     P = wl.base_params(40, 28, 1, prescribed_u=True)
     _check(gpu, oracle_mod, P, _random_state(P, 64), [2], [1, 5])
