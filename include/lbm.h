@@ -58,10 +58,9 @@ enum {
                                  /* f is still stepped (its p is reported) but its first moment is ignored             */
 /* Kernel selection.  The defaults are chosen by measurement per precision and grid; these flags force
  * the plainer kernels (all are parity-tested; results agree to rounding).  They change speed, never the method. */
-#define LBM_FLAG_TWO_LAUNCHES 8u  /* K_phi and K_main as two launches per step even where one launch is available          */
 #define LBM_FLAG_POPS_GATHER 16u  /* K_main gathers the populations into registers (default of fp32 3D)                    */
 #define LBM_FLAG_POPS_STAGED 32u  /* K_main stages the populations in shared memory with cp.async (default elsewhere)      */
-#define LBM_FLAG_PHI_LDG 64u      /* K_main reads the phi stencil through L1 instead of a TMA box; implies two launches    */
+#define LBM_FLAG_PHI_LDG 64u      /* K_main reads the phi stencil through L1 instead of a TMA box                         */
 #define LBM_FLAG_NO_GRAPH 128u    /* no CUDA-graph replay of the steps of small grids                                      */
 
 /* error codes */
@@ -72,8 +71,7 @@ enum {
     LBM_E_WORKSPACE = -3, /* workspace too small or misaligned                             */
     LBM_E_CUDA = -4,      /* a CUDA runtime call failed (lbm_last_cuda_error for the code) */
     LBM_E_STATE = -5,     /* call not valid in this state (e.g. step before init)          */
-    LBM_E_NODEVICE = -6,  /* no sm_100 device / kernels not loadable                       */
-    LBM_E_HANDOVER = -7   /* the in-kernel hand-over of the single-launch step timed out (lbm_sync; never in a correct run) */
+    LBM_E_NODEVICE = -6   /* no sm_100 device / kernels not loadable                       */
 };
 
 /* which-population selectors and stages of lbm_read_pops */
@@ -148,8 +146,7 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
 int lbm_init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, const void *h_p);
 
 /* Enqueue n full coupled steps (each: K_phi = pull g + Eq.32, then K_main = stencils, closures, moments,
- * production refresh, collision of f, g, s; one launch per step where the tile shape allows it, else two) on the
- * context's stream.  Asynchronous: returns after the
+ * production refresh, collision of f, g, s) on the context's stream.  Asynchronous: returns after the
  * launches; launch errors are returned, execution errors surface at the next synchronising call.
  * The last of the n steps also stores u, p, T for lbm_read_macro. */
 int lbm_step(lbm_ctx *c, int n);
@@ -192,12 +189,6 @@ int lbm_read_pops(lbm_ctx *c, int which, int stage, void *h_pops);
 /* Block until everything enqueued on the context's stream has finished; returns LBM_E_CUDA on a fault. */
 int lbm_sync(lbm_ctx *c);
 
-/* Tuning of the single-launch step: rows of the mid axis (y in 3D) per block of the sweep and lead of the K_phi work items
- * over the K_main work items in layer pairs; 0 rows / negative lead = the built-in defaults.  Changes the order in which
- * the same work is done (i.e. how much of it is found in L2), not any result.  Synchronises.  LBM_E_STATE when the context
- * steps with two launches. */
-int lbm_set_sweep(lbm_ctx *c, int rows_per_block, int lead);
-
 /* Per-kernel device timing for measurement (off by default).  While enabled, lbm_step brackets K_phi and K_main of
  * every step (at most 4096 steps between two lbm_kernel_times calls) with CUDA events on the context's stream.
  * lbm_kernel_times synchronises, returns the summed durations in milliseconds and the number of timed steps,
@@ -209,8 +200,7 @@ int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *ste
 long long lbm_step_count(const lbm_ctx *c);
 long long lbm_launch_count(const lbm_ctx *c);
 
-/* Name of the kernel variant the context steps with, for logs: "one-launch gather+smem", "one-launch gather+phi-tma",
- * "gather+smem", "gather+phi-tma" or "direct". */
+/* Name of the kernel variant the context steps with, for logs: "gather+smem", "gather+phi-tma" or "direct". */
 const char *lbm_variant(const lbm_ctx *c);
 
 /* Last CUDA runtime error code seen by this library (cudaError_t as int), 0 if none. */

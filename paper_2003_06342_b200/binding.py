@@ -22,15 +22,15 @@ FLAG_PHASE_CHANGE = 1
 FLAG_LATENT_HEAT = 2
 FLAG_PRESCRIBED_U = 4
 # kernel selection (include/lbm.h): speed only, never the method
-FLAG_TWO_LAUNCHES, FLAG_POPS_GATHER, FLAG_POPS_STAGED, FLAG_PHI_LDG, FLAG_NO_GRAPH = 8, 16, 32, 64, 128
-KERNEL_FLAGS = {"two_launches": FLAG_TWO_LAUNCHES, "pops_gather": FLAG_POPS_GATHER, "pops_staged": FLAG_POPS_STAGED,
+FLAG_POPS_GATHER, FLAG_POPS_STAGED, FLAG_PHI_LDG, FLAG_NO_GRAPH = 16, 32, 64, 128
+KERNEL_FLAGS = {"pops_gather": FLAG_POPS_GATHER, "pops_staged": FLAG_POPS_STAGED,
                 "phi_ldg": FLAG_PHI_LDG, "no_graph": FLAG_NO_GRAPH}
 POPS_F, POPS_G, POPS_S = 0, 1, 2
 STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1
 
 EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops",
-           "lbm_sync", "lbm_set_sweep", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
+           "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
 
@@ -81,7 +81,6 @@ def load_library():
         L.lbm_read_macro.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_sync.argtypes = [C.c_void_p]
-        L.lbm_set_sweep.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.lbm_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.lbm_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.lbm_step_count.restype = C.c_longlong
@@ -118,7 +117,7 @@ def make_params(P: dict, precision: int = 64) -> lbm_params:
         setattr(s, k, float(P[k]))
     s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0) | (
         FLAG_PRESCRIBED_U if P.get("prescribed_u", False) else 0)
-    for name in P.get("kernels", ()):        # e.g. P["kernels"] = ("two_launches",): force a plainer kernel variant
+    for name in P.get("kernels", ()):        # e.g. P["kernels"] = ("pops_gather",): force a plainer kernel variant
         s.flags |= KERNEL_FLAGS[name]
     halo = P.get("halo", (0, 0))
     s.halo[0], s.halo[1] = int(halo[0]), int(halo[1])
@@ -253,9 +252,6 @@ class LBM:
 
     def sync(self):
         _check(self._L.lbm_sync(self._h), "lbm_sync")
-
-    def set_sweep(self, rows_per_block: int = 0, lead: int = -1):
-        _check(self._L.lbm_set_sweep(self._h, int(rows_per_block), int(lead)), "lbm_set_sweep")
 
     @property
     def stream(self):

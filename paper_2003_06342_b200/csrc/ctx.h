@@ -28,8 +28,7 @@ struct Layout {
     int es, es_phi;   // bytes per element: populations / Pdot / macros / caller's arrays; padded phi arrays
     int ppx, ppy, ppz, pz, xpad;
     size_t phi_pad_elems;
-    size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot[2], off_u, off_p, off_T, off_scratch, off_sync, total;
-    size_t sync_bytes;   // ticket, error flag and slice counters of the single-launch step
+    size_t off_f[2], off_g[2], off_s[2], off_phi[2], off_pdot[2], off_u, off_p, off_T, off_scratch, total;
 };
 
 // One implementation = one (lattice set, precision, tile shape); chosen once in lbm_create.
@@ -40,7 +39,6 @@ struct ImplOps {
     int (*read_macro)(lbm_ctx *, void *, void *, void *, void *);
     int (*read_pops)(lbm_ctx *, int, int, void *);
     int bx, by, bz;   // tile of nodes per CTA
-    int step_bm;      // rows of the mid axis per work item of the single-launch step (k_step.cuh); 0: tile shape not supported
 };
 
 // defined in inst_*.cu (compiled in parallel); nx selects the tile shape
@@ -74,10 +72,7 @@ struct lbm_ctx {
     bool phi_tma;
     // ... and the pulled populations, phi^n, Pdot staged by per-thread cp.async (k_main_smem.cuh)
     bool pops_smem;
-    // K_phi and K_main as work items of one launch per step (k_step.cuh)
-    bool one_launch;
-    lbm::SweepPlan sweep;
-    int attr_done[8];   // kernel attributes set on this context's device: [MODE] K_main, [4 + MODE] single-launch step
+    int attr_done[8];   // kernel attributes set on this context's device: [MODE] K_main
     // CUDA graph of two consecutive plain steps, for launch-bound (small) grids
     bool graph_ok;
     cudaGraphExec_t graph2;

@@ -6,7 +6,6 @@
 #include "k_main_phitma.cuh"
 #include "k_main_smem.cuh"
 #include "k_phi.cuh"
-#include "k_step.cuh"
 
 namespace lbm {
 
@@ -59,10 +58,6 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     static constexpr int THREADS32 = 1024;
     static constexpr int MINB = (sizeof(real) == 8 ? THREADS64 : THREADS32) / NT;
     static constexpr int PHI_NPT = 2;   // nodes per thread in K_phi (1: 0.427 ms, 2: 0.378, 4: 0.447 on config 4 fp64)
-    // the single-launch step (k_step.cuh) needs tiles of one layer of the slow axis
-    static constexpr bool STEP_OK = T::BZ == 1 && (D == 3 || T::BY == 1);
-    static constexpr int STEP_BM = D == 3 ? T::BY : 1;
-
     static Fields fields(const lbm_ctx *c, int in, int out, int phi_new, int phi_old) {
         Fields F{};
         F.f_in = wsp<sreal>(c, c->L.off_f[in]);  F.f_out = wsp<sreal>(c, c->L.off_f[out]);
@@ -115,36 +110,6 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
             <<<grid_for<T>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F);
         c->launches++;
         CK(cudaGetLastError());
-        return LBM_OK;
-    }
-
-    // the whole step in one launch (k_step.cuh); the buffers flip
-    template <int MODE, bool POPS_SMEM, bool STAGE_G = POPS_SMEM> static int launch_step_kernel(lbm_ctx *c, const Fields &F, int pnew) {
-        if constexpr (STEP_OK) {
-            using CS = SmemCfg<LF, LG, LS, sreal, preal, T::BX, D == 3 ? T::BY : 1, 1, STAGE_G>;
-            using CP = PhiTileSmem<preal, PhiTileCfg<preal, D, T::BX, D == 3 ? T::BY : 1, 1>>;
-            constexpr size_t BYTES = POPS_SMEM ? CS::BYTES : CP::BYTES;
-            auto kern = k_step<LF, LG, LS, real, MODE, T::BX, STEP_BM, MINB, POPS_SMEM, STAGE_G, Fields>;
-            int rc = set_smem_attrs(c, kern, BYTES, c->attr_done[4 + MODE + (STAGE_G ? 0 : 2)]);
-            if (rc) return rc;
-            kern<<<c->sweep.total, NT, BYTES, c->stream>>>(dev_params<real>(c), F, wsp<preal>(c, c->L.off_phi[pnew]),
-                                                           c->map_phi_tile[pnew], c->sweep);
-            c->launches++;
-            CK(cudaGetLastError());
-            return LBM_OK;
-        } else {
-            return LBM_E_UNSUPPORTED;
-        }
-    }
-    static int launch_step(lbm_ctx *c, bool macro) {
-        const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
-        Fields F = fields(c, in, out, pnew, pold);
-        int rc;
-        if (c->pops_smem && (c->sweep.xflags & 1)) rc = macro ? launch_step_kernel<MODE_STEP_MACRO, true, false>(c, F, pnew) : launch_step_kernel<MODE_STEP, true, false>(c, F, pnew);
-        else if (c->pops_smem) rc = macro ? launch_step_kernel<MODE_STEP_MACRO, true>(c, F, pnew) : launch_step_kernel<MODE_STEP, true>(c, F, pnew);
-        else rc = macro ? launch_step_kernel<MODE_STEP_MACRO, false>(c, F, pnew) : launch_step_kernel<MODE_STEP, false>(c, F, pnew);
-        if (rc) return rc;
-        c->cur = out; c->curphi = pnew; c->nsteps++;
         return LBM_OK;
     }
 
@@ -218,18 +183,11 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
             for (auto &e : e3) CK(cudaEventCreate(&e));
             CK(cudaEventRecord(e3[0], c->stream));
         }
-        int rc;
-        if (c->one_launch) {
-            if (timed) CK(cudaEventRecord(e3[1], c->stream));
-            rc = launch_step(c, macro);
-            if (rc) return rc;
-        } else {
-            rc = launch_phi(c);
-            if (rc) return rc;
-            if (timed) CK(cudaEventRecord(e3[1], c->stream));
-            rc = launch_collide(c, macro);
-            if (rc) return rc;
-        }
+        int rc = launch_phi(c);
+        if (rc) return rc;
+        if (timed) CK(cudaEventRecord(e3[1], c->stream));
+        rc = launch_collide(c, macro);
+        if (rc) return rc;
         if (timed) {
             CK(cudaEventRecord(e3[2], c->stream));
             for (auto e : e3) c->ev.push_back(e);
@@ -325,8 +283,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     }
 
     static const ImplOps *ops() {
-        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::step_phase, &Impl::read_macro, &Impl::read_pops, T::BX, T::BY, T::BZ,
-                                  STEP_OK ? STEP_BM : 0};
+        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::step_phase, &Impl::read_macro, &Impl::read_pops, T::BX, T::BY, T::BZ};
         return &o;
     }
 };

@@ -4,20 +4,13 @@
 // The padded phi array has materialised ghost layers and a 16-byte x offset (xpad), so the box
 // [x0 - EPB, x0 + BX + EPB) x [y0 - 1, y0 + BY] x [z0 - 1, z0 + BZ] always starts 16-byte aligned and never needs wrap logic.
 //
-// The tile bodies are device functions taking the tile origin and a `ready` hook that runs after the tile's independent loads
-// have been issued and before the phi box is requested: a no-op when K_phi is its own launch (the kernels below), the wait for
-// the producing K_phi items when both run in one launch (k_step.cuh).
+// The tile bodies are device functions taking the tile origin, so that other kernels can run a tile at a place of their own.
 #pragma once
 
 #include "k_main.cuh"
 #include "ptx.cuh"
 
 namespace lbm {
-
-struct NoWait {
-    static constexpr bool WAITS = false;
-    __device__ __forceinline__ void operator()() const {}
-};
 
 template <class real, int D, int BX, int BY, int BZ> struct PhiTileCfg {
     static constexpr int EPB = 16 / (int)sizeof(real);
@@ -60,9 +53,9 @@ template <class preal, class TC> struct PhiTileSmem {
 };
 
 // one tile of BX x BY x BZ nodes with origin (x0, y0, z0); smem_raw: PhiTileSmem::BYTES bytes, 128-byte aligned
-template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, class Fields, class Ready>
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, class Fields>
 __device__ __forceinline__ void main_tile_phitma(const DevParams<real> &P, const Fields &Fd, const CUtensorMap *phi_map,
-                                                 unsigned char *smem_raw, int x0, int y0, int z0, const Ready &ready) {
+                                                 unsigned char *smem_raw, int x0, int y0, int z0) {
     using preal = typename Fields::preal;
     using TC = PhiTileCfg<preal, LF::D, BX, BY, BZ>;
     using SM = PhiTileSmem<preal, TC>;
@@ -75,23 +68,9 @@ __device__ __forceinline__ void main_tile_phitma(const DevParams<real> &P, const
         mbar_init(bar_a, 1);
         fence_mbar_init();
         fence_proxy_async();
-        if constexpr (!Ready::WAITS) {
-            mbar_expect_tx(bar_a, TC::BYTES);
-            // padded coordinates of node (x0 - EPB, y0 - 1, z0 - 1): (x0, y0, z0 + pz - 1)
-            tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
-        }
-    }
-    if constexpr (Ready::WAITS) {
-        // single-launch step (k_step.cuh): warp 0 waits for the producers of phi^{n+1} in the box, then requests it
-        if (t < 32) {
-            ready();
-            __syncwarp();
-            if (t == 0) {
-                fence_proxy_async_global();   // the acquired generic-proxy writes of phi^{n+1} before the async-proxy read
-                mbar_expect_tx(bar_a, TC::BYTES);
-                tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
-            }
-        }
+        mbar_expect_tx(bar_a, TC::BYTES);
+        // padded coordinates of node (x0 - EPB, y0 - 1, z0 - 1): (x0, y0, z0 + pz - 1)
+        tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
     }
     __syncthreads();   // the barrier is initialised before anybody waits on it
     const int x = x0 + tx, y = y0 + ty, z = z0 + tz;
@@ -113,7 +92,7 @@ k_main_phitma(const DevParams<real> P, const Fields Fd, const __grid_constant__ 
     using SM = PhiTileSmem<preal, PhiTileCfg<preal, LF::D, BX, BY, BZ>>;
     __shared__ __align__(128) unsigned char smem_raw[SM::BYTES];
     main_tile_phitma<LF, LG, LS, real, MODE, BX, BY, BZ>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, blockIdx.y * BY,
-                                                          blockIdx.z * BZ, NoWait{});
+                                                          blockIdx.z * BZ);
 }
 
 }  // namespace lbm

@@ -17,8 +17,7 @@ template <class L, int I> __device__ __forceinline__ unsigned pull_offset(unsign
 }
 
 // shared-memory carve-up of one CTA of NT threads
-// STAGE_G: g is read once (at its collision), so staging it only buys the early issue -- which is what the single-launch step
-// wants (k_step.cuh: the g lines K_phi has just pulled are re-read while they are still in L2).
+// STAGE_G: g is read once (at its collision), so staging it only buys the early issue (measured: no gain; off).
 template <class LF, class LG, class LS, class sreal, class preal, int BX, int BY, int BZ, bool STAGE_G_ = false> struct SmemCfg {
     using TC = PhiTileCfg<preal, LF::D, BX, BY, BZ>;
     static constexpr int NT = BX * BY * BZ;
@@ -90,9 +89,9 @@ template <class LF, class LG, class LS, class real, class C, class Fields> struc
 };
 
 // one tile of BX x BY x BZ nodes with origin (x0, y0, z0); smem_raw: SmemCfg::BYTES bytes of dynamic shared memory
-template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, bool STAGE_G = false, class Fields, class Ready>
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, bool STAGE_G = false, class Fields>
 __device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const Fields &Fd, const CUtensorMap *phi_map,
-                                               unsigned char *smem_raw, int x0, int y0, int z0, const Ready &ready) {
+                                               unsigned char *smem_raw, int x0, int y0, int z0) {
     using sreal = typename Fields::sreal;
     using preal = typename Fields::preal;
     using C = SmemCfg<LF, LG, LS, sreal, preal, BX, BY, BZ, STAGE_G>;
@@ -108,23 +107,8 @@ __device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const F
         mbar_init(bar_a, 1);
         fence_mbar_init();
         fence_proxy_async();
-        if constexpr (!Ready::WAITS) {
-            mbar_expect_tx(bar_a, TC::BYTES);
-            tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
-        }
-    }
-    if constexpr (Ready::WAITS) {
-        // single-launch step (k_step.cuh): warp 0 waits for the producers of phi^{n+1} in the box BEFORE it issues its own
-        // population copies (the polls would queue behind them), then requests the box; the other warps go straight on
-        if (t < 32) {
-            ready();
-            __syncwarp();
-            if (t == 0) {
-                fence_proxy_async_global();   // the acquired generic-proxy writes of phi^{n+1} before the async-proxy read
-                mbar_expect_tx(bar_a, TC::BYTES);
-                tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
-            }
-        }
+        mbar_expect_tx(bar_a, TC::BYTES);
+        tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
     }
     const int x = x0 + tx, y = y0 + ty, z = z0 + tz;
     const bool active = x < P.nx && y < P.ny && z < P.nz;
@@ -134,7 +118,7 @@ __device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const F
         g = make_geom(P, x, y, z);
         if (!bc) {
             const SrcSmem<LF, LG, LS, real, C, Fields> src(P, Fd, g, tile, phiold, pops, bar_a, t, tx, ty, tz);
-            src.prefetch();   // before the barrier below: the copies fly while the CTA assembles (and while `ready` waits)
+            src.prefetch();   // before the barrier below: the copies fly while the CTA assembles
         }
     }
     __syncthreads();   // the mbarrier is initialised before anybody waits on it
@@ -153,7 +137,7 @@ __global__ void __launch_bounds__(BX *BY *BZ, MINB)
 k_main_smem(const DevParams<real> P, const Fields Fd, const __grid_constant__ CUtensorMap phi_map) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     main_tile_smem<LF, LG, LS, real, MODE, BX, BY, BZ>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, blockIdx.y * BY,
-                                                        blockIdx.z * BZ, NoWait{});
+                                                        blockIdx.z * BZ);
 }
 
 }  // namespace lbm

@@ -91,38 +91,6 @@ template <class sreal_, class preal_> struct DevFieldsT {
 };
 template <class real> using DevFields = DevFieldsT<real, real>;   // one type throughout (fp64)
 
-// n / d for n < 2^31 by one multiplication: q = (n * m) >> s with s = 31 + ceil(log2 d), m = ceil(2^s / d) < 2^32
-struct FastDiv {
-    unsigned m;
-    int s;
-    unsigned d;
-    __host__ __device__ __forceinline__ unsigned div(unsigned n) const { return (unsigned)(((unsigned long long)n * m) >> s); }
-};
-
-// Host-computed description of the sweep of the single-launch step (lbm.cu make_sweep_plan, k_step.cuh); passed by value.
-// The launch is a logical 3D grid (gx, gy, J), x fastest: z = block of the mid axis, y = position k along the slow axis,
-// x = item within group k: first cPmax slots for the P items of pair position k, then cMmax slots for the M items of
-// pair k - head.  Slots beyond what a block class or the ends of the sweep need exit at once.
-struct SweepPlan {
-    int nmid, nslow;        // extents of the mid axis (ny in 3D, 1 in 2D) and of the slow axis (nz in 3D, ny in 2D)
-    int NP;                 // layer pairs: ceil(nslow / 2)
-    int J, By;              // blocks of the mid axis (the last one takes the remainder), rows per block
-    int xt;                 // x tiles per row
-    int head;               // lead of P over M in pair positions (>= 2: the pair after the one M works on must be done)
-    int prows[3];           // rows of the P window per block class (0 first, 1 middle, 2 last)
-    int ptiles[3], mtiles[3];   // row tiles per slice: P items cover 2 BM window rows (x 2 layers), M items BM rows (x 1 layer)
-    int cP[3];              // P items per slice = ptiles * xt: what the slice counter reaches per step
-    int cPmax, mtmax;       // slots per group: cPmax for P, 2 * mtmax * xt for M
-    FastDiv d_gx, d_gy, d_xt;
-    unsigned total;         // gx * gy * J
-    int ticketed;           // 1: CTAs take their place in the order from the global ticket; 0: from blockIdx.x
-    int xflags;             // EXPERIMENT switches
-    unsigned long long *ticket;      // device: (epoch << 32) | next ticket of the launch
-    unsigned long long *done;        // device: [J][NP] finished P items per slice, running on over the steps
-    unsigned long long *left;        // device (blockIdx order): CTAs of all launches that have arrived and read this counter
-    int *err;                        // device: set when a wait gave up (never in a correct run)
-};
-
 // ---- per-node geometry ------------------------------------------------------------------------------------
 // Element offsets are 32-bit: Q * N < 2^32 is checked by the host (lbm_create).
 struct NodeGeom {

@@ -24,7 +24,6 @@ namespace {
 using namespace lbm;
 
 constexpr size_t ALIGN = 256;
-constexpr int SWEEP_MIN_ROWS = 4;   // smallest mid-axis block of the single-launch step
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 int lattice_q(int id) {
@@ -109,13 +108,6 @@ Layout make_layout(const lbm_params *p) {
     L.off_p = take(N, es);
     L.off_T = take(N, es);
     L.off_scratch = take(N, es);
-    // single-launch step (k_step.cuh): ticket + error flag + one counter per (mid block, layer pair) slice, at least
-    // SWEEP_MIN_ROWS rows per block
-    {
-        const size_t nmid = p->nz > 1 ? (size_t)p->ny : 1, nslow = p->nz > 1 ? (size_t)p->nz : (size_t)p->ny;
-        L.sync_bytes = 8 * (4 + (nmid / SWEEP_MIN_ROWS + 1) * ((nslow + 1) / 2));
-        L.off_sync = take(L.sync_bytes, 1);
-    }
     L.total = o;
     return L;
 }
@@ -216,67 +208,6 @@ bool build_phi_tile_maps(lbm_ctx *c) {
 
 // Order of the work items of the single-launch step (k_step.cuh): rows per mid-axis block and lead of K_phi over K_main in
 // layer pairs; 0 / negative = the defaults chosen by measurement.
-FastDiv fast_div(unsigned d) {
-    FastDiv f;
-    int k = 0;
-    while ((1ull << k) < d) ++k;
-    f.s = 31 + k;
-    f.m = (unsigned)(((1ull << f.s) + d - 1) / d);
-    f.d = d;
-    return f;
-}
-
-bool make_sweep_plan(lbm_ctx *c, int rows_per_block, int lead) {
-    SweepPlan &S = c->sweep;
-    const int bm = c->ops->step_bm;
-    if (bm <= 0) return false;
-    const bool three_d = c->P.nz > 1;
-    S.nmid = three_d ? c->P.ny : 1;
-    S.nslow = three_d ? c->P.nz : c->P.ny;
-    S.NP = (S.nslow + 1) / 2;
-    S.xt = (c->P.nx + c->ops->bx - 1) / c->ops->bx;
-    S.xflags = lead >= 0 ? lead >> 8 : 0;
-    if (lead >= 0) lead &= 255;
-    S.ticketed = (S.xflags & 2) ? 0 : 1;
-    if (lead < 0) lead = 1;
-    S.head = 2 + lead;
-    // mid-axis blocks: a block should hold about a megabyte of phi and g per layer pair so that the slices K_main works on
-    // while K_phi runs ahead stay in L2; multiples of the P item height, at least SWEEP_MIN_ROWS rows
-    int By = rows_per_block > 0 ? rows_per_block : 32;
-    By = (By + 2 * bm - 1) / (2 * bm) * (2 * bm);
-    if (By < SWEEP_MIN_ROWS) By = (SWEEP_MIN_ROWS + 2 * bm - 1) / (2 * bm) * (2 * bm);
-    int J = S.nmid / By;
-    if (J < 2) { J = 1; By = S.nmid > 0 ? S.nmid : 1; }
-    S.J = J; S.By = By;
-    const int last_rows = S.nmid - (J - 1) * By;
-    int mrows[3];
-    if (J == 1) { mrows[0] = S.nmid; S.prows[0] = S.nmid; }
-    else { mrows[0] = By; S.prows[0] = By + 2; }
-    mrows[1] = By; S.prows[1] = By;
-    mrows[2] = last_rows; S.prows[2] = last_rows - 2;
-    S.cPmax = 0; S.mtmax = 0;
-    for (int k = 0; k < 3; ++k) {
-        const bool used = k == 0 || (k == 1 && J > 2) || (k == 2 && J > 1);
-        S.ptiles[k] = used ? (S.prows[k] + 2 * bm - 1) / (2 * bm) : 0;
-        S.mtiles[k] = used ? (mrows[k] + bm - 1) / bm : 0;
-        S.cP[k] = S.ptiles[k] * S.xt;
-        if (S.cP[k] > S.cPmax) S.cPmax = S.cP[k];
-        if (S.mtiles[k] > S.mtmax) S.mtmax = S.mtiles[k];
-    }
-    const unsigned long long gx = (unsigned long long)S.cPmax + 2ull * S.mtmax * S.xt, gy = (unsigned long long)S.NP + S.head;
-    const unsigned long long total = gx * gy * (unsigned long long)J;
-    if (total >= (1ull << 31) || gx * gy >= (1ull << 31)) return false;
-    S.d_gx = fast_div((unsigned)gx); S.d_gy = fast_div((unsigned)gy); S.d_xt = fast_div((unsigned)S.xt);
-    S.total = (unsigned)total;
-    if ((size_t)8 * (4 + (size_t)J * S.NP) > c->L.sync_bytes) return false;
-    unsigned long long *base = reinterpret_cast<unsigned long long *>(c->ws + c->L.off_sync);
-    S.ticket = base;
-    S.left = base + 1;
-    S.err = reinterpret_cast<int *>(base + 2);
-    S.done = base + 4;
-    return true;
-}
-
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------ C ABI
@@ -335,10 +266,6 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         // fp64 (+3..9% on every large grid) and fp32 in 2D (+8%); fp32 3D stays on the register gather (-1..5%)
         const bool smem_default = p->precision == 64 || p->nz == 1;
         c->pops_smem = c->phi_tma && ((fl & LBM_FLAG_POPS_STAGED) ? true : (fl & LBM_FLAG_POPS_GATHER) ? false : smem_default);
-        // one launch per step (k_step.cuh) where the tile shape allows it; slabs need the two phases, the prescribed-velocity
-        // mode runs the plain kernel
-        c->one_launch = c->phi_tma && !(fl & LBM_FLAG_TWO_LAUNCHES) && !(p->halo[0] | p->halo[1]) &&
-                        !(fl & LBM_FLAG_PRESCRIBED_U) && make_sweep_plan(c, 0, -1);
     }
     *out = c;
     return LBM_OK;
@@ -346,17 +273,7 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
 
 int lbm_init(lbm_ctx *c, const void *h_phi, const void *h_T, const void *h_u, const void *h_p) {
     if (!c || !h_phi) return LBM_E_INVALID;
-    CK(cudaMemsetAsync(c->ws + c->L.off_sync, 0, c->L.sync_bytes, c->stream));   // ticket, error flag, slice counters
     return c->ops->init(c, h_phi, h_T, h_u, h_p);
-}
-
-int lbm_set_sweep(lbm_ctx *c, int rows_per_block, int lead) {
-    if (!c) return LBM_E_INVALID;
-    if (!c->one_launch) return LBM_E_STATE;
-    CK(cudaStreamSynchronize(c->stream));
-    if (!make_sweep_plan(c, rows_per_block, lead)) return LBM_E_INVALID;
-    CK(cudaMemsetAsync(c->ws + c->L.off_sync, 0, c->L.sync_bytes, c->stream));
-    return LBM_OK;
 }
 
 int lbm_set_velocity(lbm_ctx *c, const void *h_u) {
@@ -398,11 +315,6 @@ int lbm_read_pops(lbm_ctx *c, int which, int stage, void *h_pops) {
 int lbm_sync(lbm_ctx *c) {
     if (!c) return LBM_E_INVALID;
     CK(cudaStreamSynchronize(c->stream));
-    if (c->one_launch) {   // the hand-over inside the single-launch step gave up waiting (never in a correct run)
-        int err = 0;
-        CK(cudaMemcpy(&err, c->sweep.err, sizeof(int), cudaMemcpyDeviceToHost));
-        if (err) return LBM_E_HANDOVER;
-    }
     return LBM_OK;
 }
 
@@ -435,7 +347,6 @@ long long lbm_step_count(const lbm_ctx *c) { return c ? c->nsteps : -1; }
 long long lbm_launch_count(const lbm_ctx *c) { return c ? c->launches : -1; }
 const char *lbm_variant(const lbm_ctx *c) {
     if (!c) return "";
-    if (c->one_launch) return c->pops_smem ? "one-launch gather+smem" : "one-launch gather+phi-tma";
     return c->phi_tma ? (c->pops_smem ? "gather+smem" : "gather+phi-tma") : "direct";
 }
 int lbm_last_cuda_error(void) { return g_last_cuda_error; }
@@ -449,7 +360,6 @@ const char *lbm_strerror(int code) {
     case LBM_E_CUDA: return "CUDA runtime error (see lbm_last_cuda_error)";
     case LBM_E_STATE: return "call not valid in this state";
     case LBM_E_NODEVICE: return "no sm_100 CUDA device";
-    case LBM_E_HANDOVER: return "hand-over inside the single-launch step timed out";
     default: return "unknown error";
     }
 }

@@ -111,7 +111,7 @@ def test_3d_periodic_ragged(gpu, oracle_mod):
 def test_3d_mid_tiles(gpu, oracle_mod):
     """Rows that are a multiple of 64 but not worth a 128-wide tile (192, 320; here 64 and 192) run 64 x 2 tiles in fp64 3D."""
     P = wl.base_params(64, 7, 5, grav=[1e-4, -1e-4, -2e-4])
-    sim = gpu.LBM(P, 64); assert sim.variant == "one-launch gather+smem"; sim.destroy()
+    sim = gpu.LBM(P, 64); assert sim.variant == "gather+smem"; sim.destroy()
     _run_parity(gpu, oracle_mod, P, _random_state(P, 61), [1, 12], label="3d 64-wide periodic")
     P = wl.base_params(192, 5, 6, grav=[0.0, 0.0, -1e-4], lat_f="D3Q15")
     P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
@@ -215,9 +215,8 @@ def _with_kernels(P, *names):
 
 def test_kernel_variants(gpu, oracle_mod):
     """The step by how it is launched and what K_main stages in shared memory (include/lbm.h "Kernel selection").
-    Defaults: one launch per step (k_step.cuh) on tiles of one layer, "gather+smem" (phi halo tile by one TMA box per CTA,
-    the node's populations, phi^n, Pdot by per-thread cp.async) in fp64 and fp32 2D, "gather+phi-tma" (populations gathered
-    into registers) in fp32 3D.  The flags force the plainer kernels.  Every one must match the oracle on periodic and
+    Defaults: "gather+smem" (phi halo tile by one TMA box per CTA, the node's populations, phi^n, Pdot by per-thread
+    cp.async) in fp64 and fp32 2D, "gather+phi-tma" (populations gathered into registers) in fp32 3D.  The flags force the plainer kernels.  Every one must match the oracle on periodic and
     walled, 2D and 3D, narrow- and wide-tile grids (the other tests in this file run the defaults)."""
     P3 = wl.base_params(40, 10, 7, grav=[1e-4, 0.0, -2e-4])                     # narrow tiles, ragged
     P3w = wl.base_params(256, 6, 5, grav=[1e-4, 0.0, -2e-4], force=[0.0, 1e-5, 0.0])   # wide tiles, two per row
@@ -230,69 +229,24 @@ def test_kernel_variants(gpu, oracle_mod):
     P3z["bc_T"][2] = [1.0, 0.0]
     cases = ((P3, 34), (P3w, 44), (P2, 35), (P2w, 45), (P3z, 46))
     # (flags, variant of the wide 3D case in fp64, in fp32)
-    for names, want64, want32 in (((), "one-launch gather+smem", "one-launch gather+phi-tma"),
-                                  (("two_launches",), "gather+smem", "gather+phi-tma"),
-                                  (("pops_gather",), "one-launch gather+phi-tma", "one-launch gather+phi-tma"),
-                                  (("pops_staged",), "one-launch gather+smem", "one-launch gather+smem"),
-                                  (("two_launches", "pops_gather"), "gather+phi-tma", "gather+phi-tma"),
+    for names, want64, want32 in (((), "gather+smem", "gather+phi-tma"),
+                                  (("pops_gather",), "gather+phi-tma", "gather+phi-tma"),
+                                  (("pops_staged",), "gather+smem", "gather+smem"),
                                   (("phi_ldg",), "direct", "direct")):
         sim = gpu.LBM(_with_kernels(P3w, *names), 64); assert sim.variant == want64, (names, sim.variant); sim.destroy()
         sim = gpu.LBM(_with_kernels(P3w, *names), 32); assert sim.variant == want32, (names, sim.variant); sim.destroy()
         for P, seed in cases:
             _run_parity(gpu, oracle_mod, _with_kernels(P, *names), _random_state(P, seed), [1, 12],
                         label="%s %dx%dx%d" % (names, P["nx"], P["ny"], P["nz"]))
-    # narrow tiles span two layers: two launches whatever the flags
-    sim = gpu.LBM(P3, 64); assert sim.variant == "gather+smem", sim.variant; sim.destroy()
     # fp32 with the staged kernel (3D opt-in, 2D default): inside the fp32 bar
     for P, seed in ((P3w, 44), (P2w, 45)):
-        for names in (("pops_staged",), ("pops_staged", "two_launches")):
-            init = _random_state(P, seed)
-            o = oracle_mod.Oracle(P); o.init(*init); o.step(12)
-            sim = gpu.LBM(_with_kernels(P, *names), 32); sim.init(*[a.astype(np.float32) for a in init]); sim.step(12)
-            assert sim.variant.endswith("gather+smem")
-            for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
-                assert _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30) <= REL32, name
-            sim.destroy(); o.close()
-
-
-def test_one_launch_step_sweep_orders(gpu, oracle_mod):
-    """The single-launch step (k_step.cuh) must give the same result whatever the order of its work items: mid-axis blocks of
-    4..16 rows (several blocks, ragged last block, the shifted K_phi windows), leads 0..3, odd and even numbers of layers,
-    periodic and walled slow / mid axes.  Every order gives the same bits (same kernel, same arithmetic per node); the
-    two-launch step (other instantiations: the compiler contracts differently) agrees to rounding, the oracle within 1e-10."""
-    cases = []
-    P = wl.base_params(250, 37, 9, grav=[1e-4, -1e-4, -2e-4], force=[1e-5, 0.0, 2e-5])     # wide tiles, ragged x, odd nz
-    cases.append((P, 81))
-    P = wl.base_params(128, 22, 8, grav=[0.0, 0.0, -1e-4])                                  # y and z walls
-    for a in (1, 2):
-        P["bc_f"][a] = ["wall", "wall"]; P["bc_g"][a] = ["zeroflux", "dirichlet" if a == 1 else "zeroflux"]
-        P["bc_s"][a] = ["dirichlet", "dirichlet"]; P["bc_T"][a] = [1.0, 0.0]; P["bc_phi"][a] = [0.0, 1.0]
-    cases.append((P, 82))
-    P = wl.base_params(64, 26, 7, grav=[1e-4, 0.0, -2e-4])                                  # 64 x 2 tiles
-    cases.append((P, 83))
-    P = wl.base_params(256, 19, 1, grav=[1e-4, -1e-4, 0.0])                                 # 2D: the slow axis is y
-    cases.append((P, 84))
-    for P, seed in cases:
         init = _random_state(P, seed)
-        o = oracle_mod.Oracle(P); o.init(*init); o.step(9)
-        ref = gpu.LBM(_with_kernels(P, "two_launches"), 64); ref.init(*init); ref.step(9)
-        want = ref.read_macro() + tuple(ref.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
-        ref.destroy()
-        first = None
-        for rows, lead in ((0, -1), (4, 0), (4, 3), (6, 1), (8, 2), (16, 1), (1000, 0)):
-            sim = gpu.LBM(P, 64)
-            assert sim.variant.startswith("one-launch")
-            sim.set_sweep(rows, lead)
-            sim.init(*init); sim.step(4); sim.step(5)
-            sim.sync()
-            got = sim.read_macro() + tuple(sim.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
-            first = first or got
-            for a, b, w in zip(got, first, want):
-                assert np.array_equal(a, b), (P["nx"], P["ny"], P["nz"], rows, lead, _maxabs(a, b))
-                assert _maxabs(a, w) <= 1e-13, (P["nx"], P["ny"], P["nz"], rows, lead, _maxabs(a, w))
-            _compare_state(gpu, sim, o, oracle_mod, TOL64, True, "one launch rows %d lead %d" % (rows, lead))
-            sim.destroy()
-        o.close()
+        o = oracle_mod.Oracle(P); o.init(*init); o.step(12)
+        sim = gpu.LBM(_with_kernels(P, "pops_staged"), 32); sim.init(*[a.astype(np.float32) for a in init]); sim.step(12)
+        assert sim.variant == "gather+smem"
+        for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
+            assert _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30) <= REL32, name
+        sim.destroy(); o.close()
 
 
 def test_cuda_graph_replay_on_side_stream(gpu, oracle_mod):
@@ -336,7 +290,7 @@ def test_d3q15_lattice_set(gpu, oracle_mod):
     _run_parity(gpu, oracle_mod, Pc, (I["phi"], I["T"]), [1, 100], pops=False, label="D3Q15 config4 48x40x64")
 
 
-@pytest.mark.parametrize("names", [("phi_ldg",), ("two_launches",), ("pops_gather",)])
+@pytest.mark.parametrize("names", [("phi_ldg",), ("pops_gather",)])
 def test_d3q15_variants(gpu, oracle_mod, names):
     P1, P2, _ = _d3q15_cases()
     _run_parity(gpu, oracle_mod, _with_kernels(P1, *names), _random_state(P1, 74), [1, 8], label="D3Q15 periodic %s" % (names,))
