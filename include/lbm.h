@@ -71,7 +71,8 @@ enum {
     LBM_E_WORKSPACE = -3, /* workspace too small or misaligned                             */
     LBM_E_CUDA = -4,      /* a CUDA runtime call failed (lbm_last_cuda_error for the code) */
     LBM_E_STATE = -5,     /* call not valid in this state (e.g. step before init)          */
-    LBM_E_NODEVICE = -6   /* no sm_100 device / kernels not loadable                       */
+    LBM_E_NODEVICE = -6,  /* no sm_100 device / kernels not loadable                       */
+    LBM_E_TOOLARGE = -7   /* lbm_read_pops_noalloc: the lattice does not fit the static scratch array */
 };
 
 /* which-population selectors and stages of lbm_read_pops */
@@ -185,6 +186,21 @@ int lbm_read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T);
 /* Debug / parity access: copy populations [Q][z][y][x] of lattice `which` at `stage` to HOST.  Synchronises.
  * Not on the hot path. */
 int lbm_read_pops(lbm_ctx *c, int which, int stage, void *h_pops);
+
+/* lbm_read_pops for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc).  lbm_read_pops stages the streamed populations (LBM_STAGE_STREAMED: the pull of PAPER.md:175 with the
+ * boundary rules of PAPER.md:285, 418 applied) in a temporary from cudaMalloc; this call stages them in a file-scope
+ * static __device__ array of LBM_NOALLOC_SCRATCH_BYTES bytes instead and calls no cudaMalloc, cudaFree or allocating
+ * library routine.  Same arguments, same result.  Limits and sharing:
+ *   - Q * nx * ny * nz * sizeof(element) of lattice `which` must be <= LBM_NOALLOC_SCRATCH_BYTES, else LBM_E_TOOLARGE
+ *     (e.g. D3Q19 in double: 55 188 nodes, 38^3; D2Q9 in double: 116 508 nodes, 341^2);
+ *   - every GPU that loads the library holds the array until the process exits;
+ *   - ALL contexts of a device share the one array, which keeps the last call's contents.  The call overwrites the part it
+ *     reads back (nothing has to start at zero) and returns after its own copy has finished, but two calls that overlap on
+ *     the GPU (different contexts on different streams or host threads) race: serialise them;
+ *   - the context's device must be current (as for every call); the array's device address is resolved once per device. */
+#define LBM_NOALLOC_SCRATCH_BYTES (8u << 20)
+int lbm_read_pops_noalloc(lbm_ctx *c, int which, int stage, void *h_pops);
 
 /* Block until everything enqueued on the context's stream has finished; returns LBM_E_CUDA on a fault. */
 int lbm_sync(lbm_ctx *c);

@@ -28,8 +28,9 @@ KERNEL_FLAGS = {"pops_gather": FLAG_POPS_GATHER, "pops_staged": FLAG_POPS_STAGED
 POPS_F, POPS_G, POPS_S = 0, 1, 2
 STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1
+NOALLOC_SCRATCH_BYTES = 8 << 20
 
-EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops",
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
            "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
@@ -80,6 +81,7 @@ def load_library():
         L.lbm_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_read_macro.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.lbm_read_pops_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_sync.argtypes = [C.c_void_p]
         L.lbm_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.lbm_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
@@ -248,6 +250,12 @@ class LBM:
     def read_pops(self, which: int, stage: int = STAGE_STREAMED):
         out = np.empty((self.Q[which],) + self.shape, self.dtype)
         _check(self._L.lbm_read_pops(self._h, int(which), int(stage), C.c_void_p(out.ctypes.data)), "lbm_read_pops")
+        return out
+
+    def read_pops_noalloc(self, which: int, stage: int = STAGE_STREAMED):
+        """read_pops without any device allocation (static scratch of NOALLOC_SCRATCH_BYTES; include/lbm.h)."""
+        out = np.empty((self.Q[which],) + self.shape, self.dtype)
+        _check(self._L.lbm_read_pops_noalloc(self._h, int(which), int(stage), C.c_void_p(out.ctypes.data)), "lbm_read_pops_noalloc")
         return out
 
     def sync(self):

@@ -38,6 +38,7 @@ struct ImplOps {
     int (*step_phase)(lbm_ctx *, int, int);
     int (*read_macro)(lbm_ctx *, void *, void *, void *, void *);
     int (*read_pops)(lbm_ctx *, int, int, void *);
+    int (*read_pops_scratch)(lbm_ctx *, int, int, void *, void *, size_t);   // staged in a caller-given device scratch (noalloc.cu)
     int bx, by, bz;   // tile of nodes per CTA
 };
 

@@ -282,8 +282,32 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         return LBM_E_INVALID;
     }
 
+    // lbm_read_pops_noalloc (noalloc.cu): the streamed populations staged in d_tmp (`cap` bytes, device memory that is not part
+    // of the workspace) instead of a temporary from cudaMalloc.  Allocates nothing.
+    template <class L> static int read_pops_scratch_one(lbm_ctx *c, int which, const size_t (&off)[2], void *h, void *d_tmp, size_t cap) {
+        const size_t N = (size_t)c->L.N, bytes = (size_t)L::Q * N * sizeof(sreal);
+        if (bytes > cap) return LBM_E_TOOLARGE;
+        if (c->nsteps < 1) return LBM_E_STATE;
+        sreal *tmp = static_cast<sreal *>(d_tmp);
+        k_stream_only<L, real, TP::BX, TP::BY, TP::BZ><<<grid_for<TP>(c->P), NTP, 0, c->stream>>>(
+            dev_params<real>(c), (const sreal *)wsp<sreal>(c, off[1 - c->cur]), tmp, which,
+            which == LBM_POPS_G ? (const sreal *)wsp<sreal>(c, c->L.off_pdot[1 - c->cur]) : (const sreal *)nullptr);
+        c->launches++;
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(h, tmp, bytes, cudaMemcpyDefault, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        return LBM_OK;
+    }
+    static int read_pops_scratch(lbm_ctx *c, int which, int stage, void *h, void *d_tmp, size_t cap) {
+        if (stage == LBM_STAGE_POSTCOLLISION) return read_pops(c, which, stage, h);   // that stage never allocated
+        if (which == LBM_POPS_F) return read_pops_scratch_one<LF>(c, which, c->L.off_f, h, d_tmp, cap);
+        if (which == LBM_POPS_G) return read_pops_scratch_one<LG>(c, which, c->L.off_g, h, d_tmp, cap);
+        if (which == LBM_POPS_S) return read_pops_scratch_one<LS>(c, which, c->L.off_s, h, d_tmp, cap);
+        return LBM_E_INVALID;
+    }
+
     static const ImplOps *ops() {
-        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::step_phase, &Impl::read_macro, &Impl::read_pops, T::BX, T::BY, T::BZ};
+        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::step_phase, &Impl::read_macro, &Impl::read_pops, &Impl::read_pops_scratch, T::BX, T::BY, T::BZ};
         return &o;
     }
 };

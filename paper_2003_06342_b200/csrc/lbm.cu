@@ -360,6 +360,7 @@ const char *lbm_strerror(int code) {
     case LBM_E_CUDA: return "CUDA runtime error (see lbm_last_cuda_error)";
     case LBM_E_STATE: return "call not valid in this state";
     case LBM_E_NODEVICE: return "no sm_100 CUDA device";
+    case LBM_E_TOOLARGE: return "lattice larger than the static scratch array of the no-alloc entry point (LBM_NOALLOC_SCRATCH_BYTES)";
     default: return "unknown error";
     }
 }
