@@ -73,6 +73,7 @@ struct lbm_ctx {
     bool phi_tma;
     // ... and the pulled populations, phi^n, Pdot staged by per-thread cp.async (k_main_smem.cuh)
     bool pops_smem;
+    bool pdl;   // K_main launched with programmatic stream serialisation behind K_phi
     int attr_done[8];   // kernel attributes set on this context's device: [MODE] K_main
     // CUDA graph of two consecutive plain steps, for launch-bound (small) grids
     bool graph_ok;

@@ -86,6 +86,19 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         return LBM_OK;
     }
 
+    // K_main right behind K_phi in the stream, with programmatic dependent launch (unless LBM_FLAG_NO_PDL): its CTAs may start
+    // while K_phi drains; they wait (griddepcontrol.wait, k_main_*.cuh) before they request their phi box
+    template <class K> static cudaError_t launch_after_phi(lbm_ctx *c, K kern, size_t smem, const DevParams<real> &P, const Fields &F,
+                                                           const CUtensorMap &map) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid_for<T>(c->P); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = c->pdl ? 1 : 0;
+        return cudaLaunchKernelEx(&cfg, kern, P, F, map);
+    }
+
     template <int MODE> static int launch_main(lbm_ctx *c, const Fields &F, int pnew = 0) {
         if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU) {
             if (c->phi_tma && c->pops_smem) {
@@ -93,16 +106,14 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
                 auto kern = k_main_smem<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB, Fields>;
                 int rc = set_smem_attrs(c, kern, C::BYTES, c->attr_done[MODE]);
                 if (rc) return rc;
-                kern<<<grid_for<T>(c->P), NT, C::BYTES, c->stream>>>(dev_params<real>(c), F, c->map_phi_tile[pnew]);
+                CK(launch_after_phi(c, kern, C::BYTES, dev_params<real>(c), F, c->map_phi_tile[pnew]));
                 c->launches++;
-                CK(cudaGetLastError());
                 return LBM_OK;
             }
             if (c->phi_tma) {
-                k_main_phitma<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB>
-                    <<<grid_for<T>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F, c->map_phi_tile[pnew]);
+                auto kern = k_main_phitma<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB, Fields>;
+                CK(launch_after_phi(c, kern, 0, dev_params<real>(c), F, c->map_phi_tile[pnew]));
                 c->launches++;
-                CK(cudaGetLastError());
                 return LBM_OK;
             }
         }

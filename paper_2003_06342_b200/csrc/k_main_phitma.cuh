@@ -68,6 +68,7 @@ __device__ __forceinline__ void main_tile_phitma(const DevParams<real> &P, const
         mbar_init(bar_a, 1);
         fence_mbar_init();
         fence_proxy_async();
+        pdl_wait();   // phi^{n+1} is K_phi's output: the only input of this kernel that the preceding launch writes
         mbar_expect_tx(bar_a, TC::BYTES);
         // padded coordinates of node (x0 - EPB, y0 - 1, z0 - 1): (x0, y0, z0 + pz - 1)
         tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);

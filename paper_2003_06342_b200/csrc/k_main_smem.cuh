@@ -107,8 +107,6 @@ __device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const F
         mbar_init(bar_a, 1);
         fence_mbar_init();
         fence_proxy_async();
-        mbar_expect_tx(bar_a, TC::BYTES);
-        tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
     }
     const int x = x0 + tx, y = y0 + ty, z = z0 + tz;
     const bool active = x < P.nx && y < P.ny && z < P.nz;
@@ -120,6 +118,13 @@ __device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const F
             const SrcSmem<LF, LG, LS, real, C, Fields> src(P, Fd, g, tile, phiold, pops, bar_a, t, tx, ty, tz);
             src.prefetch();   // before the barrier below: the copies fly while the CTA assembles
         }
+    }
+    if (t == 0) {
+        // phi^{n+1} is K_phi's output, the only input the preceding launch writes: with programmatic dependent launch this CTA
+        // may be running before K_phi has finished, its population copies (above) already in flight
+        pdl_wait();
+        mbar_expect_tx(bar_a, TC::BYTES);
+        tma_load_3d(smem_u32(tile), phi_map, bar_a, x0, y0, LF::D == 3 ? z0 : 0);
     }
     __syncthreads();   // the mbarrier is initialised before anybody waits on it
     if (!active) return;

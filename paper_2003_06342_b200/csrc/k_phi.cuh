@@ -4,6 +4,7 @@
 #pragma once
 
 #include "kernels.cuh"
+#include "ptx.cuh"
 
 namespace lbm {
 
@@ -91,6 +92,7 @@ __global__ void __launch_bounds__(BX *BY *BZ)
 k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, preal *__restrict__ phi_new) {
     using vreal = typename std::conditional<std::is_same<real, sreal>::value, real, preal>::type;
     constexpr bool ALONG_Z = LG::D == 3;
+    pdl_launch_dependents();   // K_main may start filling the SMs as this grid drains; it waits (griddepcontrol.wait) before it reads phi
     const int t = threadIdx.x;
     const int x0 = blockIdx.x * BX;
     const int y0 = blockIdx.y * BY * (ALONG_Z ? 1 : NPT);

@@ -260,6 +260,7 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         c->graph_ok = c->stream != nullptr && L.N <= (1ll << 21) && !(fl & LBM_FLAG_NO_GRAPH);
         c->graph2 = nullptr; c->graph_launches = 0;
         for (int &a : c->attr_done) a = 0;
+        c->pdl = !(fl & LBM_FLAG_NO_PDL);
         // phi halo tile of K_main: one TMA box per CTA into shared memory (default) or plain loads through L1
         c->phi_tma = !(fl & LBM_FLAG_PHI_LDG) && build_phi_tile_maps(c);
         // pulled populations of K_main: staged in shared memory by cp.async (k_main_smem.cuh) where that measured faster --

@@ -51,4 +51,11 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
+// ---- programmatic dependent launch (PDL) -------------------------------------------------------------------------------
+// launch_dependents: the next kernel of the stream, if it was launched with programmatic stream serialisation, may start once
+// every CTA of this grid has got here (or exited).  wait: blocks until the preceding grid has COMPLETED and its memory is
+// visible; a no-op for a kernel launched the plain way.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 }  // namespace lbm

@@ -36,6 +36,22 @@ def test_sass_is_sm100a(lib):
     assert "sm_100a" in out
 
 
+def test_sass_has_tma_and_async_copies(lib):
+    """The Blackwell-native staging must really be in the shipped binary (B200_PROFILING.md "What proves a Blackwell-native
+    kernel"): UTMALDG = the phi halo box by cp.async.bulk.tensor, SYNCS = its mbarrier, LDGSTS = the per-thread cp.async of the
+    populations.  A regression to plain loads would pass every parity test; this one fails."""
+    sass = os.popen("cuobjdump -sass %s 2>/dev/null" % binding.LIB_PATH).read()
+    assert sass.count("UTMALDG") >= 16 and sass.count("SYNCS.PHASECHK") >= 16 and sass.count("LDGSTS") >= 100
+    # per kernel family: the default K_main of every lattice set and precision carries all three
+    funcs = sass.split("Function : ")[1:]
+    smem = [f for f in funcs if f.startswith("_ZN3lbm11k_main_smem")]
+    assert len(smem) >= 16
+    for f in smem:
+        assert "UTMALDG" in f and "LDGSTS" in f and "SYNCS" in f, f[:200]
+    phitma = [f for f in funcs if f.startswith("_ZN3lbm13k_main_phitma")]
+    assert phitma and all("UTMALDG" in f for f in phitma)
+
+
 def test_workspace_bytes_accounting(lib):
     P, _ = wl.config4_film3d(nx=8, ny=8, nz=8)      # parameters only matter
     P.update(nx=256, ny=256, nz=512)

@@ -232,6 +232,7 @@ def test_kernel_variants(gpu, oracle_mod):
     for names, want64, want32 in (((), "gather+smem", "gather+phi-tma"),
                                   (("pops_gather",), "gather+phi-tma", "gather+phi-tma"),
                                   (("pops_staged",), "gather+smem", "gather+smem"),
+                                  (("no_pdl",), "gather+smem", "gather+phi-tma"),
                                   (("phi_ldg",), "direct", "direct")):
         sim = gpu.LBM(_with_kernels(P3w, *names), 64); assert sim.variant == want64, (names, sim.variant); sim.destroy()
         sim = gpu.LBM(_with_kernels(P3w, *names), 32); assert sim.variant == want32, (names, sim.variant); sim.destroy()
@@ -592,7 +593,7 @@ def test_paper_film_boiling_bubble_detaches(gpu):
     (512 x 512 nodes, lambda = 0.64 > lambda_c = 0.2738): the crest of the film grows, a bubble detaches from it ("node",
     PAPER.md:535) and rises; T stays within a few percent of [theta_sat, theta_w], phi within [0, 1].  Measured on the full
     1024^2 domain: first detached bubbles at t* = t/t_s of about 29 (profiles/r1_full_horizon.md)."""
-    from paper_2003_06342_b200 import run_configs as rc
+    import observables as rc
     P, I = wl.paper_film_boiling(nx=512, ny=512)
     sim = gpu.LBM(P, 64)
     sim.init(I["phi"], I["T"])

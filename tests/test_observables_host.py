@@ -1,10 +1,11 @@
-"""Host logic of the full-horizon runner (paper_2003_06342_b200/run_configs.py) and of the paper's film-boiling recipe:
-no GPU, no arithmetic of the method -- the reductions that turn fields into the observables of PAPER.md:535."""
+"""Host logic of the observables helpers (tests/observables.py) and of the paper's film-boiling recipe: no GPU, no
+arithmetic of the method -- the reductions that turn fields into the observables of PAPER.md:535."""
 import math
 
 import numpy as np
 
-from paper_2003_06342_b200 import run_configs as rc, workloads as wl
+import observables as rc
+from paper_2003_06342_b200 import workloads as wl
 
 
 def test_interface_position_by_linear_interpolation():
