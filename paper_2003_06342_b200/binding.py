@@ -170,7 +170,7 @@ def _host_ptr(a, dtype, shape, name, output=False):
 class LBM:
     """One simulation context on the current CUDA device and stream."""
 
-    def __init__(self, P: dict, precision: int = 64, stream=None):
+    def __init__(self, P: dict, precision: int = 64, stream=None, workspace=None):
         import torch
         if not torch.cuda.is_available():
             raise LBMError("no CUDA device: the library has no CPU path")
@@ -187,7 +187,12 @@ class LBM:
             raise LBMError("lbm_workspace_bytes rejected the parameters")
         self.workspace_bytes = nbytes
         # device memory is allocated by torch and lent to the library (torch allocations are 512-byte aligned)
-        self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        # (or by the caller: ``workspace`` = a uint8 CUDA tensor of at least ``lbm_workspace_bytes`` bytes, 256-byte aligned)
+        if workspace is None:
+            workspace = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        elif workspace.dtype != torch.uint8 or workspace.device.type != "cuda" or not workspace.is_contiguous() or workspace.numel() < nbytes:
+            raise ValueError("workspace: contiguous uint8 CUDA tensor of at least %d bytes expected" % nbytes)
+        self._ws = workspace
         # A stream of the context's own unless the caller gives one: every call below is enqueued there, and the CUDA-graph
         # replay of small grids needs a stream that can be captured (the legacy default stream cannot).
         self._stream = stream if stream is not None else torch.cuda.Stream()
