@@ -322,18 +322,29 @@ def run_slabs(args):
             raise SystemExit("bench.py: --parallelism slabs is defined for config4 (stacked along z)")
         P, _ = wl.config4_film3d(16, 16, 16)                      # parameters only
         P.update(nx=256, ny=256, nz=512 * world)
-        sim = slabs.DistSlab(P, rank, world, prec)
+        sim = slabs.DistSlab(P, rank, world, prec, overlap=not args.no_overlap)
         z0, z1 = sim.slab.layer_range()
         _, I = wl.config4_film3d(256, 256, 512 * world, zrange=(z0, z1))
         sim.init(I["phi"], I["T"], local=True)
         n_slabs, mode = world, "slabs x%d (one per rank, NCCL p2p ghost exchange)" % world
         owned = sim.slab.P["slab"]["count"] * 256 * 256
+        scaling = "weak"
+    elif args.parallelism == "slabs-strong":
+        # the paper's decomposed runs: ONE domain cut into one slab per rank along its slowest axis,
+        # e.g. --workload config3_1024x1024_q9 on 4 ranks (4 x 1024x256), config3_4096x3072_q9_mm on 8
+        P, I = make_workload(args.workload)
+        sim = slabs.DistSlab(P, rank, world, prec, overlap=not args.no_overlap)
+        sim.init(I["phi"], I["T"])
+        n_slabs, mode = world, "one domain cut into %d slabs (one per rank, NCCL p2p ghost exchange)" % world
+        owned = sim.slab.P["slab"]["count"] * (P["nx"] * P["ny"] if P["nz"] > 1 else P["nx"])
+        scaling = "strong"
     else:
         P, I = make_workload(args.workload)
-        sim = slabs.SlabGroup(P, args.slabs, prec)
+        sim = slabs.SlabGroup(P, args.slabs, prec, overlap=not args.no_overlap)
         sim.init(I["phi"], I["T"])
-        n_slabs, mode = args.slabs, "slabs x%d in one process on one GPU (sequential)" % args.slabs
+        n_slabs, mode = args.slabs, "slabs x%d in one process on one GPU" % args.slabs
         owned = P["nx"] * P["ny"] * P["nz"]
+        scaling = "weak"
     del I
     sim.step(W)
     torch.cuda.synchronize()
@@ -342,7 +353,7 @@ def run_slabs(args):
     torch.cuda.synchronize()
     e0.record(sim.stream)
     sim.step(K)
-    e1.record(sim.stream)
+    e1.record(sim.stream)          # the compute stream: every step ends there, after the last exchange has been waited for
     torch.cuda.synchronize()
     replicas.barrier()
     ms_job, lu_job = replicas.reduce_job(e0.elapsed_time(e1), float(owned) * K, dev)
@@ -352,10 +363,11 @@ def run_slabs(args):
         print(json.dumps({
             "metric": METRIC if prec == 64 else "MLUPS (full coupled step, fp32)",
             "value": replicas.job_throughput_mlups(ms_job, lu_job), "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_job / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_job / K, "higher_is_better": True, "scaling": scaling, "vs_baseline": None,
             "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
             "config": {"workload": args.workload, "grid": [P["nx"], P["ny"], P["nz"]], "parallelism": mode,
-                       "slabs": n_slabs, "finite": finite}}))
+                       "slabs": n_slabs, "finite": finite,
+                       "schedule": "plain (one stream)" if args.no_overlap else "boundary layers first, exchange on a second stream"}}))
     sim.destroy()
     return 0
 
@@ -369,8 +381,10 @@ def main():
     ap.add_argument("--precision", type=int, default=64, choices=(32, 64))
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--parallelism", default="replicas", choices=("replicas", "slabs"),
-                    help="N > 1: independent replicas (default, the bench contract) or one slab of a stacked domain per rank")
+    ap.add_argument("--parallelism", default="replicas", choices=("replicas", "slabs", "slabs-strong"),
+                    help="N > 1: independent replicas (default, the bench contract), one slab of a stacked domain per rank (weak), "
+                         "or ONE domain cut into one slab per rank (strong; the paper's decomposed runs)")
+    ap.add_argument("--no-overlap", action="store_true", help="slabs: the plain one-stream schedule instead of boundary layers first")
     ap.add_argument("--slabs", type=int, default=0, help="cut the workload into this many slabs on ONE GPU (overhead measurement)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
@@ -380,7 +394,7 @@ def main():
             args.steps = 20          # bounded: the oracle runs at a few MLUPS
         args.warmup = min(args.warmup, 2)
         return run_reference(args)
-    if args.slabs > 0 or args.parallelism == "slabs":
+    if args.slabs > 0 or args.parallelism in ("slabs", "slabs-strong"):
         return run_slabs(args)
     return run_ours(args)
 

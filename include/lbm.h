@@ -176,6 +176,21 @@ int lbm_set_velocity(lbm_ctx *c, const void *h_u);
  * after the pack and the unpack after the transfer.  LBM_E_INVALID if the context has no ghost layer on that side. */
 enum { LBM_HALO_PHI = 0, LBM_HALO_POPS = 1 };
 int lbm_step_phase(lbm_ctx *c, int phase, int store_macros);
+
+/* A phase in parts, for schedules that overlap the exchange with the interior (boundary layers first; PAPER.md:324, 559 is
+ * the paper's decomposition, the overlap is this library's): run `phase` on the layers [first, first + count) of the slowest
+ * axis only.  The caller covers every layer whose results it needs exactly once per phase -- the ghost layers need none: what
+ * a step reads from them arrives by lbm_halo_unpack -- and marks the last part with last != 0, which completes the phase
+ * (after phase 1 the buffers flip).  count == 0 is allowed (a bare "last").  While parts of phase 0 are outstanding
+ * LBM_HALO_PHI may already be packed (from layers done) and unpacked; while parts of phase 1 are outstanding LBM_HALO_POPS
+ * refers to the populations being written by this step.  Ordering between the parts, the packs and the transfers on the
+ * device is the caller's (one stream, or events between two: lbm_set_stream).  Not with LBM_FLAG_PRESCRIBED_U unless the
+ * one part is the whole grid. */
+int lbm_step_layers(lbm_ctx *c, int phase, int first, int count, int store_macros, int last);
+
+/* Enqueue the following calls of this context on another cudaStream_t (e.g. the packs and unpacks on an exchange stream while
+ * the interior runs on the compute stream).  The caller orders the streams with events. */
+int lbm_set_stream(lbm_ctx *c, void *cuda_stream);
 int lbm_halo_bytes(const lbm_ctx *c, int what, size_t *bytes);
 int lbm_halo_pack(lbm_ctx *c, int what, int side, void *d_buf);
 int lbm_halo_unpack(lbm_ctx *c, int what, int side, const void *d_buf);

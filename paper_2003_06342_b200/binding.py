@@ -30,7 +30,7 @@ STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1
 NOALLOC_SCRATCH_BYTES = 8 << 20
 
-EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
            "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
@@ -76,6 +76,8 @@ def load_library():
         L.lbm_step.argtypes = [C.c_void_p, C.c_int]
         L.lbm_set_velocity.argtypes = [C.c_void_p, C.c_void_p]
         L.lbm_step_phase.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.lbm_step_layers.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.lbm_set_stream.argtypes = [C.c_void_p, C.c_void_p]
         L.lbm_halo_bytes.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_size_t)]
         L.lbm_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
@@ -218,6 +220,15 @@ class LBM:
     # slab contexts (P["halo"]): the two phases of a step and the ghost-layer buffers, see include/lbm.h
     def step_phase(self, phase: int, store_macros: bool = False):
         _check(self._L.lbm_step_phase(self._h, int(phase), 1 if store_macros else 0), "lbm_step_phase")
+
+    def step_layers(self, phase: int, first: int, count: int, store_macros: bool = False, last: bool = False):
+        _check(self._L.lbm_step_layers(self._h, int(phase), int(first), int(count), 1 if store_macros else 0, 1 if last else 0),
+               "lbm_step_layers")
+
+    def set_stream(self, stream):
+        """Enqueue the following calls on ``stream`` (a torch.cuda.Stream); the caller orders the streams with events."""
+        _check(self._L.lbm_set_stream(self._h, C.c_void_p(stream.cuda_stream)), "lbm_set_stream")
+        self._stream = stream
 
     def halo_bytes(self, what: int) -> int:
         n = C.c_size_t()

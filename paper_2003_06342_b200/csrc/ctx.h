@@ -36,6 +36,7 @@ struct ImplOps {
     int (*init)(lbm_ctx *, const void *, const void *, const void *, const void *);
     int (*step)(lbm_ctx *, int);
     int (*step_phase)(lbm_ctx *, int, int);
+    int (*step_layers)(lbm_ctx *, int, int, int, int, int);   // phase, first layer, count, store macros, last part of the phase
     int (*read_macro)(lbm_ctx *, void *, void *, void *, void *);
     int (*read_pops)(lbm_ctx *, int, int, void *);
     int (*read_pops_scratch)(lbm_ctx *, int, int, void *, void *, size_t);   // staged in a caller-given device scratch (noalloc.cu)
@@ -65,6 +66,7 @@ struct lbm_ctx {
     int curphi;    // padded phi buffer of the current level
     bool inited;
     int phase;     // slab contexts: the phase lbm_step_phase expects next (0 or 1)
+    bool partial;  // lbm_step_layers has run parts of that phase, its last part is still due
     long long nsteps, launches;
     lbm::DevParams<double> pd;
     lbm::DevParams<float> pf;

@@ -53,7 +53,8 @@ bool make_plan(const lbm_ctx *c, int what, int side, bool ghost, HaloPlan &pl) {
         // padded array: layer l of the domain is padded layer l + 1 along the slab axis; whole padded layer with its images
         const size_t layer_elems = three_d ? (size_t)c->L.ppx * c->L.ppy : (size_t)c->L.ppx;
         pl.elems = layer_elems;
-        const int pnew = c->phase == 1 ? 1 - c->curphi : c->curphi;   // between the phases phi^{n+1} is the other buffer
+        // between the phases -- and while parts of phase 0 are running (lbm_step_layers) -- phi^{n+1} is the other buffer
+        const int pnew = (c->phase == 1 || c->partial) ? 1 - c->curphi : c->curphi;
         pl.ptr[pl.count++] = c->ws + c->L.off_phi[pnew] + (size_t)(layer + 1) * layer_elems * esp;
         return true;
     }
@@ -61,26 +62,29 @@ bool make_plan(const lbm_ctx *c, int what, int side, bool ghost, HaloPlan &pl) {
     // A ghost layer of side s RECEIVES what the neighbour sent towards its 1 - s side, i.e. e_axis pointing inwards.
     const int dir = ghost ? (side == 0 ? +1 : -1) : (side == 0 ? -1 : +1);
     pl.elems = three_d ? (unsigned long long)P.nx * P.ny : (unsigned long long)P.nx;
+    // the populations of the level just collided: the current buffers, or -- while parts of phase 1 are running and the
+    // buffers have not flipped yet (lbm_step_layers) -- the other ones
+    const int cur = (c->phase == 1 && c->partial) ? 1 - c->cur : c->cur;
     switch (c->set) {
     case SET_2D_995:
-        add_pops<D2Q9>(pl, c, c->L.off_f[c->cur], axis, dir, layer, es);
-        add_pops<D2Q9>(pl, c, c->L.off_g[c->cur], axis, dir, layer, es);
-        add_pops<D2Q5>(pl, c, c->L.off_s[c->cur], axis, dir, layer, es);
+        add_pops<D2Q9>(pl, c, c->L.off_f[cur], axis, dir, layer, es);
+        add_pops<D2Q9>(pl, c, c->L.off_g[cur], axis, dir, layer, es);
+        add_pops<D2Q5>(pl, c, c->L.off_s[cur], axis, dir, layer, es);
         break;
     case SET_2D_999:
-        add_pops<D2Q9>(pl, c, c->L.off_f[c->cur], axis, dir, layer, es);
-        add_pops<D2Q9>(pl, c, c->L.off_g[c->cur], axis, dir, layer, es);
-        add_pops<D2Q9>(pl, c, c->L.off_s[c->cur], axis, dir, layer, es);
+        add_pops<D2Q9>(pl, c, c->L.off_f[cur], axis, dir, layer, es);
+        add_pops<D2Q9>(pl, c, c->L.off_g[cur], axis, dir, layer, es);
+        add_pops<D2Q9>(pl, c, c->L.off_s[cur], axis, dir, layer, es);
         break;
     case SET_3D_1977:
-        add_pops<D3Q19>(pl, c, c->L.off_f[c->cur], axis, dir, layer, es);
-        add_pops<D3Q7>(pl, c, c->L.off_g[c->cur], axis, dir, layer, es);
-        add_pops<D3Q7>(pl, c, c->L.off_s[c->cur], axis, dir, layer, es);
+        add_pops<D3Q19>(pl, c, c->L.off_f[cur], axis, dir, layer, es);
+        add_pops<D3Q7>(pl, c, c->L.off_g[cur], axis, dir, layer, es);
+        add_pops<D3Q7>(pl, c, c->L.off_s[cur], axis, dir, layer, es);
         break;
     case SET_3D_1577:
-        add_pops<D3Q15>(pl, c, c->L.off_f[c->cur], axis, dir, layer, es);
-        add_pops<D3Q7>(pl, c, c->L.off_g[c->cur], axis, dir, layer, es);
-        add_pops<D3Q7>(pl, c, c->L.off_s[c->cur], axis, dir, layer, es);
+        add_pops<D3Q15>(pl, c, c->L.off_f[cur], axis, dir, layer, es);
+        add_pops<D3Q7>(pl, c, c->L.off_g[cur], axis, dir, layer, es);
+        add_pops<D3Q7>(pl, c, c->L.off_s[cur], axis, dir, layer, es);
         break;
     default: return false;
     }
@@ -91,8 +95,10 @@ int halo_copy(lbm_ctx *c, int what, int side, void *d_buf, bool pack) {
     if (!c || !d_buf || (what != LBM_HALO_PHI && what != LBM_HALO_POPS) || (side != 0 && side != 1)) return LBM_E_INVALID;
     if (!c->P.halo[side]) return LBM_E_INVALID;
     if (!c->inited) return LBM_E_STATE;
-    // phi travels between the phases, the populations after phase 1 (or after lbm_init)
-    if ((what == LBM_HALO_PHI) != (c->phase == 1)) return LBM_E_STATE;
+    // phi travels between the phases or while parts of phase 0 are running; the populations after phase 1 (or after lbm_init)
+    // or while parts of phase 1 are running (lbm_step_layers: boundary layers first)
+    const bool phi_time = (c->phase == 1 && !c->partial) || (c->phase == 0 && c->partial);
+    if ((what == LBM_HALO_PHI) != phi_time) return LBM_E_STATE;
     HaloPlan pl;
     if (!make_plan(c, what, side, /*ghost=*/!pack, pl)) return LBM_E_INVALID;
     const unsigned gx = (unsigned)((pl.elems + 1023) / 1024 > 0 ? (pl.elems + 1023) / 1024 : 1);

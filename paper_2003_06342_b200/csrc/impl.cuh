@@ -29,6 +29,14 @@ struct TileWide2 { static constexpr int BX = 128, BY = 2, BZ = 1; using PhiTile 
 struct TileWide2K { static constexpr int BX = 128, BY = 1, BZ = 1; using PhiTile = TileWide2; };
 struct TileNarrow2 { static constexpr int BX = 32, BY = 8, BZ = 1; using PhiTile = TileNarrow2; };
 
+// grid of a K_phi / K_main launch over the layers [pd.s0, pd.s1) of the slowest axis (lbm_ctx::pd, pf carry the same range)
+template <class T> dim3 grid_layers(const lbm_ctx *c) {
+    const lbm_params &P = c->P;
+    const int n = c->pd.s1 - c->pd.s0;
+    if (P.nz > 1) return dim3((P.nx + T::BX - 1) / T::BX, (P.ny + T::BY - 1) / T::BY, (n + T::BZ - 1) / T::BZ);
+    return dim3((P.nx + T::BX - 1) / T::BX, (n + T::BY - 1) / T::BY, 1);
+}
+
 template <class real> const DevParams<real> &dev_params(const lbm_ctx *c);
 template <> inline const DevParams<double> &dev_params<double>(const lbm_ctx *c) { return c->pd; }
 template <> inline const DevParams<float> &dev_params<float>(const lbm_ctx *c) { return c->pf; }
@@ -91,7 +99,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     template <class K> static cudaError_t launch_after_phi(lbm_ctx *c, K kern, size_t smem, const DevParams<real> &P, const Fields &F,
                                                            const CUtensorMap &map) {
         cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = grid_for<T>(c->P); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+        cfg.gridDim = grid_layers<T>(c); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[0].val.programmaticStreamSerializationAllowed = 1;
@@ -118,7 +126,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
             }
         }
         k_main_direct<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB>
-            <<<grid_for<T>(c->P), NT, 0, c->stream>>>(dev_params<real>(c), F);
+            <<<grid_layers<T>(c), NT, 0, c->stream>>>(dev_params<real>(c), F);
         c->launches++;
         CK(cudaGetLastError());
         return LBM_OK;
@@ -152,7 +160,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         if (rc) return rc;
         CK(cudaStreamSynchronize(c->stream));
         c->nsteps = 0;
-        c->inited = true; c->phase = 0;
+        c->inited = true; c->phase = 0; c->partial = false;
         return LBM_OK;
     }
 
@@ -160,7 +168,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     static int launch_phi(lbm_ctx *c) {
         const DevParams<real> &P = dev_params<real>(c);
         const int in = c->cur, pnew = 1 - c->curphi;
-        dim3 gphi = grid_for<TP>(c->P);
+        dim3 gphi = grid_layers<TP>(c);
         if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
         k_phi<LG, real, TP::BX, TP::BY, TP::BZ, PHI_NPT><<<gphi, NTP, 0, c->stream>>>(
             P, (const sreal *)wsp<sreal>(c, c->L.off_g[in]), wsp<preal>(c, c->L.off_phi[pnew]));
@@ -169,8 +177,8 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         return LBM_OK;
     }
 
-    // phase 1 of a step: K_main, then the buffers flip
-    static int launch_collide(lbm_ctx *c, bool macro) {
+    // phase 1 of a step: K_main, then (flip) the buffers flip
+    static int launch_collide(lbm_ctx *c, bool macro, bool flip = true) {
         const DevParams<real> &P = dev_params<real>(c);
         const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
         Fields F = fields(c, in, out, pnew, pold);
@@ -178,8 +186,20 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         if (P.prescribed_u) rc = launch_main<MODE_STEP_PU>(c, F, pnew);   // direct kernel only
         else rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, pnew) : launch_main<MODE_STEP>(c, F, pnew);
         if (rc) return rc;
-        c->cur = out; c->curphi = pnew; c->nsteps++;
+        if (flip) { c->cur = out; c->curphi = pnew; c->nsteps++; }
         return LBM_OK;
+    }
+
+    // one phase on the layers [first, first + count) of the slowest axis only (lbm_step_layers, include/lbm.h)
+    static int step_layers(lbm_ctx *c, int phase, int first, int count, int macro, int last) {
+        if (count == 0) {   // nothing to launch: the last "part" of phase 1 still flips the buffers
+            if (phase == 1 && last) { c->cur = 1 - c->cur; c->curphi = 1 - c->curphi; c->nsteps++; }
+            return LBM_OK;
+        }
+        c->pd.s0 = c->pf.s0 = first; c->pd.s1 = c->pf.s1 = first + count;
+        const int rc = phase == 0 ? launch_phi(c) : launch_collide(c, macro != 0, last != 0);
+        c->pd.s0 = c->pf.s0 = 0; c->pd.s1 = c->pf.s1 = D == 3 ? c->P.nz : c->P.ny;
+        return rc;
     }
 
     // the two phases separately, for slab contexts whose ghost layers are exchanged in between (include/lbm.h)
@@ -318,7 +338,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     }
 
     static const ImplOps *ops() {
-        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::step_phase, &Impl::read_macro, &Impl::read_pops, &Impl::read_pops_scratch, T::BX, T::BY, T::BZ};
+        static const ImplOps o = {&Impl::init, &Impl::step, &Impl::step_phase, &Impl::step_layers, &Impl::read_macro, &Impl::read_pops, &Impl::read_pops_scratch, T::BX, T::BY, T::BZ};
         return &o;
     }
 };

@@ -285,9 +285,11 @@ template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, in
 __global__ void __launch_bounds__(BX *BY *BZ, MINB)
 k_main_direct(const DevParams<real> P, const Fields Fd) {
     const int t = threadIdx.x;
-    const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY, z0 = blockIdx.z * BZ;
+    const int x0 = blockIdx.x * BX;
+    int y0, z0;
+    tile_origin<LF::D>(P, BY, BZ, y0, z0);
     const int x = x0 + t % BX, y = y0 + (t / BX) % BY, z = z0 + t / (BX * BY);
-    if (x >= P.nx || y >= P.ny || z >= P.nz) return;
+    if (!node_active<LF::D>(P, x, y, z)) return;
     const NodeGeom g = make_geom(P, x, y, z);
     if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) {
         const SrcGlobal<LF, LG, LS, real, true, Fields> src(P, Fd, g);

@@ -75,7 +75,7 @@ __device__ __forceinline__ void main_tile_phitma(const DevParams<real> &P, const
     }
     __syncthreads();   // the barrier is initialised before anybody waits on it
     const int x = x0 + tx, y = y0 + ty, z = z0 + tz;
-    if (x >= P.nx || y >= P.ny || z >= P.nz) return;
+    if (!node_active<LF::D>(P, x, y, z)) return;
     const NodeGeom g = make_geom(P, x, y, z);
     if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ)) {
         const SrcGlobalPhiSmem<LF, LG, LS, real, true, TC, Fields> src(P, Fd, g, tile, bar_a, tx, ty, tz);
@@ -92,8 +92,9 @@ k_main_phitma(const DevParams<real> P, const Fields Fd, const __grid_constant__ 
     using preal = typename Fields::preal;
     using SM = PhiTileSmem<preal, PhiTileCfg<preal, LF::D, BX, BY, BZ>>;
     __shared__ __align__(128) unsigned char smem_raw[SM::BYTES];
-    main_tile_phitma<LF, LG, LS, real, MODE, BX, BY, BZ>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, blockIdx.y * BY,
-                                                          blockIdx.z * BZ);
+    int y0, z0;
+    tile_origin<LF::D>(P, BY, BZ, y0, z0);
+    main_tile_phitma<LF, LG, LS, real, MODE, BX, BY, BZ>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, y0, z0);
 }
 
 }  // namespace lbm

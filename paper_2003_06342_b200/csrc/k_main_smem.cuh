@@ -109,7 +109,7 @@ __device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const F
         fence_proxy_async();
     }
     const int x = x0 + tx, y = y0 + ty, z = z0 + tz;
-    const bool active = x < P.nx && y < P.ny && z < P.nz;
+    const bool active = node_active<LF::D>(P, x, y, z);
     const bool bc = tile_touches_bc(P, x0, y0, z0, BX, BY, BZ);
     NodeGeom g;
     if (active) {
@@ -141,8 +141,9 @@ template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, in
 __global__ void __launch_bounds__(BX *BY *BZ, MINB)
 k_main_smem(const DevParams<real> P, const Fields Fd, const __grid_constant__ CUtensorMap phi_map) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    main_tile_smem<LF, LG, LS, real, MODE, BX, BY, BZ>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, blockIdx.y * BY,
-                                                        blockIdx.z * BZ);
+    int y0, z0;
+    tile_origin<LF::D>(P, BY, BZ, y0, z0);
+    main_tile_smem<LF, LG, LS, real, MODE, BX, BY, BZ>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, y0, z0);
 }
 
 }  // namespace lbm

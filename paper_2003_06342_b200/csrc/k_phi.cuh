@@ -95,8 +95,8 @@ k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, preal *__restrict
     pdl_launch_dependents();   // K_main may start filling the SMs as this grid drains; it waits (griddepcontrol.wait) before it reads phi
     const int t = threadIdx.x;
     const int x0 = blockIdx.x * BX;
-    const int y0 = blockIdx.y * BY * (ALONG_Z ? 1 : NPT);
-    const int z0 = blockIdx.z * BZ * (ALONG_Z ? NPT : 1);
+    const int y0 = ALONG_Z ? blockIdx.y * BY : P.s0 + blockIdx.y * BY * NPT;   // this launch covers the layers [P.s0, P.s1)
+    const int z0 = ALONG_Z ? P.s0 + blockIdx.z * BZ * NPT : 0;
     const int x = x0 + t % BX, yb = y0 + (t / BX) % BY, zb = z0 + t / (BX * BY);
     if (x >= P.nx) return;
     const bool bc = tile_touches_bc(P, x0, y0, z0, BX, BY * (ALONG_Z ? 1 : NPT), BZ * (ALONG_Z ? NPT : 1));
@@ -106,7 +106,7 @@ k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, preal *__restrict
 #pragma unroll
     for (int j = 0; j < NPT; ++j) {
         const int y = yb + (ALONG_Z ? 0 : j * BY), z = zb + (ALONG_Z ? j * BZ : 0);
-        ok[j] = y < P.ny && z < P.nz;
+        ok[j] = ALONG_Z ? (y < P.ny && z < P.s1) : (y < P.s1);
         if (ok[j]) {
             g[j] = make_geom(P, x, y, z);
             if (bc) pull<LG, vreal, true>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);

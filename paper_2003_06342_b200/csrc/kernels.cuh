@@ -48,6 +48,7 @@ template <class L, int I, class real> __device__ __forceinline__ real dot_e(real
 // ---- kernel parameters (passed by value) ------------------------------------------------------------------
 template <class real> struct DevParams {
     int nx, ny, nz;
+    int s0, s1;            // layers [s0, s1) of the slowest axis (z in 3D, y in 2D) that THIS launch of K_phi / K_main covers
     long long N;           // nx*ny*nz
     int ppx, ppy, pz;      // padded phi: row pitch, ny+2, z offset (1 in 3D, 0 in 2D)
     int xpad;              // padded phi: x offset of node 0 (16 bytes of elements, so TMA boxes start 16-byte aligned)
@@ -179,6 +180,17 @@ __device__ __forceinline__ void pull(const sreal *__restrict__ src, unsigned N, 
         constexpr int I = decltype(ic)::value;
         out[I] = pull_one<L, I, real, BC>(src, N, g, bc, val);
     });
+}
+
+// Origin of a CTA's tile and activity of a node for launches that cover the layers [P.s0, P.s1) of the slowest axis
+// (whole grid: 0 .. nz, or 0 .. ny in 2D; slab contexts launch their boundary layers and their interior separately).
+template <int D, class real>
+__device__ __forceinline__ void tile_origin(const DevParams<real> &P, int BY, int BZ, int &y0, int &z0) {
+    if (D == 3) { y0 = blockIdx.y * BY; z0 = P.s0 + blockIdx.z * BZ; }
+    else { y0 = P.s0 + blockIdx.y * BY; z0 = 0; }
+}
+template <int D, class real> __device__ __forceinline__ bool node_active(const DevParams<real> &P, int x, int y, int z) {
+    return D == 3 ? (x < P.nx && y < P.ny && z < P.s1) : (x < P.nx && y < P.s1);
 }
 
 // does the tile [x0,x0+bx) x [y0,y0+by) x [z0,z0+bz) touch a non-periodic face?  (block-uniform)

@@ -115,6 +115,7 @@ Layout make_layout(const lbm_params *p) {
 template <class real> DevParams<real> make_dev_params(const lbm_params *p, const Layout &L) {
     DevParams<real> d{};
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.N = L.N;
+    d.s0 = 0; d.s1 = p->nz > 1 ? p->nz : p->ny;   // K_phi / K_main launches cover every layer unless lbm_step_layers narrows them
     d.ppx = L.ppx; d.ppy = L.ppy; d.pz = L.pz; d.xpad = L.xpad; d.pplane = (long long)L.ppx * L.ppy;
     for (int a = 0; a < 3; ++a) {
         for (int s = 0; s < 2; ++s) {
@@ -250,7 +251,7 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
     }
     c->ws = static_cast<char *>(d_workspace);
     c->stream = static_cast<cudaStream_t>(cuda_stream);
-    c->cur = 0; c->curphi = 0; c->phase = 0; c->inited = false; c->nsteps = 0; c->launches = 0; c->timing = false;
+    c->cur = 0; c->curphi = 0; c->phase = 0; c->partial = false; c->inited = false; c->nsteps = 0; c->launches = 0; c->timing = false;
     c->pd = make_dev_params<double>(p, L);
     c->pf = make_dev_params<float>(p, L);
     c->num_sms = prop.multiProcessorCount;
@@ -289,12 +290,32 @@ int lbm_set_velocity(lbm_ctx *c, const void *h_u) {
 int lbm_step(lbm_ctx *c, int n) {
     if (!c || n < 0) return LBM_E_INVALID;
     if (!c->inited || (c->P.halo[0] | c->P.halo[1])) return LBM_E_STATE;   // slabs step by phases (ghost exchange in between)
+    if (c->phase != 0 || c->partial) return LBM_E_STATE;
     return c->ops->step(c, n);
+}
+
+int lbm_step_layers(lbm_ctx *c, int phase, int first, int count, int store_macros, int last) {
+    if (!c || (phase != 0 && phase != 1)) return LBM_E_INVALID;
+    const int nslow = c->P.nz > 1 ? c->P.nz : c->P.ny;
+    if (first < 0 || count < 0 || first + count > nslow) return LBM_E_INVALID;
+    if (!c->inited || phase != c->phase) return LBM_E_STATE;
+    if (c->P.flags & LBM_FLAG_PRESCRIBED_U) { if (first != 0 || count != nslow || !last) return LBM_E_UNSUPPORTED; }
+    const int rc = c->ops->step_layers(c, phase, first, count, store_macros, last);
+    if (rc) return rc;
+    c->partial = !last;
+    if (last) c->phase = 1 - phase;
+    return LBM_OK;
+}
+
+int lbm_set_stream(lbm_ctx *c, void *cuda_stream) {
+    if (!c) return LBM_E_INVALID;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    return LBM_OK;
 }
 
 int lbm_step_phase(lbm_ctx *c, int phase, int store_macros) {
     if (!c || (phase != 0 && phase != 1)) return LBM_E_INVALID;
-    if (!c->inited || phase != c->phase) return LBM_E_STATE;
+    if (!c->inited || phase != c->phase || c->partial) return LBM_E_STATE;
     const int rc = c->ops->step_phase(c, phase, store_macros);
     if (rc == LBM_OK) c->phase = 1 - phase;
     return rc;

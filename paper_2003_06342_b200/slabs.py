@@ -5,8 +5,11 @@ the C ABI whose parameters declare a ghost layer on every cut side (``lbm_params
 
     K_phi (phase 0)  ->  exchange LBM_HALO_PHI  ->  K_main (phase 1)  ->  exchange LBM_HALO_POPS
 
-and the exchanges move one padded phi layer and the 7 (3D) populations that cross the cut, per side.  Everything the
-method computes still runs in the kernels; this module only decides who owns which layers and moves the packed buffers:
+and the exchanges move one padded phi layer and the 7 (3D) populations that cross the cut, per side.  The default schedule
+overlaps them with the interior (:func:`step_overlapped`: boundary layers first on the compute stream, pack / transfer /
+unpack on a second stream, ordered by events; the ghost layers themselves are never computed); ``overlap=False`` keeps the
+plain one-stream sequence above.  Everything the method computes still runs in the kernels; this module only decides who owns
+which layers and moves the packed buffers:
 
 * :class:`SlabGroup`  -- all slabs in ONE process on one GPU (the buffers are handed over directly); this is how the
   decomposition is parity-tested on a single GPU (tests/test_gpu_slabs.py): the stitched result equals the undecomposed
@@ -149,6 +152,102 @@ def exchange_dist(slab, what: int, rank: int, world: int, periodic: bool, group=
             slab.halo_unpack(what, side, src)
 
 
+# ------------------------------------------------------------------------------------------- overlapped schedule (host logic)
+def layer_parts(n_local: int, halo):
+    """Owned layers of a slab with ``n_local`` layers (ghosts included) by role: ``boundary`` = [(first, count)] of the owned
+    layers next to a ghost layer (what the neighbours wait for), ``interior`` = (first, count) of the other owned layers."""
+    lo, hi = halo[0], n_local - halo[1]                 # owned layers [lo, hi)
+    boundary = []
+    if halo[0]:
+        boundary.append((lo, 1))
+    if halo[1] and (hi - 1 != lo or not halo[0]):
+        boundary.append((hi - 1, 1))
+    first = lo + (1 if halo[0] else 0)
+    last = hi - (1 if halo[1] else 0)
+    return {"boundary": boundary, "interior": (first, max(last - first, 0))}
+
+
+class NoStreams:
+    """Stand-in for :class:`TwoStreams` where everything is ordered by the host (CPU tests)."""
+
+    def begin_exchange(self, slabs):
+        pass
+
+    def end_exchange(self, slabs):
+        pass
+
+    def wait_exchange(self):
+        pass
+
+    def exchange_context(self):
+        import contextlib
+        return contextlib.nullcontext()
+
+
+class TwoStreams:
+    """Compute stream C and exchange stream X (pack, transfer, unpack, and K_main of the boundary layers), ordered by events:
+    X continues after what C has enqueued so far (begin_exchange); C waits for X where it needs its results (wait_exchange)."""
+
+    def __init__(self, compute, exchange):
+        self.C, self.X, self.pending = compute, exchange, None
+
+    def begin_exchange(self, slabs):
+        import torch
+        ev = torch.cuda.Event()
+        ev.record(self.C)
+        self.X.wait_event(ev)
+        for s in slabs:
+            s.set_stream(self.X)
+
+    def end_exchange(self, slabs):
+        import torch
+        self.pending = torch.cuda.Event()
+        self.pending.record(self.X)
+        for s in slabs:
+            s.set_stream(self.C)
+
+    def wait_exchange(self):
+        if self.pending is not None:
+            self.C.wait_event(self.pending)
+            self.pending = None
+
+    def exchange_context(self):
+        import torch
+        return torch.cuda.stream(self.X)        # torch.distributed orders its transfers against the CURRENT stream
+
+
+def step_overlapped(slabs, exchange, sched, n: int):
+    """``n`` steps of the slabs of this process, boundary layers first, on two streams:
+
+        C:  K_phi(boundary) . K_phi(interior) ............ K_main(interior) ............................ | next step
+        X:                  . exchange phi    . K_main(boundary) . exchange populations ............... -^
+
+    C is the compute stream, X the exchange stream (higher priority).  K_main of the boundary layers -- less than one wave of
+    CTAs -- runs on X while the interior fills the SMs on C; the next step on C waits for X once, at its start.
+    ``slabs[i].run_part(phase, which, store_macros, last)`` enqueues one part on the slab's current stream, ``exchange(what)``
+    packs, moves and unpacks, ``sched`` switches the slabs between the streams and orders these with events."""
+    for k in range(n):
+        macro = k == n - 1
+        sched.wait_exchange()                              # boundary layers and ghost populations of the previous level
+        for s in slabs:
+            s.run_part(0, "boundary", False, False)
+        sched.begin_exchange(slabs)                        # X: after K_phi(boundary)
+        with sched.exchange_context():
+            exchange(HALO_PHI)
+        sched.end_exchange(slabs)
+        for s in slabs:
+            s.run_part(0, "interior", False, True)
+        sched.begin_exchange(slabs)                        # X: after K_phi(interior) as well
+        for s in slabs:
+            s.run_part(1, "boundary", macro, False)
+        with sched.exchange_context():
+            exchange(HALO_POPS)
+        sched.end_exchange(slabs)
+        for s in slabs:
+            s.run_part(1, "interior", macro, True)
+    sched.wait_exchange()
+
+
 # ------------------------------------------------------------------------------------------------------ slab contexts
 class Slab:
     """One slab context plus its exchange buffers.  Device memory comes from torch (plumbing)."""
@@ -181,6 +280,19 @@ class Slab:
     def halo_unpack(self, what, side, buf):
         self.sim.halo_unpack(what, side, buf)
 
+    def set_stream(self, stream):
+        self.sim.set_stream(stream)
+
+    def run_part(self, phase, which, store_macros, last):
+        """One part of a phase (lbm_step_layers): the owned layers next to the ghost layers, or the other owned layers."""
+        n = int(self.P["nz"]) if slab_axis(self.P) == 2 else int(self.P["ny"])
+        parts = layer_parts(n, self.halo)
+        ranges = parts["boundary"] if which == "boundary" else [parts["interior"]]
+        if not ranges:
+            ranges = [(0, 0)]
+        for i, (first, count) in enumerate(ranges):
+            self.sim.step_layers(phase, first, count, store_macros, last and i == len(ranges) - 1)
+
     def init(self, phi, T=None, u=None, p=None):
         """GLOBAL initial fields; the slab takes its layers and the ghost copies."""
         args = [local_block(a, self.Pg, self.rank, self.world) for a in (phi, T, u, p)]
@@ -209,13 +321,15 @@ class Slab:
 class SlabGroup:
     """``nslabs`` slabs of one domain in one process, on the current device and stream."""
 
-    def __init__(self, P: dict, nslabs: int, precision: int = 64):
+    def __init__(self, P: dict, nslabs: int, precision: int = 64, overlap: bool = True):
         import torch
         self.P = P
         self.periodic = axis_is_periodic(P)
-        self.stream = torch.cuda.Stream()   # one stream for all slabs: pack, hand-over and unpack are ordered by it
+        self.stream = torch.cuda.Stream()   # compute stream of all slabs
         self.slabs = [Slab(P, r, nslabs, precision, stream=self.stream) for r in range(nslabs)]
         self.any_halo = any(s.has_halo for s in self.slabs)
+        self.overlap = overlap and not P.get("prescribed_u", False)
+        self.sched = TwoStreams(self.stream, torch.cuda.Stream(priority=-1)) if self.overlap else None
 
     def init(self, phi, T=None, u=None, p=None):
         for s in self.slabs:
@@ -226,6 +340,9 @@ class SlabGroup:
     def step(self, n: int = 1):
         if not self.any_halo:
             self.slabs[0].sim.step(n)
+            return
+        if self.overlap:
+            step_overlapped(self.slabs, lambda what: exchange_local(self.slabs, what, self.periodic), self.sched, n)
             return
         for k in range(n):
             for s in self.slabs:
@@ -253,23 +370,38 @@ class SlabGroup:
 class DistSlab:
     """The slab of this rank in a ``torch.distributed`` job (one process per GPU)."""
 
-    def __init__(self, P: dict, rank: int, world: int, precision: int = 64, group=None):
+    def __init__(self, P: dict, rank: int, world: int, precision: int = 64, group=None, overlap: bool = True):
         self.periodic = axis_is_periodic(P)
         import torch
         self.rank, self.world, self.group = rank, world, group
-        # the transfers (torch.distributed) are enqueued on torch's current stream: the slab's kernels go there too
-        self.slab = Slab(P, rank, world, precision, stream=torch.cuda.current_stream())
+        self.overlap = overlap and not P.get("prescribed_u", False)
+        if self.overlap:
+            # kernels on a compute stream of the slab's own; packs, transfers and unpacks on the exchange stream
+            self.slab = Slab(P, rank, world, precision)
+            self.stream = self.slab.sim.stream
+            self.sched = TwoStreams(self.stream, torch.cuda.Stream(priority=-1))
+        else:
+            # the transfers (torch.distributed) are enqueued on torch's current stream: the slab's kernels go there too
+            self.stream = torch.cuda.current_stream()
+            self.slab = Slab(P, rank, world, precision, stream=self.stream)
+            self.sched = None
 
     def init(self, phi, T=None, u=None, p=None, local=False):
         """GLOBAL fields, or with ``local=True`` this rank's layers including the ghost copies (Slab.layer_range)."""
+        import torch
         (self.slab.init_local if local else self.slab.init)(phi, T, u, p)
         if self.slab.has_halo:
-            exchange_dist(self.slab, HALO_POPS, self.rank, self.world, self.periodic, self.group)
+            with torch.cuda.stream(self.stream):     # packs, transfers and unpacks of level 0 on the compute stream
+                exchange_dist(self.slab, HALO_POPS, self.rank, self.world, self.periodic, self.group)
 
     def step(self, n: int = 1):
         s = self.slab
         if not s.has_halo:
             s.sim.step(n)
+            return
+        if self.overlap:
+            step_overlapped([s], lambda what: exchange_dist(s, what, self.rank, self.world, self.periodic, self.group),
+                            self.sched, n)
             return
         for k in range(n):
             s.sim.step_phase(0)

@@ -3,8 +3,9 @@ contexts in one process, ghost layers handed over with lbm_halo_pack / lbm_halo_
 The stitched result must equal the undecomposed CUDA run -- BIT FOR BIT when every face is periodic (same kernels, same
 neighbour values); to a few ulp when physical faces are present, because a node may then fall into a tile that takes the
 boundary instantiation of the kernel in one run and the plain one in the other (the two are compiled separately and
-contract multiply-adds differently) -- and the CPU oracle of the whole domain within the fp64 tolerance.  The slabs run one after the other on one stream -- no kernel waits
-on another."""
+contract multiply-adds differently) -- and the CPU oracle of the whole domain within the fp64 tolerance.  Both schedules are
+checked: the overlapped one (boundary layers first, exchanges on a second stream ordered by events, ghost layers not
+computed; the default) and the plain one-stream sequence.  No kernel waits on another: the order is the streams'."""
 import numpy as np
 import pytest
 
@@ -38,7 +39,8 @@ def _state(group_or_sim, gpu):
 def _check(gpu, oracle_mod, P, init, nslabs_list, horizons, precision=64, oracle=True, exact=True):
     single = gpu.LBM(P, precision)
     single.init(*init)
-    groups = [slabs.SlabGroup(P, n, precision) for n in nslabs_list]
+    nslabs_list = [n for n in nslabs_list for _ in range(2)]
+    groups = [slabs.SlabGroup(P, n, precision, overlap=(i % 2 == 0)) for i, n in enumerate(nslabs_list)]
     for g in groups:
         g.init(*init)
     o = None

@@ -62,6 +62,19 @@ def test_local_block_and_strip():
     assert np.array_equal(slabs.local_block(a2, P2, 1, 2)[0, :, 0], a2[0, 4:9, 0])   # rows 4..8: ghost 4, owned 5..8
 
 
+def test_layer_parts():
+    assert slabs.layer_parts(10, (1, 1)) == {"boundary": [(1, 1), (8, 1)], "interior": (2, 6)}
+    assert slabs.layer_parts(10, (0, 1)) == {"boundary": [(8, 1)], "interior": (0, 8)}          # physical face below
+    assert slabs.layer_parts(10, (1, 0)) == {"boundary": [(1, 1)], "interior": (2, 8)}
+    assert slabs.layer_parts(3, (1, 1)) == {"boundary": [(1, 1)], "interior": (2, 0)}           # one owned layer
+    assert slabs.layer_parts(4, (1, 1)) == {"boundary": [(1, 1), (2, 1)], "interior": (2, 0)}   # two owned layers
+    assert slabs.layer_parts(6, (0, 0)) == {"boundary": [], "interior": (0, 6)}
+    for n, halo in ((10, (1, 1)), (10, (0, 1)), (3, (1, 1)), (4, (1, 1)), (5, (1, 0)), (2, (0, 1))):   # every owned layer once
+        parts = slabs.layer_parts(n, halo)
+        got = sorted(l for f, c in parts["boundary"] + [parts["interior"]] for l in range(f, f + c))
+        assert got == list(range(halo[0], n - halo[1])), (n, halo, parts)
+
+
 class TaggedSlab:
     """Stand-in for slabs.Slab: one number per layer.  ``layers`` holds the global layer index of every local layer
     (ghosts start at -1); pack/unpack move [layer id, what, sender side] so that the test can see who sent what."""
@@ -72,6 +85,7 @@ class TaggedSlab:
         self.halo = (0 if lo is None else 1, 0 if hi is None else 1)
         self.layers = [-1] * self.halo[0] + list(range(start, start + count)) + [-1] * self.halo[1]
         self.seen = {}
+        self.log = []
         self._send = {w: {s: torch.zeros(3, dtype=torch.int64) for s in range(2) if self.halo[s]} for w in range(2)}
         self._recv = {w: {s: torch.zeros(3, dtype=torch.int64) for s in range(2) if self.halo[s]} for w in range(2)}
 
@@ -84,12 +98,20 @@ class TaggedSlab:
     def halo_pack(self, what, side, buf):
         owned = self.layers[1] if side == 0 else self.layers[-2]
         buf.copy_(torch.tensor([owned, what, side]))
+        self.log.append(("pack", what, side))
 
     def halo_unpack(self, what, side, buf):
         layer, w, sender_side = (int(v) for v in buf)
         assert w == what and sender_side == 1 - side
         self.layers[0 if side == 0 else -1] = layer
         self.seen[(what, side)] = layer
+        self.log.append(("unpack", what, side))
+
+    # overlapped schedule (slabs.step_overlapped): what ran, in host order
+    log = None
+
+    def run_part(self, phase, which, store_macros, last):
+        self.log.append(("part", phase, which, bool(store_macros), bool(last)))
 
 
 def _expected_layers(n_global, rank, world, periodic):
@@ -111,6 +133,60 @@ def test_exchange_local(world, periodic):
         slabs.exchange_local(S, what, periodic)
     for r, s in enumerate(S):
         assert s.layers == _expected_layers(n, r, world, periodic)
+
+
+def _expected_log(halo, nsteps):
+    """Host order of the overlapped schedule for one slab: boundary part, exchange, interior part -- per phase."""
+    sides = [s for s in range(2) if halo[s]]
+    out = []
+    for k in range(nsteps):
+        macro = k == nsteps - 1
+        for phase, what in ((0, slabs.HALO_PHI), (1, slabs.HALO_POPS)):
+            m = macro and phase == 1
+            out.append(("part", phase, "boundary", m, False))
+            out += [("pack", what, s) for s in sides] + [("unpack", what, s) for s in sides]
+            out.append(("part", phase, "interior", m, True))
+    return out
+
+
+@pytest.mark.parametrize("world,periodic", [(1, True), (3, True), (3, False)])
+def test_step_overlapped_local_order(world, periodic):
+    n = 11
+    S = [TaggedSlab(n, r, world, periodic) for r in range(world)]
+    slabs.step_overlapped(S, lambda what: slabs.exchange_local(S, what, periodic), slabs.NoStreams(), 2)
+    for r, s in enumerate(S):
+        assert s.layers == _expected_layers(n, r, world, periodic)
+        assert s.log == _expected_log(s.halo, 2), (r, s.log)
+
+
+def _worker_overlapped(rank, world, port, periodic, out):
+    os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    s = TaggedSlab(11, rank, world, periodic)
+    slabs.step_overlapped([s], lambda what: slabs.exchange_dist(s, what, rank, world, periodic), slabs.NoStreams(), 3)
+    out.put((rank, (s.layers, s.log == _expected_log(s.halo, 3))))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,periodic", [(2, True), (2, False), (3, True)])
+def test_step_overlapped_dist_gloo(world, periodic):
+    """The boundary-first schedule over torch.distributed (gloo): two exchanges per step between the parts of a phase, three
+    steps in a row -- messages of consecutive exchanges to the same peer must not cross-match (world 2, periodic: both
+    neighbours are the same rank)."""
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker_overlapped, args=(r, world, port, periodic, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = dict(out.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for r in range(world):
+        assert res[r][0] == _expected_layers(11, r, world, periodic), (r, res[r])
+        assert res[r][1], "rank %d: parts and exchanges out of order" % r
 
 
 def _free_port():
