@@ -30,6 +30,8 @@ CAC_MODIFIED_EQ = 0
 CAC_SOURCE = 1
 POPS_POSTCOLLISION = 0
 POPS_STREAMED = 1
+GRAD_SCHEMES = {"central": 0, "biased1": 1, "biased2": 2}
+DIV_SCHEMES = {"product": 0, "stencil": 1}                  # DESIGN.md readings S5 / S17
 
 
 class _Params(C.Structure):
@@ -46,6 +48,7 @@ class _Params(C.Structure):
         ("L_latent", C.c_double), ("Cp", C.c_double), ("T_sat", C.c_double), ("theta_I", C.c_double),
         ("A", C.c_double), ("eps_n", C.c_double),
         ("flags", C.c_uint),
+        ("grad_scheme", C.c_int), ("div_scheme", C.c_int),
     ]
 
 
@@ -75,6 +78,7 @@ def lib():
         L.oracle_read_macro.argtypes = [C.c_void_p, dp, dp, dp, dp]
         L.oracle_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
         L.oracle_read_aux.argtypes = [C.c_void_p, dp, dp, dp, dp]
+        L.oracle_read_div.argtypes = [C.c_void_p, dp]
         L.oracle_set_cac_form.argtypes = [C.c_void_p, C.c_int]
         L.oracle_set_velocity.argtypes = [C.c_void_p, dp]
         L.oracle_num_threads.restype = C.c_int
@@ -107,6 +111,8 @@ def fill_params(P: dict) -> _Params:
         s.force[a] = float(P.get("force", (0.0, 0.0, 0.0))[a])
     s.flags = (FLAG_PHASE_CHANGE if P["phase_change"] else 0) | (FLAG_LATENT_HEAT if P["latent_heat"] else 0) | (
         FLAG_PRESCRIBED_U if P.get("prescribed_u", False) else 0)
+    s.grad_scheme = GRAD_SCHEMES[P.get("grad_scheme", "central")]
+    s.div_scheme = DIV_SCHEMES[P.get("div_scheme", "product")]
     return s
 
 
@@ -187,6 +193,12 @@ class Oracle:
     def read_pops(self, which, stage=POPS_STREAMED):
         out = np.empty((self.Q[which],) + self.shape)
         assert lib().oracle_read_pops(self._h, int(which), int(stage), _ptr(out)) == 0
+        return out
+
+    def read_div(self):
+        """div(u phi) of the current level by the stencil (div_scheme "stencil" only)."""
+        out = np.empty(self.shape)
+        assert lib().oracle_read_div(self._h, _ptr(out)) == 0
         return out
 
     def read_aux(self):

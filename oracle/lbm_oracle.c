@@ -47,6 +47,8 @@ struct oracle_ctx {
     double *u_next;
     /* derived fields of phi at level n */
     double *grad, *lap;
+    /* ORA_DIV_STENCIL: div(u phi) at level n by the directional-derivative stencil (else NULL) */
+    double *divuphi;
 };
 
 /* ------------------------------------------------------------------------------------------------
@@ -160,6 +162,8 @@ oracle_ctx *oracle_create(const oracle_params *p)
     if (!(p->dx > 0) || !(p->dt > 0) || !(p->W > 0) || !(p->rho_l > 0) || !(p->rho_g > 0)) return NULL;
     if (!(p->nu_l > 0) || !(p->nu_g > 0) || !(p->M > 0) || !(p->alpha_l > 0) || !(p->alpha_g > 0)) return NULL;
     if (!(p->Cp > 0) || p->L_latent == 0.0 || !(p->A > 0)) return NULL;
+    if (p->grad_scheme < ORA_GRAD_CENTRAL || p->grad_scheme > ORA_GRAD_BIASED2) return NULL;
+    if (p->div_scheme < ORA_DIV_PRODUCT || p->div_scheme > ORA_DIV_STENCIL) return NULL;
     oracle_ctx *c = (oracle_ctx *)calloc(1, sizeof(*c));
     if (!c) return NULL;
     c->P = *p;
@@ -197,6 +201,10 @@ oracle_ctx *oracle_create(const oracle_params *p)
     c->pdot = (double *)calloc(N, sizeof(double));
     c->grad = (double *)calloc(3 * N, sizeof(double));
     c->lap = (double *)calloc(N, sizeof(double));
+    if (p->div_scheme == ORA_DIV_STENCIL) {
+        c->divuphi = (double *)calloc(N, sizeof(double));
+        if (!c->divuphi) { oracle_destroy(c); return NULL; }
+    }
     if (!c->f || !c->g || !c->s || !c->fpost || !c->gpost || !c->spost || !c->phi || !c->phi_prev ||
         !c->dtphi || !c->u || !c->p || !c->T || !c->pdot || !c->grad || !c->lap) {
         oracle_destroy(c); return NULL;
@@ -209,7 +217,7 @@ void oracle_destroy(oracle_ctx *c)
     if (!c) return;
     free(c->f); free(c->g); free(c->s); free(c->fpost); free(c->gpost); free(c->spost);
     free(c->phi); free(c->phi_prev); free(c->dtphi); free(c->u); free(c->p); free(c->T); free(c->pdot);
-    free(c->grad); free(c->lap); free(c->u_next);
+    free(c->grad); free(c->lap); free(c->u_next); free(c->divuphi);
     free(c);
 }
 
@@ -229,9 +237,10 @@ int oracle_set_velocity(oracle_ctx *c, const double *u)
 
 /* ------------------------------------------------------------------------------------------------
  * phi at a possibly out-of-domain position (reading S8-iv): the value a ghost layer filled axis by
- * axis (x, then y, then z) would hold.  Periodic axis: wrap.  Zero-flux face: mirror,
- * phi(-1) = phi(0).  Dirichlet face with value v (wall half a cell outside the first node):
- * phi(-1) = 2 v - phi(0).
+ * axis (x, then y, then z) would hold.  Periodic axis: wrap.  Zero-flux face: mirror in the wall, which
+ * sits half a cell outside the first node: phi(-1) = phi(0), phi(-2) = phi(1) (the second ghost layer is
+ * reached by the second-order biased difference only).  Dirichlet face with value v:
+ * phi(-1) = 2 v - phi(0), phi(-2) = 2 v - phi(1).
  * ---------------------------------------------------------------------------------------------- */
 static double phi_at(const oracle_ctx *c, const double *phi, int x, int y, int z)
 {
@@ -245,7 +254,7 @@ static double phi_at(const oracle_ctx *c, const double *phi, int x, int y, int z
         if (c->P.bc_g[a][side] == ORA_S_PERIODIC) {
             q[a] = ((q[a] % n) + n) % n;
         } else {
-            q[a] = side == 0 ? 0 : n - 1;
+            q[a] = side == 0 ? -1 - q[a] : 2 * n - 1 - q[a];
             kind[a] = c->P.bc_g[a][side];
             val[a] = c->P.bc_phi[a][side];
         }
@@ -257,7 +266,9 @@ static double phi_at(const oracle_ctx *c, const double *phi, int x, int y, int z
 }
 
 /* P1 -- directional-derivative gradient and Laplacian, Eq.(35a,b) and (36a,b), PAPER.md:291-315,
- * on the NS lattice's directions with the printed factor 3 read as 1/e2 (reading S2). */
+ * on the NS lattice's directions with the printed factor 3 read as 1/e2 (reading S2).
+ * The directional derivative inside Eq.(35b) is the central one, Eq.(35a), or one of the biased differences the paper
+ * defines at PAPER.md:318; the Laplacian is Eq.(36a,b) in every case. */
 static void pass_derive(oracle_ctx *c)
 {
     const lattice_t *L = &c->Lf;
@@ -274,6 +285,12 @@ static void pass_derive(oracle_ctx *c)
                     double php = phi_at(c, c->phi, x + L->e[i][0], y + L->e[i][1], z + L->e[i][2]);
                     double phm = phi_at(c, c->phi, x - L->e[i][0], y - L->e[i][1], z - L->e[i][2]);
                     double d1 = (php - phm) / (2.0 * dx);              /* Eq.(35a) */
+                    if (c->P.grad_scheme == ORA_GRAD_BIASED1) {
+                        d1 = (php - ph0) / dx;                         /* first-order biased */
+                    } else if (c->P.grad_scheme == ORA_GRAD_BIASED2) { /* second-order biased */
+                        double php2 = phi_at(c, c->phi, x + 2 * L->e[i][0], y + 2 * L->e[i][1], z + 2 * L->e[i][2]);
+                        d1 = (-php2 + 4.0 * php - 3.0 * ph0) / (2.0 * dx);
+                    }
                     double d2 = (php - 2.0 * ph0 + phm) / (dx * dx);   /* Eq.(36a) */
                     gx += L->w[i] * L->e[i][0] * d1;                   /* Eq.(35b) */
                     gy += L->w[i] * L->e[i][1] * d1;
@@ -285,6 +302,55 @@ static void pass_derive(oracle_ctx *c)
                 c->grad[N + n] = gy / L->e2;
                 c->grad[2 * N + n] = gz / L->e2;
                 c->lap[n] = lp / L->e2;
+            }
+}
+
+/* Velocity at a possibly out-of-domain position, for the stencil divergence (reading S17; the paper gives no rule).
+ * Periodic axis: wrap.  No-slip wall half a cell outside the first node: odd reflection, u(-1) = -u(0), so that the
+ * value interpolated on the wall is zero.  Open face: even reflection, u(-1) = u(0) (no normal gradient). */
+static double u_at(const oracle_ctx *c, int comp, int x, int y, int z)
+{
+    int q[3] = { x, y, z };
+    double sign = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        int n = axis_len(c, a);
+        if (q[a] >= 0 && q[a] < n) continue;
+        int side = q[a] < 0 ? 0 : 1;
+        if (c->P.bc_f[a][side] == ORA_F_PERIODIC) {
+            q[a] = ((q[a] % n) + n) % n;
+        } else {
+            q[a] = side == 0 ? -1 - q[a] : 2 * n - 1 - q[a];
+            if (c->P.bc_f[a][side] == ORA_F_WALL) sign = -sign;
+        }
+    }
+    return sign * c->u[(long)comp * c->N + idx(c, q[0], q[1], q[2])];
+}
+
+/* ORA_DIV_STENCIL -- div(u phi) of Eq.(33d),(34) with the paper's own difference operator: each
+ * d_a(u_a phi) by the directional derivatives Eq.(35a) assembled as in Eq.(35b), on the NS lattice,
+ *   div(u phi) = (1/e2) sum_i w_i sum_a e_ia [ (u_a phi)(x + e_i) - (u_a phi)(x - e_i) ] / (2 dx),
+ * from u and phi of the SAME level (reading S17).  The alternative to the product rule of reading S5. */
+static void pass_divergence(oracle_ctx *c)
+{
+    const lattice_t *L = &c->Lf;
+    const double dx = c->P.dx;
+    const int nx = c->P.nx, ny = c->P.ny, nz = c->P.nz;
+#pragma omp parallel for collapse(2)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                double d = 0.0;
+                for (int i = 1; i < L->Q; ++i) {
+                    int xp = x + L->e[i][0], yp = y + L->e[i][1], zp = z + L->e[i][2];
+                    int xm = x - L->e[i][0], ym = y - L->e[i][1], zm = z - L->e[i][2];
+                    double php = phi_at(c, c->phi, xp, yp, zp), phm = phi_at(c, c->phi, xm, ym, zm);
+                    for (int a = 0; a < 3; ++a) {
+                        if (!L->e[i][a]) continue;
+                        double dd = (u_at(c, a, xp, yp, zp) * php - u_at(c, a, xm, ym, zm) * phm) / (2.0 * dx);
+                        d += L->w[i] * L->e[i][a] * dd;
+                    }
+                }
+                c->divuphi[idx(c, x, y, z)] = d / L->e2;
             }
 }
 
@@ -348,6 +414,7 @@ static void node_eq_sources(const oracle_ctx *c, long n, node_terms *t)
     double mdot = P->rho_g * pdot;                                               /* mass production rate */
     /* div(u phi) = u.grad phi + phi div u with div u = mdot (1/rho_g - 1/rho_l), Eq.(11a) (reading S5) */
     double D = u[0] * grad[0] + u[1] * grad[1] + u[2] * grad[2] + phi * mdot * drho;
+    if (c->divuphi) D = c->divuphi[n];   /* ... or the stencil divergence of this level (reading S17) */
     /* relaxation rates: tau_bar = nu/(c_s^2 dt) PAPER.md:208, M/(c_s^2 dt) PAPER.md:236,
      * alpha/(c_s^2 dt) PAPER.md:272; om = 1/(tau_bar + 1/2), Eq.(25) */
     t->om[0] = 1.0 / (nu / (cs2f * dt) + 0.5);
@@ -485,20 +552,18 @@ static void pass_moments(oracle_ctx *c)
     }
     /* 3: derived fields of the new phi */
     pass_derive(c);
-    /* 4-8 */
+    /* 4: rho u = (1/c_s^2) sum f c_i + dt/2 F_tot, Eq.(28a) PAPER.md:224 -- for every node before any of 5-8, because the
+     * stencil divergence (ORA_DIV_STENCIL) reads the neighbours' new velocity */
 #pragma omp parallel for
     for (long n = 0; n < N; ++n) {
         double phi = c->phi[n];
         double grad[3] = { c->grad[n], c->grad[N + n], c->grad[2 * N + n] };
         double rho = phi * P->rho_g + (1.0 - phi) * P->rho_l;
-        double F[3], grho[3], u[3];
+        double F[3], u[3];
         total_force(c, phi, grad, c->lap[n], rho, F);
-        for (int a = 0; a < 3; ++a) grho[a] = (P->rho_g - P->rho_l) * grad[a];
-        /* 4: rho u = (1/c_s^2) sum f c_i + dt/2 F_tot, Eq.(28a) */
-        double m0 = 0.0, m1[3] = { 0, 0, 0 };
+        double m1[3] = { 0, 0, 0 };
         for (int i = 0; i < c->Lf.Q; ++i) {
             double fi = c->f[(long)i * N + n];
-            m0 += fi;
             for (int a = 0; a < 3; ++a) m1[a] += fi * cc * c->Lf.e[i][a];
         }
         for (int a = 0; a < 3; ++a) u[a] = (m1[a] / cs2f + 0.5 * dt * F[a]) / rho;
@@ -507,9 +572,24 @@ static void pass_moments(oracle_ctx *c)
             const double *up = c->u_next ? c->u_next : c->u;   /* u(x, t^{n+1}) */
             for (int a = 0; a < 3; ++a) u[a] = up[(long)a * N + n];
         }
+        for (int a = 0; a < 3; ++a) c->u[(long)a * N + n] = u[a];
+    }
+    if (c->divuphi) pass_divergence(c);   /* div(u^{n+1} phi^{n+1}) by the stencil (reading S17) */
+    /* 5-8 */
+#pragma omp parallel for
+    for (long n = 0; n < N; ++n) {
+        double phi = c->phi[n];
+        double grad[3] = { c->grad[n], c->grad[N + n], c->grad[2 * N + n] };
+        double rho = phi * P->rho_g + (1.0 - phi) * P->rho_l;
+        double grho[3], u[3];
+        for (int a = 0; a < 3; ++a) grho[a] = (P->rho_g - P->rho_l) * grad[a];
+        for (int a = 0; a < 3; ++a) u[a] = c->u[(long)a * N + n];
+        double m0 = 0.0;
+        for (int i = 0; i < c->Lf.Q; ++i) m0 += c->f[(long)i * N + n];
         /* 5: m''' from the stored Pdot; D = div(u phi) (S5) */
         double mdot = P->rho_g * c->pdot[n];
         double D = u[0] * grad[0] + u[1] * grad[1] + u[2] * grad[2] + phi * mdot * drho;
+        if (c->divuphi) D = c->divuphi[n];
         /* 6: T = sum s - dt/2 (L/Cp) [dphi/dt + div(u phi)], Eq.(34) */
         double T = 0.0;
         for (int i = 0; i < c->Ls.Q; ++i) T += c->s[(long)i * N + n];
@@ -517,7 +597,6 @@ static void pass_moments(oracle_ctx *c)
         /* 7: p = sum f + dt/2 { c_s^2 u.grad rho + rho c_s^2 m''' (1/rho_g - 1/rho_l) }, Eq.(28b) */
         double ugr = u[0] * grho[0] + u[1] * grho[1] + u[2] * grho[2];
         double p = m0 + 0.5 * dt * (cs2f * ugr + rho * cs2f * mdot * drho);
-        for (int a = 0; a < 3; ++a) c->u[(long)a * N + n] = u[a];
         c->T[n] = T;
         c->p[n] = p;
         /* 8: refresh the production field with the new macros, Eq.(18) */
@@ -544,6 +623,7 @@ int oracle_init(oracle_ctx *c, const double *phi, const double *T, const double 
     }
     c->nsteps = 0;
     pass_derive(c);
+    if (c->divuphi) pass_divergence(c);
     const lattice_t *Ls[3] = { &c->Lf, &c->Lg, &c->Ls };
     double *pops[3] = { c->f, c->g, c->s };
 #pragma omp parallel for
@@ -595,6 +675,13 @@ int oracle_read_pops(oracle_ctx *c, int which, int stage, double *out)
         src = which == 0 ? c->fpost : (which == 1 ? c->gpost : c->spost);
     }
     memcpy(out, src, (size_t)L->Q * c->N * sizeof(double));
+    return 0;
+}
+
+int oracle_read_div(oracle_ctx *c, double *div)
+{
+    if (!c || !div || !c->divuphi) return -1;
+    memcpy(div, c->divuphi, (size_t)c->N * sizeof(double));
     return 0;
 }
 

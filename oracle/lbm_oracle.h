@@ -43,6 +43,12 @@ enum { ORA_PHASE_CHANGE = 1u /* Eq.(18) production rate on */,
        ORA_PRESCRIBED_U = 4u /* u is the field given to oracle_init and is not updated from f */ };
 /* conservative Allen-Cahn collision form */
 enum { ORA_CAC_MODIFIED_EQ = 0 /* Eq.(31a,b) */, ORA_CAC_SOURCE = 1 /* Eq.(29a,b),(30a,b) */ };
+/* directional derivative e_i.grad(phi) used in the gradient Eq.(35b): central Eq.(35a), or the biased differences of
+ * first order [phi(x+e) - phi(x)]/dx, second order [-phi(x+2e) + 4 phi(x+e) - 3 phi(x)]/(2 dx) */
+enum { ORA_GRAD_CENTRAL = 0, ORA_GRAD_BIASED1 = 1, ORA_GRAD_BIASED2 = 2 };
+/* div(u phi) of Eq.(33d),(34): product rule u.grad(phi) + phi div u with Eq.(11a) (reading S5), or the directional-derivative
+ * stencil Eq.(35a,b) applied to the components of u phi (reading S17) */
+enum { ORA_DIV_PRODUCT = 0, ORA_DIV_STENCIL = 1 };
 /* stage selector of oracle_read_pops */
 enum { ORA_POPS_POSTCOLLISION = 0, ORA_POPS_STREAMED = 1 };
 
@@ -65,6 +71,8 @@ typedef struct oracle_params {
     double A;                     /* script-A of Eq.(18); 10/48 in the paper      */
     double eps_n;                 /* regularisation of n = grad phi / |grad phi| (reading S7)    */
     unsigned flags;
+    int grad_scheme;              /* ORA_GRAD_*: directional derivative inside Eq.(35b) */
+    int div_scheme;               /* ORA_DIV_*: discretisation of div(u phi)                          */
 } oracle_params;
 
 typedef struct oracle_ctx oracle_ctx;
@@ -80,6 +88,8 @@ int oracle_read_macro(oracle_ctx *c, double *phi, double *u, double *p, double *
 int oracle_read_pops(oracle_ctx *c, int which, int stage, double *out);
 /* auxiliary fields for the pins: grad phi [3][N], laplacian [N], production rate Pdot [N], dphi/dt [N] */
 int oracle_read_aux(oracle_ctx *c, double *grad, double *lap, double *pdot, double *dtphi);
+/* ORA_DIV_STENCIL only: the stencil divergence of (u phi) at the current level [N] */
+int oracle_read_div(oracle_ctx *c, double *div);
 void oracle_set_cac_form(oracle_ctx *c, int form);
 /* ORA_PRESCRIBED_U only: u [3][z][y][x] of the next time level (time-dependent prescribed velocity) */
 int oracle_set_velocity(oracle_ctx *c, const double *u);

@@ -47,30 +47,57 @@ class NPModel:
         self.H = 12.0 * P["sigma"] / P["W"]
         self.c = P["dx"] / P["dt"]
 
-    # ---- ghost-padded phi (axis order x, y, z; array axes are (z, y, x)) -------------------------------
-    def _pad_phi(self, phi):
+    # ---- ghost-padded fields (axis order x, y, z; array axes are (z, y, x)) ----------------------------
+    @staticmethod
+    def _ghosts(a, ax, depth, periodic):
+        """(low ghosts, high ghosts) of array a along axis ax: periodic images, or mirror images in the faces (which sit
+        half a cell outside the first / last node: ghost -1 <-> node 0, ghost -2 <-> node 1)."""
+        n = a.shape[ax]
+        if periodic:     # (modular: a 2D grid is one periodic layer thick in z)
+            return (np.take(a, [k % n for k in range(-depth, 0)], axis=ax),
+                    np.take(a, [k % n for k in range(n, n + depth)], axis=ax))
+        first = np.take(a, range(depth), axis=ax)
+        last = np.take(a, range(n - depth, n), axis=ax)
+        return np.flip(first, axis=ax), np.flip(last, axis=ax)
+
+    def _pad_phi(self, phi, depth=1):
         P = self.P
         a = phi
         for axis_phys, ax in ((0, 2), (1, 1), (2, 0)):
             kinds = P["bc_g"][axis_phys]
-            lo = np.take(a, [0], axis=ax)
-            hi = np.take(a, [-1], axis=ax)
-            if kinds[0] == "periodic":
-                glo, ghi = hi, lo
-            else:
-                glo = lo if kinds[0] == "zeroflux" else 2.0 * P["bc_phi"][axis_phys][0] - lo
-                ghi = hi if kinds[1] == "zeroflux" else 2.0 * P["bc_phi"][axis_phys][1] - hi
+            glo, ghi = self._ghosts(a, ax, depth, kinds[0] == "periodic")
+            if kinds[0] == "dirichlet":
+                glo = 2.0 * P["bc_phi"][axis_phys][0] - glo
+            if kinds[1] == "dirichlet":
+                ghi = 2.0 * P["bc_phi"][axis_phys][1] - ghi
+            a = np.concatenate([glo, a, ghi], axis=ax)
+        return a
+
+    def _pad_u(self, ua):
+        """One velocity component with one ghost layer (reading S17): periodic image; no-slip wall: odd reflection (zero on
+        the wall); open face: even reflection."""
+        P = self.P
+        a = ua
+        for axis_phys, ax in ((0, 2), (1, 1), (2, 0)):
+            kinds = P["bc_f"][axis_phys]
+            glo, ghi = self._ghosts(a, ax, 1, kinds[0] == "periodic")
+            if kinds[0] == "wall":
+                glo = -glo
+            if kinds[1] == "wall":
+                ghi = -ghi
             a = np.concatenate([glo, a, ghi], axis=ax)
         return a
 
     def derive(self, phi):
-        """grad phi Eq.(35a,b), lap phi Eq.(36a,b) on the NS lattice."""
+        """grad phi Eq.(35a,b), lap phi Eq.(36a,b) on the NS lattice; the directional derivative inside
+        Eq.(35b) central (35a) or one of the biased differences of PAPER.md:318."""
         P = self.P
         nz, ny, nx = self.shape
-        pad = self._pad_phi(phi)
+        scheme = P.get("grad_scheme", "central")
+        pad = self._pad_phi(phi, 2)
 
         def sh(v):
-            return pad[1 + v[2]:1 + v[2] + nz, 1 + v[1]:1 + v[1] + ny, 1 + v[0]:1 + v[0] + nx]
+            return pad[2 + v[2]:2 + v[2] + nz, 2 + v[1]:2 + v[1] + ny, 2 + v[0]:2 + v[0] + nx]
 
         grad = np.zeros((3,) + self.shape)
         lap = np.zeros(self.shape)
@@ -78,11 +105,31 @@ class NPModel:
             if not v.any():
                 continue
             plus, minus = sh(v), sh(-v)
-            dd = (plus - minus) / (2 * P["dx"])
+            if scheme == "central":
+                dd = (plus - minus) / (2 * P["dx"])
+            elif scheme == "biased1":
+                dd = (plus - phi) / P["dx"]
+            else:
+                dd = (4 * plus - sh(2 * v) - 3 * phi) / (2 * P["dx"])
             for a in range(3):
                 grad[a] += w * v[a] * dd
             lap += w * (plus - 2 * phi + minus) / P["dx"] ** 2
         return grad / self.e2f, lap / self.e2f
+
+    def div_uphi(self, u, phi, grad, mdot):
+        """div(u phi): product rule with Eq.(11a) (reading S5) or the directional-derivative stencil on u phi (S17)."""
+        P = self.P
+        if P.get("div_scheme", "product") == "product":
+            return (u * grad).sum(axis=0) + phi * mdot * (1 / P["rho_g"] - 1 / P["rho_l"])
+        nz, ny, nx = self.shape
+        pphi = self._pad_phi(phi, 1)
+        flux = [self._pad_u(u[a]) * pphi for a in range(3)]
+        D = np.zeros(self.shape)
+        for v, w in zip(self.ef, self.wf):
+            for a in range(3):
+                if v[a]:
+                    D += w * v[a] * flux[a][1 + v[2]:1 + v[2] + nz, 1 + v[1]:1 + v[1] + ny, 1 + v[0]:1 + v[0] + nx]
+        return D / (self.e2f * P["dx"])
 
     def pdot_of(self, phi, T):
         P = self.P
@@ -119,7 +166,7 @@ class NPModel:
         nrm = grad / np.sqrt((grad ** 2).sum(axis=0) + P["eps_n"] ** 2)
         drho = 1 / P["rho_g"] - 1 / P["rho_l"]
         mdot = P["rho_g"] * self.pdot
-        D = (u * grad).sum(axis=0) + phi * mdot * drho
+        D = self.div_uphi(u, phi, grad, mdot)
         out = {}
         # NS
         cs2 = self.e2f * c * c
@@ -214,7 +261,7 @@ class NPModel:
                 self.u = (m1 / cs2 + 0.5 * dt * F) / rho                                           # Eq.(28a)
             drho = 1 / P["rho_g"] - 1 / P["rho_l"]
             mdot = P["rho_g"] * self.pdot
-            D = (self.u * self.grad).sum(axis=0) + self.phi * mdot * drho
+            D = self.div_uphi(self.u, self.phi, self.grad, mdot)
             self.T = self.pops["s"].sum(axis=0)
             if P["latent_heat"]:
                 self.T = self.T - 0.5 * dt * (P["L_latent"] / P["Cp"]) * (self.dtphi + D)          # Eq.(34)
