@@ -422,3 +422,60 @@ def test_open_face_hydrostatic_column(oracle_mod):
     assert np.abs(exact).max() > 5e-3
     assert np.abs(p[0] - exact[None, :]).max() < 1e-6
     assert np.abs(u).max() < 1e-6
+
+
+def test_flat_interface_3d_d3q7_keeps_its_width(oracle_mod):
+    """3D, g on the paper's D3Q7 lattice (e2 = 1/4): the equilibrium profile of Eq.(5) balances the diffusive
+    flux M grad(phi), whose coefficient the LBM realises as tau_bar_g c_s^2 dt, against the counter term
+    M (4/W) phi (1 - phi) n of Eq.(31b), which carries 1/c_s^2 explicitly.  If the two disagreed about c_s^2
+    (1/3 typed for 1/4 in either place) the interface would settle at 3/4 or 4/3 of W.  Fit: atanh(2 phi - 1) = 2 (z - z0)/W_eff.
+    The discrete profile is wider than W by O((dx/W)^2): measured W_eff/W = 1.025 at W = 4, 1.011 at W = 6 (used here)."""
+    nz, W = 64, 6.0
+    P = wl.base_params(4, 4, nz, phase_change=False, latent_heat=False, W=W)
+    assert P["lat_g"] == "D3Q7"
+    z = np.arange(nz) + 0.5
+    prof = 0.5 * (np.tanh(2 * (z - 16) / W) - np.tanh(2 * (z - 48) / W))
+    phi0 = np.tile(prof[:, None, None], (1, 4, 4))
+    o = oracle_mod.Oracle(P)
+    o.init(phi0)
+    o.step(2000)
+    phi, u, _, _ = o.read_macro()
+    o.close()
+    col = phi[:32, 0, 0]
+    m = (col > 0.1) & (col < 0.9)
+    slope, _ = np.polyfit(z[:32][m], np.arctanh(2 * col[m] - 1), 1)
+    assert abs((2 / slope) / W - 1) < 0.02, 2 / slope
+    assert abs(_interface(col, True) - 16.0) < 1e-3 and np.abs(u).max() < 1e-7
+    assert np.abs(phi - phi[:, :1, :1]).max() < 1e-14          # stays plane
+
+
+def test_phi_ghost_beyond_a_dirichlet_face_is_2v_minus_mirror(oracle_mod):
+    """Reading S8-iv: the ghost value of phi beyond a Dirichlet face (the paper's Stefan set-up and top wall: phi = 1 | 0,
+    PAPER.md:486, 520) is 2 v - phi(mirror), so that phi = v ON the face, half a cell outside the first node.  A profile that
+    is linear through the face value then has the exact gradient at the wall node; with ghost = mirror (the zero-flux
+    rule) the wall node would see half of it, and the Laplacian there would not vanish."""
+    P = wl.base_params(6, 12, 1, phase_change=False, latent_heat=False)
+    P["bc_f"][1] = ["wall", "wall"]; P["bc_g"][1] = ["dirichlet", "dirichlet"]; P["bc_s"][1] = ["zeroflux", "zeroflux"]
+    P["bc_phi"][1] = [1.0, 0.0]
+    y = (np.arange(12) + .5)[None, :, None] + np.zeros((1, 1, 6))
+    o = oracle_mod.Oracle(P)
+    o.init(1.0 - y / 12)
+    grad, lap, _, _ = o.read_aux()
+    o.close()
+    assert np.abs(grad[1] + 1 / 12).max() < 1e-15 and np.abs(grad[0]).max() < 1e-15 and np.abs(lap).max() < 1e-14
+
+
+def test_dirichlet_anti_bounce_back_linear_profile_3d_d3q7(oracle_mod):
+    """P9 in 3D on the D3Q7 heat lattice (w = 1/8, e2 = 1/4): steady T between two anti-bounce-back faces s_i = -s*_ibar +
+    2 w_i T_face is linear with the faces half a cell outside the end nodes.  Catches the 2D weight typed
+    into the 3D rule and a face placed on the node."""
+    P = wl.base_params(4, 4, 16, phase_change=False, latent_heat=False)
+    P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]
+    P["bc_s"][2] = ["dirichlet", "dirichlet"]; P["bc_T"][2] = [1.0, 0.25]
+    o = oracle_mod.Oracle(P)
+    o.init(np.zeros((16, 4, 4)), np.zeros((16, 4, 4)))
+    o.step(30000)
+    T = o.read_macro()[3][:, 0, 0]
+    o.close()
+    z = np.arange(16) + 0.5
+    assert np.abs(T - (1.0 + (0.25 - 1.0) * z / 16)).max() < 1e-9
