@@ -51,6 +51,18 @@ enum {
     LBM_S_DIRICHLET = 2 /* anti-bounce-back s_i = -s*_ibar + 2 w_i value */
 };
 
+/* Model variants the paper defines beside the scheme it runs.  Both default to 0 = the paper's scheme;
+ * a non-zero value runs the step on the plain direct kernel (parity-tested, not tuned) and stores u, p, T every step.
+ * grad_scheme: directional derivative e_i.grad(phi) inside the gradient Eq.(35b): central Eq.(35a), or the biased differences
+ *   of PAPER.md:318, first order [phi(x+e) - phi(x)]/dx (assembled over all directions it equals the central gradient up to
+ *   rounding) and second order [-phi(x+2e) + 4 phi(x+e) - 3 phi(x)]/(2 dx).  The Laplacian stays Eq.(36).
+ * div_scheme: div(u phi) of Eq.(33d),(34): product rule u.grad(phi) + phi mdot (1/rho_g - 1/rho_l), mdot the mass production rate
+ *   (reading S5), or Eq.(35a,b) applied to the components of u phi with u and phi of the same level (reading S17:
+ *   one more pass per step for the velocity; ghost velocity odd in no-slip walls, even in open faces).
+ * Not available on slab contexts (halo) -- the ghost layers are one deep. */
+enum { LBM_GRAD_CENTRAL = 0, LBM_GRAD_BIASED1 = 1, LBM_GRAD_BIASED2 = 2 };
+enum { LBM_DIV_PRODUCT = 0, LBM_DIV_STENCIL = 1 };
+
 /* flags */
 #define LBM_FLAG_PHASE_CHANGE 1u /* production rate Eq.(18) on (otherwise m''' = 0)        */
 #define LBM_FLAG_LATENT_HEAT 2u  /* source of the heat equation Eq.(33c,d),(34) on          */
@@ -123,6 +135,8 @@ typedef struct lbm_params {
     double eps_n;           /* n = grad phi / sqrt(|grad phi|^2 + eps_n^2) (reading S7)   */
     unsigned flags;         /* LBM_FLAG_*                                                           */
     int halo[2];            /* ghost layer on the low / high side of the slowest axis (0 or 1)      */
+    int grad_scheme;        /* LBM_GRAD_*                                              */
+    int div_scheme;         /* LBM_DIV_*                                                             */
 } lbm_params;
 
 typedef struct lbm_ctx lbm_ctx;
@@ -194,6 +208,15 @@ int lbm_set_stream(lbm_ctx *c, void *cuda_stream);
 int lbm_halo_bytes(const lbm_ctx *c, int what, size_t *bytes);
 int lbm_halo_pack(lbm_ctx *c, int what, int side, void *d_buf);
 int lbm_halo_unpack(lbm_ctx *c, int what, int side, const void *d_buf);
+
+/* Schedule of lbm_step on 3D fp64 contexts (elsewhere LBM_E_UNSUPPORTED unless chunk_layers == 0).  chunk_layers > 0: K_phi and
+ * K_main alternate over chunks of that many z-layers, K_phi one chunk ahead, so that the g* lines and the phi^{n+1} layers K_phi
+ * touched are still in L2 when K_main reads them (the paper's own fusion / traffic trade-off).
+ * hints: L2 eviction priority of those launches, two bits each (0 normal, 1 evict-first, 2 evict-last): bits 0-1 K_main's
+ * streamed reads (f, s, Pdot, phi^n), 2-3 its read of g, 4-5 its stores, 6-7 K_phi's reads of g, 8-9 its phi store; bit 16: K_phi
+ * launched programmatically behind K_main.  chunk_layers == 0: two launches over the whole grid (the default).  Changes speed,
+ * never results. */
+int lbm_set_schedule(lbm_ctx *c, int chunk_layers, unsigned hints);
 
 /* Copy the macroscopic fields of the current time level to HOST arrays; any pointer may be NULL.
  * h_u is [3][z][y][x].  Synchronises. */

@@ -18,6 +18,8 @@ LATTICES = {"D2Q5": 0, "D2Q9": 1, "D3Q7": 2, "D3Q19": 3, "D3Q15": 4}
 LATTICE_Q = {"D2Q5": 5, "D2Q9": 9, "D3Q7": 7, "D3Q19": 19, "D3Q15": 15}
 F_KINDS = {"periodic": 0, "wall": 1, "open": 2}
 S_KINDS = {"periodic": 0, "zeroflux": 1, "dirichlet": 2}
+GRAD_SCHEMES = {"central": 0, "biased1": 1, "biased2": 2}   # lbm_params.grad_scheme (LBM_GRAD_*)
+DIV_SCHEMES = {"product": 0, "stencil": 1}                  # lbm_params.div_scheme (LBM_DIV_*)
 FLAG_PHASE_CHANGE = 1
 FLAG_LATENT_HEAT = 2
 FLAG_PRESCRIBED_U = 4
@@ -30,7 +32,7 @@ STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1
 NOALLOC_SCRATCH_BYTES = 8 << 20
 
-EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_set_schedule", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
            "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
@@ -52,6 +54,7 @@ class lbm_params(C.Structure):
         ("A", C.c_double), ("eps_n", C.c_double),
         ("flags", C.c_uint),
         ("halo", C.c_int * 2),
+        ("grad_scheme", C.c_int), ("div_scheme", C.c_int),
     ]
 
 
@@ -86,6 +89,7 @@ def load_library():
         L.lbm_read_pops_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_sync.argtypes = [C.c_void_p]
         L.lbm_set_timing.argtypes = [C.c_void_p, C.c_int]
+        L.lbm_set_schedule.argtypes = [C.c_void_p, C.c_int, C.c_uint]
         L.lbm_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.lbm_step_count.restype = C.c_longlong
         L.lbm_step_count.argtypes = [C.c_void_p]
@@ -125,6 +129,8 @@ def make_params(P: dict, precision: int = 64) -> lbm_params:
         s.flags |= KERNEL_FLAGS[name]
     halo = P.get("halo", (0, 0))
     s.halo[0], s.halo[1] = int(halo[0]), int(halo[1])
+    s.grad_scheme = GRAD_SCHEMES[P.get("grad_scheme", "central")]     # model variants (include/lbm.h)
+    s.div_scheme = DIV_SCHEMES[P.get("div_scheme", "product")]
     return s
 
 
@@ -281,6 +287,10 @@ class LBM:
     def stream(self):
         """The torch.cuda.Stream every kernel and copy of this context is enqueued on (record timing events there)."""
         return self._stream
+
+    def set_schedule(self, chunk_layers: int, hints: int = 0):
+        """lbm_set_schedule: K_phi / K_main alternate over chunks of z-layers (3D fp64); 0 = two launches over the whole grid."""
+        _check(self._L.lbm_set_schedule(self._h, int(chunk_layers), int(hints)), "lbm_set_schedule")
 
     def set_timing(self, enable: bool):
         _check(self._L.lbm_set_timing(self._h, 1 if enable else 0), "lbm_set_timing")

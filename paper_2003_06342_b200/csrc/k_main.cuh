@@ -41,6 +41,30 @@ template <class LF, class LG, class LS, class real, bool BC, class Fields = DevF
     template <int I, bool AGAIN = false> __device__ __forceinline__ real f() const { return pull_one<LF, I, real, BC, AGAIN>(Fd.f_in, (unsigned)P.N, g, P.bc_f, P.bc_p); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real s() const { return pull_one<LS, I, real, BC, AGAIN>(Fd.s_in, (unsigned)P.N, g, P.bc_s, P.bc_T); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real gg() const { return pull_one<LG, I, real, BC, AGAIN>(Fd.g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi); }
+    template <class sreal, class wreal> __device__ __forceinline__ void st(sreal *p, wreal v) const { st_pop(p, v); }
+    // ---- variant modes only ----
+    // phi^{n+1} up to two nodes away (second neighbour of the second-order biased difference), with the ghost
+    // rule of reading S8-iv carried two layers deep: periodic image; zero-flux mirror; Dirichlet 2 v - mirror
+    __device__ __forceinline__ preal phi_far(int dx, int dy, int dz) const {
+        int q[3] = {g.x + dx, g.y + dy, g.z + dz}, cross[3];
+        ghost_source(P, P.bc_g, q, cross);
+        preal v = __ldg(Fd.phi_new + ((unsigned)(q[2] + P.pz) * (unsigned)P.ppy + (unsigned)(q[1] + 1)) * (unsigned)P.ppx + (unsigned)(q[0] + P.xpad));
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            if (cross[a] && P.bc_g[a][cross[a] - 1] == BC_ANTI) v = preal(2) * preal(P.bc_phi[a][cross[a] - 1]) - v;
+        return v;
+    }
+    // component `comp` of the velocity array at a neighbour (stencil divergence, reading S17): periodic image; odd
+    // reflection in a no-slip wall (zero on the wall); even reflection in an open face
+    __device__ __forceinline__ real u_nb(int comp, int dx, int dy, int dz) const {
+        int q[3] = {g.x + dx, g.y + dy, g.z + dz}, cross[3];
+        ghost_source(P, P.bc_f, q, cross);
+        real v = real(Fd.u[(unsigned)comp * (unsigned)P.N + ((unsigned)q[2] * (unsigned)P.ny + (unsigned)q[1]) * (unsigned)P.nx + (unsigned)q[0]]);
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            if (cross[a] && P.bc_f[a][cross[a] - 1] == BC_BOUNCE) v = -v;
+        return v;
+    }
 };
 
 template <class LF, class LG, class LS, class real, int MODE, class Src, class Fields>
@@ -69,7 +93,15 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
         if constexpr (I > 0 && I < LF::opp(I)) {
             constexpr int ex = LF::ex(I), ey = LF::ey(I), ez = LF::ez(I);
             const preal pp = src.phi(ex, ey, ez), pm = src.phi(-ex, -ey, -ez);
-            const real d = real(pp - pm);
+            real d = real(pp - pm);   // central difference Eq.(35a), the pair (e, -e) at once
+            if constexpr (mode_has_variants<MODE>::value) {
+                // biased differences of PAPER.md:318 inside Eq.(35b), again both directions of the pair
+                if (P.grad_scheme == 1) d = real((pp - phi_p) - (pm - phi_p));
+                else if (P.grad_scheme == 2) {
+                    const preal pp2 = src.phi_far(2 * ex, 2 * ey, 2 * ez), pm2 = src.phi_far(-2 * ex, -2 * ey, -2 * ez);
+                    d = real(preal(0.5) * ((preal(4) * pp - pp2 - preal(3) * phi_p) - (preal(4) * pm - pm2 - preal(3) * phi_p)));
+                }
+            }
             constexpr real w = real(LF::w(I));
             if constexpr (ex != 0) gx += (ex > 0 ? w : -w) * d;
             if constexpr (ey != 0) gy += (ey > 0 ? w : -w) * d;
@@ -104,6 +136,28 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     const real om_f = den * (rall * rds);
     const real om_s = rall * (rho * df);
 
+    // variant modes, div_scheme = stencil: div(u phi) by Eq.(35a,b) on the components of u phi, from the velocity ARRAY
+    // (this level's u of every node: the input at initialisation, written by the MODE_U pass before a step) -- reading S17
+    real D_st = real(0);
+    bool use_st = false;
+    if constexpr (MODE == MODE_INIT || MODE == MODE_STEP_VAR) {
+        if (P.div_scheme) {
+            use_st = true;
+            static_for<LF::Q>([&](auto ic) {
+                constexpr int I = decltype(ic)::value;
+                if constexpr (I > 0 && I < LF::opp(I)) {
+                    constexpr int ex = LF::ex(I), ey = LF::ey(I), ez = LF::ez(I);
+                    real up = real(0), um = real(0);
+                    if constexpr (ex != 0) { up += real(ex) * src.u_nb(0, ex, ey, ez); um += real(ex) * src.u_nb(0, -ex, -ey, -ez); }
+                    if constexpr (ey != 0) { up += real(ey) * src.u_nb(1, ex, ey, ez); um += real(ey) * src.u_nb(1, -ex, -ey, -ez); }
+                    if constexpr (ez != 0) { up += real(ez) * src.u_nb(2, ex, ey, ez); um += real(ez) * src.u_nb(2, -ex, -ey, -ez); }
+                    D_st += real(LF::w(I)) * (up * real(src.phi(ex, ey, ez)) - um * real(src.phi(-ex, -ey, -ez)));
+                }
+            });
+            D_st *= P.inv_dx * real(1.0 / LF::e2);
+        }
+    }
+
     real ux, uy, uz, p, T, dtphi;
     real pd_old = real(0);   // production rate of the previous level: in the moment corrections and folded into the stored g_0
     if constexpr (MODE == MODE_INIT) {
@@ -128,11 +182,21 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
         if constexpr (MODE == MODE_STEP_PU) {   // Zalesak / vortex verifications: u is the field given at init
             ux = real(Fd.u[n]); uy = real(Fd.u[N + n]); uz = (LF::D == 3) ? real(Fd.u[2 * N + n]) : real(0);
         }
+        if constexpr (MODE == MODE_U) {         // velocity pass: u^{n+1} of this node for its neighbours' stencil divergence
+            Fd.u[n] = sreal(ux); Fd.u[N + n] = sreal(uy);
+            if constexpr (LF::D == 3) Fd.u[2 * N + n] = sreal(uz);
+            return;
+        }
+        if constexpr (MODE == MODE_STEP_VAR) {  // prescribed, or already in the array (the value the neighbours saw)
+            if (P.prescribed_u || P.div_scheme) {
+                ux = real(Fd.u[n]); uy = real(Fd.u[N + n]); uz = (LF::D == 3) ? real(Fd.u[2 * N + n]) : real(0);
+            }
+        }
         // ---- H1 (time derivative), H5: heat moment with the STORED production rate (reading S3; Eq.34)
         dtphi = real(phi_p - src.phi_old()) * P.inv_dt;                              // reading S4
         pd_old = src.pdot_old();
         const real mdot_old = P.rho_g * pd_old;
-        const real D_old = ux * gx + uy * gy + uz * gz + phi * mdot_old * P.drho;   // reading S5
+        const real D_old = use_st ? D_st : ux * gx + uy * gy + uz * gz + phi * mdot_old * P.drho;   // reading S5 (or S17)
         T = sum_s;
         if (P.latent_heat) T -= P.hdt * P.LCp * (dtphi + D_old);
         // pressure (Eq.28b)
@@ -152,11 +216,15 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
         Fd.p[n] = sreal(p); Fd.T[n] = sreal(T);
     }
     if constexpr (MODE == MODE_STEP_PU) { Fd.p[n] = sreal(p); Fd.T[n] = sreal(T); }
+    if constexpr (MODE == MODE_STEP_VAR) {
+        Fd.p[n] = sreal(p); Fd.T[n] = sreal(T);
+        if (!(P.prescribed_u || P.div_scheme)) { Fd.u[n] = sreal(ux); Fd.u[N + n] = sreal(uy); Fd.u[2 * N + n] = sreal(uz); }
+    }
 
     // ---- H7: sources, equilibria, BGK (Eq.25)
     const real mdot = P.rho_g * pdot;
     const real ug = ux * gx + uy * gy + uz * gz;
-    const real D = ug + phi * mdot * P.drho;
+    const real D = use_st ? D_st : ug + phi * mdot * P.drho;
     const real uu = ux * ux + uy * uy + uz * uz;
 
     // BGK with the source shift folded in: out_i = a bar_i + om eq_i + b S_i, with (a, om, b) = (1-om, om, dt(1-om/2)),
@@ -186,7 +254,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
             constexpr real w = real(LF::w(0));
             real bar = real(0);
             if constexpr (MODE != MODE_INIT) bar = src.template f<0, true>();
-            st_pop(Fd.f_out + (n), a * bar + w * (U * K1 + K2));
+            src.st(Fd.f_out + (n), a * bar + w * (U * K1 + K2));
         }
         static_for<LF::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
@@ -199,8 +267,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
                 const real q = real(0.5) * t * t + U;
                 const real h = dot_e<LF, I, real>(Hbx, Hby, Hbz);
                 const real fb = dot_e<LF, I, real>(Fbx, Fby, Fbz);
-                st_pop(Fd.f_out + ((unsigned)I * N + n), a * bi + w * ((q + t) * (K1 + h) + (K2 + fb)));
-                st_pop(Fd.f_out + ((unsigned)J * N + n), a * bj + w * ((q - t) * (K1 - h) + (K2 - fb)));
+                src.st(Fd.f_out + ((unsigned)I * N + n), a * bi + w * ((q + t) * (K1 + h) + (K2 + fb)));
+                src.st(Fd.f_out + ((unsigned)J * N + n), a * bj + w * ((q - t) * (K1 - h) + (K2 - fb)));
             }
         });
     }
@@ -218,7 +286,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
             constexpr real w = real(LS::w(0));
             real bar = real(0);
             if constexpr (MODE != MODE_INIT) bar = src.template s<0, true>();
-            st_pop(Fd.s_out + (n), a * bar + w * (TO * U1 + bQ));
+            src.st(Fd.s_out + (n), a * bar + w * (TO * U1 + bQ));
         }
         static_for<LS::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
@@ -229,8 +297,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
                 if constexpr (MODE != MODE_INIT) { bi = src.template s<I, true>(); bj = src.template s<J, true>(); }
                 const real t = dot_e<LS, I, real>(tx, ty, tz);
                 const real q = real(0.5) * t * t + U1;
-                st_pop(Fd.s_out + ((unsigned)I * N + n), a * bi + w * (TO * (q + t) + bQ));
-                st_pop(Fd.s_out + ((unsigned)J * N + n), a * bj + w * (TO * (q - t) + bQ));
+                src.st(Fd.s_out + ((unsigned)I * N + n), a * bi + w * (TO * (q + t) + bQ));
+                src.st(Fd.s_out + ((unsigned)J * N + n), a * bj + w * (TO * (q - t) + bQ));
             }
         });
     }
@@ -261,7 +329,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
             const greal hdtg = greal(0.5) * dtg;
             greal bar = greal(0);
             if constexpr (MODE != MODE_INIT) bar = greal(src.template gg<0>()) - hdtg * greal(pd_old);
-            st_pop(Fd.g_out + (n), a * bar + w * (PO * U1 + bP) + hdtg * greal(pdot));
+            src.st(Fd.g_out + (n), a * bar + w * (PO * U1 + bP) + hdtg * greal(pdot));
         }
         static_for<LG::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
@@ -273,8 +341,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
                 const greal t = dot_e<LG, I, greal>(tx, ty, tz);
                 const greal q = greal(0.5) * t * t + U1;
                 const greal cn = dot_e<LG, I, greal>(bx, by, bz);
-                st_pop(Fd.g_out + ((unsigned)I * N + n), a * bi + w * (PO * (q + t) + (bP + cn)));
-                st_pop(Fd.g_out + ((unsigned)J * N + n), a * bj + w * (PO * (q - t) + (bP - cn)));
+                src.st(Fd.g_out + ((unsigned)I * N + n), a * bi + w * (PO * (q + t) + (bP + cn)));
+                src.st(Fd.g_out + ((unsigned)J * N + n), a * bj + w * (PO * (q - t) + (bP - cn)));
             }
         });
     }

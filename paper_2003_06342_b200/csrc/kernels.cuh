@@ -23,7 +23,12 @@ namespace lbm {
 enum { BC_PERIODIC = 0, BC_BOUNCE = 1 /* wall / zero-flux */, BC_ANTI = 2 /* open / Dirichlet */ };
 // MODE_STEP_PU: prescribed-velocity step (LBM_FLAG_PRESCRIBED_U): u is read from the macro array instead of Eq.(28a),
 // p and T are stored every step.  A separate instantiation so that the production kernels carry no trace of it.
-enum { MODE_STEP = 0, MODE_STEP_MACRO = 1, MODE_INIT = 2, MODE_STEP_PU = 3 };
+// MODE_STEP_VAR: step with one of the model variants of lbm_params.grad_scheme / div_scheme (biased directional derivatives,
+// PAPER.md:318; stencil divergence of u phi, reading S17); stores u, p, T every step.  MODE_U: the velocity pass
+// that precedes it when the divergence is a stencil (u^{n+1} of every node, Eq.28a, and nothing else).
+enum { MODE_STEP = 0, MODE_STEP_MACRO = 1, MODE_INIT = 2, MODE_STEP_PU = 3, MODE_STEP_VAR = 4, MODE_U = 5 };
+// modes that know the variants (all run the direct kernel; the production kernels carry no trace of them)
+template <int MODE> struct mode_has_variants { static constexpr bool value = MODE == MODE_INIT || MODE == MODE_STEP_VAR || MODE == MODE_U; };
 
 // ---- compile-time loop over directions ---------------------------------------------------------------
 template <class F, int... I>
@@ -72,6 +77,10 @@ template <class real> struct DevParams {
     real LCp, CpL, T_sat, theta_I, pc_coef;   // L/Cp, Cp/L, 4/(A W^2)
     real eps_n2;
     int phase_change, latent_heat, prescribed_u;
+    int grad_scheme, div_scheme;   // LBM_GRAD_*, LBM_DIV_* (include/lbm.h)
+    // L2 eviction priorities of the kernels built with HINT (chunked schedule, impl.cuh), two bits each (ptx.cuh l2_policy):
+    // bits 0-1 K_main's streamed reads (f, s, Pdot, phi^n), 2-3 its read of g, 4-5 its stores, 6-7 K_phi's reads of g, 8-9 its phi store
+    unsigned hints;
 };
 
 // Storage types are separate from the arithmetic type `real` of the kernels (include/lbm.h "precision"):
@@ -118,6 +127,11 @@ __device__ __forceinline__ NodeGeom make_geom(const DevParams<real> &P, int x, i
     g.sz[0] = (unsigned)(g.hi[2] ? 0 : z + 1) * plane;  g.sz[1] = (unsigned)z * plane;
     g.sz[2] = (unsigned)(g.lo[2] ? P.nz - 1 : z - 1) * plane;
     return g;
+}
+
+// element offset of the pull source of direction I (periodic wrap only)
+template <class L, int I> __device__ __forceinline__ unsigned pull_offset(unsigned N, const NodeGeom &g) {
+    return (unsigned)I * N + g.sz[L::ez(I) + 1] + g.sy[L::ey(I) + 1] + g.sx[L::ex(I) + 1];
 }
 
 // Loads.  ld_first: read-only path, free for the compiler to schedule.  ld_again: the SAME address read a second time
@@ -180,6 +194,26 @@ __device__ __forceinline__ void pull(const sreal *__restrict__ src, unsigned N, 
         constexpr int I = decltype(ic)::value;
         out[I] = pull_one<L, I, real, BC>(src, N, g, bc, val);
     });
+}
+
+// A position up to two layers outside the grid -> the node whose value stands for it: through a periodic face the periodic
+// image, through any other face the mirror image in the face, which sits half a cell outside the first / last node
+// (-1 -> 0, -2 -> 1).  cross[a] = 0, or 1 + side of the non-periodic face crossed on axis a (the caller applies that face's
+// rule to the value).  Used by the variant modes only (second neighbours of the biased difference, neighbour velocities).
+template <class real>
+__device__ __forceinline__ void ghost_source(const DevParams<real> &P, const int (&bc)[3][2], int (&q)[3], int (&cross)[3]) {
+    const int len[3] = {P.nx, P.ny, P.nz};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        cross[a] = 0;
+        if (q[a] < 0) {
+            if (bc[a][0] == BC_PERIODIC) q[a] += len[a];
+            else { q[a] = -1 - q[a]; cross[a] = 1; }
+        } else if (q[a] >= len[a]) {
+            if (bc[a][1] == BC_PERIODIC) q[a] -= len[a];
+            else { q[a] = 2 * len[a] - 1 - q[a]; cross[a] = 2; }
+        }
+    }
 }
 
 // Origin of a CTA's tile and activity of a node for launches that cover the layers [P.s0, P.s1) of the slowest axis

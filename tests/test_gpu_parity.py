@@ -269,6 +269,113 @@ def test_cuda_graph_replay_on_side_stream(gpu, oracle_mod):
     o.close()
 
 
+def test_chunked_schedule(gpu, oracle_mod):
+    """lbm_set_schedule: K_phi / K_main alternating over chunks of z-layers (K_phi one chunk ahead), with and without L2 eviction
+    hints and with K_phi launched programmatically behind K_main.  The schedule changes the order of launches only: every field
+    and population must match the oracle, and the default schedule bit for bit (to 1e-13 where the chunk origins move tiles on or off a physical face).  Periodic z (the ghost layer under layer 0 is
+    the image of the LAST layer) and z walls; chunk sizes that divide nz, that do not, 1 and >= nz."""
+    Pp = wl.base_params(256, 6, 13, grav=[1e-4, 0.0, -2e-4], force=[0.0, 1e-5, 0.0])
+    Pw = wl.base_params(40, 10, 12, grav=[0.0, 0.0, -1e-4])
+    Pw["bc_f"][2] = ["wall", "wall"]; Pw["bc_g"][2] = ["zeroflux", "zeroflux"]; Pw["bc_s"][2] = ["dirichlet", "dirichlet"]
+    Pw["bc_T"][2] = [1.0, 0.0]
+    for P, seed in ((Pp, 71), (Pw, 72)):
+        init = _random_state(P, seed)
+        o = oracle_mod.Oracle(P); o.init(*init); o.step(9)
+        base = gpu.LBM(P, 64); base.init(*init); base.step(9)
+        want = base.read_macro() + tuple(base.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
+        base.destroy()
+        for chunk, hints in ((1, 0), (4, 0), (5, 0x15), (6, 0x10015), (12, 0x10295), (64, 0x10095)):
+            sim = gpu.LBM(P, 64); sim.init(*init)
+            sim.set_schedule(chunk, hints)
+            n0 = sim.launch_count
+            sim.step(4); sim.step(5)
+            nz = P["nz"]; nch = -(-nz // chunk)
+            periodic = P["bc_f"][2][0] == "periodic"
+            nphi = nch + (1 if periodic else 0) - (1 if periodic and (nch - 1) * chunk >= nz - 1 else 0)
+            assert sim.launch_count - n0 == 9 * (nch + nphi), (chunk, sim.launch_count - n0)
+            _compare_state(gpu, sim, o, oracle_mod, TOL64, True, "chunk %d hints %#x" % (chunk, hints))
+            got = sim.read_macro() + tuple(sim.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
+            for a, b in zip(got, want):   # z walls: other tiles take the separately compiled boundary instantiation
+                assert np.array_equal(a, b) if periodic else _maxabs(a, b) <= 1e-13, (chunk, hints)
+            sim.set_schedule(0, 0); sim.step(1)
+            sim.destroy()
+        o.close()
+    # not built for 2D / fp32 contexts
+    sim = gpu.LBM(wl.base_params(40, 20, 1), 64)
+    with pytest.raises(gpu.LBMError):
+        sim.set_schedule(4, 0)
+    sim.set_schedule(0, 0)
+    sim.destroy()
+
+
+# ---------------------------------------------------------------------------- model variants (SURVEY.md 8(f) #4)
+_VARIANTS = (dict(grad_scheme="biased1"), dict(grad_scheme="biased2"), dict(div_scheme="stencil"),
+             dict(grad_scheme="biased2", div_scheme="stencil"))
+
+
+def _strip_init(P, seed):
+    """A state consistent with Dirichlet phi faces on y (a strip profile between the face values) -- a random blob against
+    phi = 0 | 1 faces makes rho < 0."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    shape = (P["nz"], P["ny"], P["nx"])
+    y = (np.arange(P["ny"]) + .5)[None, :, None] / P["ny"]
+    phi = 0.5 * (1 + np.tanh((y - 0.5) * 6)) + 0.005 * rng.uniform(-1, 1, shape)
+    T = P["T_sat"] + rng.uniform(-0.3, 0.3, shape)
+    u = 0.02 * rng.uniform(-1, 1, (3,) + shape)
+    if P["nz"] == 1:
+        u[2] = 0
+    return phi, T, u, 0.01 * rng.uniform(-1, 1, shape)
+
+
+@pytest.mark.parametrize("over", _VARIANTS, ids=lambda o: "+".join(o.values()))
+def test_model_variants(gpu, oracle_mod, over):
+    """lbm_params.grad_scheme / div_scheme: the biased directional derivatives of PAPER.md:318 inside Eq.(35b) and the stencil
+    divergence of u phi (reading S17) against the oracle, every field and population, 2D and 3D, ragged multi-tile grids,
+    every boundary kind (second neighbours and neighbour velocities beyond periodic, wall, open, zero-flux and Dirichlet faces)."""
+    P = wl.base_params(70, 21, 1, grav=[1e-4, -2e-4, 0.0], nu_l=0.05, nu_g=0.2, **over)
+    sim = gpu.LBM(P, 64); assert sim.variant == "direct (model variant)"; sim.destroy()
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 81), [1, 2, 12], label="2d periodic %s" % over)
+    P = wl.base_params(40, 20, 1, grav=[0.0, -1e-4, 0.0], **over)
+    P["bc_f"][1] = ["wall", "open"]; P["bc_g"][1] = ["zeroflux", "dirichlet"]; P["bc_s"][1] = ["dirichlet", "zeroflux"]
+    P["bc_phi"][1] = [0.0, 1.0]; P["bc_T"][1] = [0.7, 0.0]
+    _run_parity(gpu, oracle_mod, P, _strip_init(P, 82), [1, 12], label="2d wall/open %s" % over)
+    P = wl.base_params(20, 40, 1, lat_s="D2Q9", **over)
+    P["bc_f"][0] = ["wall", "wall"]; P["bc_g"][0] = ["zeroflux", "zeroflux"]; P["bc_s"][0] = ["zeroflux", "dirichlet"]
+    P["bc_f"][1] = ["open", "wall"]; P["bc_g"][1] = ["dirichlet", "dirichlet"]; P["bc_s"][1] = ["dirichlet", "dirichlet"]
+    P["bc_phi"][1] = [0.0, 1.0]; P["bc_T"][1] = [0.2, 0.0]; P["bc_T"][0] = [0.0, 0.3]
+    _run_parity(gpu, oracle_mod, P, _strip_init(P, 83), [1, 8], label="2d corners %s" % over)
+    P = wl.base_params(34, 9, 12, grav=[0.0, 0.0, -1e-4], **over)
+    P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
+    P["bc_T"][2] = [1.0, 0.0]
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 84), [1, 10], label="3d z walls %s" % over)
+    P = wl.base_params(136, 5, 6, grav=[1e-4, 0.0, -2e-4], lat_f="D3Q15", **over)
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 85), [1, 8], label="3d D3Q15 wide %s" % over)
+    P = wl.base_params(6, 3, 2, **over)       # minimal 3D grid: second neighbours wrap onto the node itself
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 86), [1, 4], label="3d tiny %s" % over)
+
+
+def test_model_variants_other_modes(gpu, oracle_mod):
+    """The variants with a prescribed velocity (no velocity pass: the field is the array), in fp32 (1e-4 bar), through the
+    CUDA-graph replay, and where they are refused: slab contexts (ghost layers are one deep) and partial launches."""
+    P = wl.base_params(48, 16, 1, prescribed_u=True, grad_scheme="biased2", div_scheme="stencil")
+    _run_parity(gpu, oracle_mod, P, _random_state(P, 87), [1, 9], label="variants, prescribed u")
+    P = wl.base_params(40, 12, 9, grav=[1e-4, 0.0, -2e-4], grad_scheme="biased2", div_scheme="stencil")
+    init = _random_state(P, 88)
+    o = oracle_mod.Oracle(P); o.init(*init); o.step(23)
+    sim = gpu.LBM(P, 64); sim.init(*init); sim.step(3); sim.step(20)      # 19 plain steps: graph replay on this small grid
+    _compare_state(gpu, sim, o, oracle_mod, TOL64, True, "variants, graph replay")
+    sim.destroy()
+    sim = gpu.LBM(P, 32); sim.init(*[a.astype(np.float32) for a in init]); sim.step(23)
+    for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
+        assert _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30) <= REL32, name
+    sim.destroy(); o.close()
+    Q = dict(P); Q["halo"] = (1, 1)
+    with pytest.raises(gpu.LBMError, match="not built"):
+        gpu.LBM(Q, 64)
+    with pytest.raises(gpu.LBMError):
+        gpu.LBM(dict(P, kernels=()), 64).set_schedule(4, 0)
+
+
 # ---------------------------------------------------------------------------- D3Q15 Navier-Stokes lattice (PAPER.md:190)
 def _d3q15_cases():
     P1 = wl.base_params(136, 10, 7, lat_f="D3Q15", grav=[1e-4, -1e-4, -2e-4], force=[1e-5, 0.0, 2e-5])   # wide tiles, ragged
