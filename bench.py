@@ -186,8 +186,6 @@ def run_ours(args):
     del I
 
     sim = binding.LBM(P, prec)
-    if args.chunk:
-        sim.set_schedule(args.chunk, int(args.hints, 0))   # K_phi / K_main alternating over chunks of z-layers (lbm_set_schedule)
     sim.init(h_phi, h_T)                      # inputs resident in HBM from here on
     sim.step(W)
     sim.sync()
@@ -199,7 +197,7 @@ def run_ours(args):
     launches0 = sim.launch_count
     # per-kernel CUDA events inside lbm_step: on large grids they ride in the timed region itself; small (launch-bound) grids
     # replay their steps from a CUDA graph, which per-kernel events would switch off, so those get a second pass for them
-    events_inside = N > (1 << 21) and not args.chunk   # (per-kernel events switch the chunked schedule off as well)
+    events_inside = N > (1 << 21)
     sim.set_timing(events_inside)
     replicas.barrier()
     torch.cuda.synchronize()
@@ -383,8 +381,6 @@ def main():
     ap.add_argument("--precision", type=int, default=64, choices=(32, 64))
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--chunk", type=int, default=0, help="3D fp64: lbm_set_schedule chunk of z-layers (0 = two launches per step)")
-    ap.add_argument("--hints", default="0", help="lbm_set_schedule L2 eviction hints word")
     ap.add_argument("--parallelism", default="replicas", choices=("replicas", "slabs", "slabs-strong"),
                     help="N > 1: independent replicas (default, the bench contract), one slab of a stacked domain per rank (weak), "
                          "or ONE domain cut into one slab per rank (strong; the paper's decomposed runs)")

@@ -209,15 +209,6 @@ int lbm_halo_bytes(const lbm_ctx *c, int what, size_t *bytes);
 int lbm_halo_pack(lbm_ctx *c, int what, int side, void *d_buf);
 int lbm_halo_unpack(lbm_ctx *c, int what, int side, const void *d_buf);
 
-/* Schedule of lbm_step on 3D fp64 contexts (elsewhere LBM_E_UNSUPPORTED unless chunk_layers == 0).  chunk_layers > 0: K_phi and
- * K_main alternate over chunks of that many z-layers, K_phi one chunk ahead, so that the g* lines and the phi^{n+1} layers K_phi
- * touched are still in L2 when K_main reads them (the paper's own fusion / traffic trade-off).
- * hints: L2 eviction priority of those launches, two bits each (0 normal, 1 evict-first, 2 evict-last): bits 0-1 K_main's
- * streamed reads (f, s, Pdot, phi^n), 2-3 its read of g, 4-5 its stores, 6-7 K_phi's reads of g, 8-9 its phi store; bit 16: K_phi
- * launched programmatically behind K_main.  chunk_layers == 0: two launches over the whole grid (the default).  Changes speed,
- * never results. */
-int lbm_set_schedule(lbm_ctx *c, int chunk_layers, unsigned hints);
-
 /* Copy the macroscopic fields of the current time level to HOST arrays; any pointer may be NULL.
  * h_u is [3][z][y][x].  Synchronises. */
 int lbm_read_macro(lbm_ctx *c, void *h_phi, void *h_u, void *h_p, void *h_T);

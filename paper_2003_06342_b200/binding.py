@@ -32,7 +32,7 @@ STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1
 NOALLOC_SCRATCH_BYTES = 8 << 20
 
-EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_set_schedule", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
            "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
@@ -89,7 +89,6 @@ def load_library():
         L.lbm_read_pops_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_sync.argtypes = [C.c_void_p]
         L.lbm_set_timing.argtypes = [C.c_void_p, C.c_int]
-        L.lbm_set_schedule.argtypes = [C.c_void_p, C.c_int, C.c_uint]
         L.lbm_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.lbm_step_count.restype = C.c_longlong
         L.lbm_step_count.argtypes = [C.c_void_p]
@@ -287,10 +286,6 @@ class LBM:
     def stream(self):
         """The torch.cuda.Stream every kernel and copy of this context is enqueued on (record timing events there)."""
         return self._stream
-
-    def set_schedule(self, chunk_layers: int, hints: int = 0):
-        """lbm_set_schedule: K_phi / K_main alternate over chunks of z-layers (3D fp64); 0 = two launches over the whole grid."""
-        _check(self._L.lbm_set_schedule(self._h, int(chunk_layers), int(hints)), "lbm_set_schedule")
 
     def set_timing(self, enable: bool):
         _check(self._L.lbm_set_timing(self._h, 1 if enable else 0), "lbm_set_timing")

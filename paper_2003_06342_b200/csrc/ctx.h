@@ -76,11 +76,7 @@ struct lbm_ctx {
     // ... and the pulled populations, phi^n, Pdot staged by per-thread cp.async (k_main_smem.cuh)
     bool pops_smem;
     bool pdl;   // K_main launched with programmatic stream serialisation behind K_phi
-    // chunked schedule (lbm_set_schedule): K_phi and K_main alternate over chunks of `chunk` layers of the slowest axis so that
-    // what K_phi leaves in L2 (g*, phi^{n+1}) is still there when K_main reads it; 0 = two launches over the whole grid
-    int chunk;
-    unsigned hints;   // DevParams::hints of the chunked launches; bit 16: K_phi launched programmatically behind K_main
-    int attr_done[12];   // kernel attributes set on this context's device: [MODE] K_main
+    int attr_done[8];   // kernel attributes set on this context's device: [MODE] K_main
     // CUDA graph of two consecutive plain steps, for launch-bound (small) grids
     bool graph_ok;
     cudaGraphExec_t graph2;

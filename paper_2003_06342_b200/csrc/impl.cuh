@@ -107,22 +107,8 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         return cudaLaunchKernelEx(&cfg, kern, P, F, map);
     }
 
-    // the chunked schedule exists where it was measured: 3D, one element type throughout (fp64)
-    static constexpr bool CHUNKABLE = D == 3 && UNIFORM;
-
-    template <int MODE> static int launch_main(lbm_ctx *c, const Fields &F, int pnew = 0, bool hint = false) {
+    template <int MODE> static int launch_main(lbm_ctx *c, const Fields &F, int pnew = 0) {
         if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU && MODE != MODE_STEP_VAR && MODE != MODE_U) {
-            if constexpr (CHUNKABLE) {
-                if (hint) {
-                    using C = SmemCfg<LF, LG, LS, sreal, preal, T::BX, T::BY, T::BZ, false, true>;
-                    auto kern = k_main_smem<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB, Fields, true>;
-                    int rc = set_smem_attrs(c, kern, C::BYTES, c->attr_done[4 + MODE]);
-                    if (rc) return rc;
-                    CK(launch_after_phi(c, kern, C::BYTES, dev_params<real>(c), F, c->map_phi_tile[pnew]));
-                    c->launches++;
-                    return LBM_OK;
-                }
-            }
             if (c->phi_tma && c->pops_smem) {
                 using C = SmemCfg<LF, LG, LS, sreal, preal, T::BX, T::BY, T::BZ>;
                 auto kern = k_main_smem<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB, Fields>;
@@ -179,25 +165,11 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     }
 
     // phase 0 of a step: K_phi (phi^{n+1} of every node, Eq.32)
-    static int launch_phi(lbm_ctx *c, bool hint = false, bool behind_main = false) {
+    static int launch_phi(lbm_ctx *c) {
         const DevParams<real> &P = dev_params<real>(c);
         const int in = c->cur, pnew = 1 - c->curphi;
         dim3 gphi = grid_layers<TP>(c);
         if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
-        if constexpr (CHUNKABLE) {
-            if (hint) {
-                cudaLaunchConfig_t cfg = {};
-                cfg.gridDim = gphi; cfg.blockDim = dim3(NTP); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
-                cudaLaunchAttribute at[1];
-                at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-                at[0].val.programmaticStreamSerializationAllowed = 1;
-                cfg.attrs = at; cfg.numAttrs = behind_main ? 1 : 0;
-                auto kern = k_phi<LG, real, TP::BX, TP::BY, TP::BZ, PHI_NPT, sreal, preal, true>;
-                CK(cudaLaunchKernelEx(&cfg, kern, P, (const sreal *)wsp<sreal>(c, c->L.off_g[in]), wsp<preal>(c, c->L.off_phi[pnew])));
-                c->launches++;
-                return LBM_OK;
-            }
-        }
         k_phi<LG, real, TP::BX, TP::BY, TP::BZ, PHI_NPT><<<gphi, NTP, 0, c->stream>>>(
             P, (const sreal *)wsp<sreal>(c, c->L.off_g[in]), wsp<preal>(c, c->L.off_phi[pnew]));
         c->launches++;
@@ -206,7 +178,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     }
 
     // phase 1 of a step: K_main, then (flip) the buffers flip
-    static int launch_collide(lbm_ctx *c, bool macro, bool flip = true, bool hint = false) {
+    static int launch_collide(lbm_ctx *c, bool macro, bool flip = true) {
         const DevParams<real> &P = dev_params<real>(c);
         const int in = c->cur, out = 1 - c->cur, pnew = 1 - c->curphi, pold = c->curphi;
         Fields F = fields(c, in, out, pnew, pold);
@@ -216,7 +188,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
             if (P.div_scheme && !P.prescribed_u) rc = launch_main<MODE_U>(c, F, pnew);
             if (!rc) rc = launch_main<MODE_STEP_VAR>(c, F, pnew);
         } else if (P.prescribed_u) rc = launch_main<MODE_STEP_PU>(c, F, pnew);   // direct kernel only
-        else rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, pnew, hint) : launch_main<MODE_STEP>(c, F, pnew, hint);
+        else rc = macro ? launch_main<MODE_STEP_MACRO>(c, F, pnew) : launch_main<MODE_STEP>(c, F, pnew);
         if (rc) return rc;
         if (flip) { c->cur = out; c->curphi = pnew; c->nsteps++; }
         return LBM_OK;
@@ -239,45 +211,8 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         return phase == 0 ? launch_phi(c) : launch_collide(c, macro != 0);
     }
 
-    static void set_layers(lbm_ctx *c, int first, int end) { c->pd.s0 = c->pf.s0 = first; c->pd.s1 = c->pf.s1 = end; }
-
-    // ONE step as K_phi / K_main launches that alternate over chunks of c->chunk layers of the slowest axis, K_phi one chunk
-    // ahead (K_main's stencil reaches one layer into the next chunk):
-    //     K_phi(0) K_phi(1) K_main(0) K_phi(2) K_main(1) ... K_main(last)
-    // so that the g* lines K_phi(k) pulled and the phi^{n+1} it wrote are still in L2 when K_main(k) reads them -- 70 instead of
-    // 78 values per update through HBM if nothing is evicted in between.  All launches sit on one
-    // stream; K_main(k) depends on K_phi(k+1) only, K_phi on nothing of the same step.
-    static int step_once_chunked(lbm_ctx *c, bool macro) {
-        const int ns = D == 3 ? c->P.nz : c->P.ny, C = c->chunk, nch = (ns + C - 1) / C;
-        const int axis = D == 3 ? 2 : 1;
-        const bool periodic = c->P.bc_f[axis][0] == LBM_F_PERIODIC && c->P.bc_f[axis][1] == LBM_F_PERIODIC;
-        const bool phi_pdl = (c->hints >> 16) & 1u;
-        int rc = LBM_OK;
-        // periodic slow axis: the ghost layer under layer 0 is the image of the LAST layer, which K_main(0) needs
-        if (periodic) { set_layers(c, ns - 1, ns); rc = launch_phi(c, true, false); }
-        const int phi_end = periodic ? ns - 1 : ns;   // ... so the last chunk's K_phi leaves that layer out
-        auto phi_chunk = [&](int k, bool behind_main) {
-            const int a = k * C, b = (k + 1) * C < phi_end ? (k + 1) * C : phi_end;
-            if (a >= b) return (int)LBM_OK;
-            set_layers(c, a, b);
-            return launch_phi(c, true, behind_main);
-        };
-        if (!rc) rc = phi_chunk(0, false);
-        for (int k = 0; k < nch && !rc; ++k) {
-            if (k + 1 < nch) rc = phi_chunk(k + 1, phi_pdl && k > 0);
-            if (rc) break;
-            set_layers(c, k * C, (k + 1) * C < ns ? (k + 1) * C : ns);
-            rc = launch_collide(c, macro, k == nch - 1, true);
-        }
-        set_layers(c, 0, ns);
-        return rc;
-    }
-
     // enqueue the kernels of ONE step and flip the buffers
     static int step_once(lbm_ctx *c, bool macro, bool timed) {
-        if constexpr (CHUNKABLE) {
-            if (c->chunk > 0 && !timed && !c->pd.prescribed_u && !c->pd.grad_scheme && !c->pd.div_scheme) return step_once_chunked(c, macro);
-        }
         cudaEvent_t e3[3] = {nullptr, nullptr, nullptr};
         if (timed) {
             for (auto &e : e3) CK(cudaEventCreate(&e));

@@ -41,7 +41,6 @@ template <class LF, class LG, class LS, class real, bool BC, class Fields = DevF
     template <int I, bool AGAIN = false> __device__ __forceinline__ real f() const { return pull_one<LF, I, real, BC, AGAIN>(Fd.f_in, (unsigned)P.N, g, P.bc_f, P.bc_p); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real s() const { return pull_one<LS, I, real, BC, AGAIN>(Fd.s_in, (unsigned)P.N, g, P.bc_s, P.bc_T); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real gg() const { return pull_one<LG, I, real, BC, AGAIN>(Fd.g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi); }
-    template <class sreal, class wreal> __device__ __forceinline__ void st(sreal *p, wreal v) const { st_pop(p, v); }
     // ---- variant modes only ----
     // phi^{n+1} up to two nodes away (second neighbour of the second-order biased difference), with the ghost
     // rule of reading S8-iv carried two layers deep: periodic image; zero-flux mirror; Dirichlet 2 v - mirror
@@ -254,7 +253,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
             constexpr real w = real(LF::w(0));
             real bar = real(0);
             if constexpr (MODE != MODE_INIT) bar = src.template f<0, true>();
-            src.st(Fd.f_out + (n), a * bar + w * (U * K1 + K2));
+            st_pop(Fd.f_out + (n), a * bar + w * (U * K1 + K2));
         }
         static_for<LF::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
@@ -267,8 +266,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
                 const real q = real(0.5) * t * t + U;
                 const real h = dot_e<LF, I, real>(Hbx, Hby, Hbz);
                 const real fb = dot_e<LF, I, real>(Fbx, Fby, Fbz);
-                src.st(Fd.f_out + ((unsigned)I * N + n), a * bi + w * ((q + t) * (K1 + h) + (K2 + fb)));
-                src.st(Fd.f_out + ((unsigned)J * N + n), a * bj + w * ((q - t) * (K1 - h) + (K2 - fb)));
+                st_pop(Fd.f_out + ((unsigned)I * N + n), a * bi + w * ((q + t) * (K1 + h) + (K2 + fb)));
+                st_pop(Fd.f_out + ((unsigned)J * N + n), a * bj + w * ((q - t) * (K1 - h) + (K2 - fb)));
             }
         });
     }
@@ -286,7 +285,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
             constexpr real w = real(LS::w(0));
             real bar = real(0);
             if constexpr (MODE != MODE_INIT) bar = src.template s<0, true>();
-            src.st(Fd.s_out + (n), a * bar + w * (TO * U1 + bQ));
+            st_pop(Fd.s_out + (n), a * bar + w * (TO * U1 + bQ));
         }
         static_for<LS::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
@@ -297,8 +296,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
                 if constexpr (MODE != MODE_INIT) { bi = src.template s<I, true>(); bj = src.template s<J, true>(); }
                 const real t = dot_e<LS, I, real>(tx, ty, tz);
                 const real q = real(0.5) * t * t + U1;
-                src.st(Fd.s_out + ((unsigned)I * N + n), a * bi + w * (TO * (q + t) + bQ));
-                src.st(Fd.s_out + ((unsigned)J * N + n), a * bj + w * (TO * (q - t) + bQ));
+                st_pop(Fd.s_out + ((unsigned)I * N + n), a * bi + w * (TO * (q + t) + bQ));
+                st_pop(Fd.s_out + ((unsigned)J * N + n), a * bj + w * (TO * (q - t) + bQ));
             }
         });
     }
@@ -329,7 +328,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
             const greal hdtg = greal(0.5) * dtg;
             greal bar = greal(0);
             if constexpr (MODE != MODE_INIT) bar = greal(src.template gg<0>()) - hdtg * greal(pd_old);
-            src.st(Fd.g_out + (n), a * bar + w * (PO * U1 + bP) + hdtg * greal(pdot));
+            st_pop(Fd.g_out + (n), a * bar + w * (PO * U1 + bP) + hdtg * greal(pdot));
         }
         static_for<LG::Q>([&](auto icn) {
             constexpr int I = decltype(icn)::value;
@@ -341,8 +340,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
                 const greal t = dot_e<LG, I, greal>(tx, ty, tz);
                 const greal q = greal(0.5) * t * t + U1;
                 const greal cn = dot_e<LG, I, greal>(bx, by, bz);
-                src.st(Fd.g_out + ((unsigned)I * N + n), a * bi + w * (PO * (q + t) + (bP + cn)));
-                src.st(Fd.g_out + ((unsigned)J * N + n), a * bj + w * (PO * (q - t) + (bP - cn)));
+                st_pop(Fd.g_out + ((unsigned)I * N + n), a * bi + w * (PO * (q + t) + (bP + cn)));
+                st_pop(Fd.g_out + ((unsigned)J * N + n), a * bj + w * (PO * (q - t) + (bP - cn)));
             }
         });
     }

@@ -44,7 +44,6 @@ template <class LF, class LG, class LS, class real, bool BC, class TC, class Fie
     template <int I, bool AGAIN = false> __device__ __forceinline__ real f() const { return pull_one<LF, I, real, BC, AGAIN>(Fd.f_in, (unsigned)P.N, g, P.bc_f, P.bc_p); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real s() const { return pull_one<LS, I, real, BC, AGAIN>(Fd.s_in, (unsigned)P.N, g, P.bc_s, P.bc_T); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real gg() const { return pull_one<LG, I, real, BC, AGAIN>(Fd.g_in, (unsigned)P.N, g, P.bc_g, P.bc_phi); }
-    template <class sreal, class wreal> __device__ __forceinline__ void st(sreal *p, wreal v) const { st_pop(p, v); }
 };
 
 // shared memory of one CTA: the phi tile and its mbarrier

@@ -13,12 +13,10 @@ namespace lbm {
 
 // shared-memory carve-up of one CTA of NT threads
 // STAGE_G: g is read once (at its collision), so staging it only buys the early issue (measured: no gain; off).
-// HINT: every global access carries an L2 eviction priority taken from DevParams::hints (chunked schedule, impl.cuh).
-template <class LF, class LG, class LS, class sreal, class preal, int BX, int BY, int BZ, bool STAGE_G_ = false, bool HINT_ = false> struct SmemCfg {
+template <class LF, class LG, class LS, class sreal, class preal, int BX, int BY, int BZ, bool STAGE_G_ = false> struct SmemCfg {
     using TC = PhiTileCfg<preal, LF::D, BX, BY, BZ>;
     static constexpr int NT = BX * BY * BZ;
     static constexpr bool STAGE_G = STAGE_G_;
-    static constexpr bool HINT = HINT_;
     static constexpr int QT = LF::Q + LS::Q + (STAGE_G ? LG::Q : 0);
     static constexpr int OFF_F = 0, OFF_S = LF::Q, OFF_G = LF::Q + LS::Q, OFF_PDOT = QT;   // sreal slots
     static constexpr size_t TILE_BYTES = ((size_t)TC::BYTES + 127) / 128 * 128;
@@ -38,20 +36,12 @@ template <class LF, class LG, class LS, class real, class C, class Fields> struc
     const preal *phiold;    // this thread's slot
     const sreal *col;       // this thread's column: value k at col[k * NT]
     uint32_t bar;
-    uint64_t pol_in, pol_g, pol_out;   // HINT only: L2 policies of the streamed reads, of the read of g, of the stores
     __device__ __forceinline__ SrcSmem(const DevParams<real> &P_, const Fields &Fd_, const NodeGeom &g_, const preal *tile_base,
                                        const preal *phiold_base, const sreal *pops_base, uint32_t bar_, int t, int tx, int ty, int tz)
         : P(P_), Fd(Fd_), g(g_), bar(bar_) {
         tile = tile_base + ((LF::D == 3 ? tz + 1 : 0) * TC::BOXY + ty + 1) * TC::BOXX + tx + TC::EPB;
         phiold = phiold_base + t;
         col = pops_base + t;
-        if constexpr (C::HINT) {
-            pol_in = l2_policy((int)(P.hints & 3u)); pol_g = l2_policy((int)((P.hints >> 2) & 3u)); pol_out = l2_policy((int)((P.hints >> 4) & 3u));
-        }
-    }
-    template <class T> __device__ __forceinline__ void copy_in(uint32_t dst, const T *src) const {
-        if constexpr (C::HINT) cp_async_val(dst, src, pol_in);
-        else cp_async_val(dst, src);
     }
     // issue every copy of this node; nothing is waited for here
     __device__ __forceinline__ void prefetch() const {
@@ -60,20 +50,20 @@ template <class LF, class LG, class LS, class real, class C, class Fields> struc
         constexpr uint32_t STEP = (uint32_t)(C::NT * sizeof(sreal));
         static_for<LS::Q>([&](auto ic) {
             constexpr int I = decltype(ic)::value;
-            copy_in(c0 + (uint32_t)(C::OFF_S + I) * STEP, Fd.s_in + pull_offset<LS, I>(N, g));
+            cp_async_val(c0 + (uint32_t)(C::OFF_S + I) * STEP, Fd.s_in + pull_offset<LS, I>(N, g));
         });
-        copy_in(c0 + (uint32_t)C::OFF_PDOT * STEP, Fd.pdot_in + g.n);
+        cp_async_val(c0 + (uint32_t)C::OFF_PDOT * STEP, Fd.pdot_in + g.n);
         const unsigned pcoff = ((unsigned)(g.z + P.pz) * (unsigned)P.ppy + (unsigned)(g.y + 1)) * (unsigned)P.ppx + (unsigned)(g.x + P.xpad);
-        copy_in(smem_u32(phiold), Fd.phi_old + pcoff);
+        cp_async_val(smem_u32(phiold), Fd.phi_old + pcoff);
         cp_async_commit();   // group 1: what the stencil and closure phase needs (s, Pdot, phi^n)
         static_for<LF::Q>([&](auto ic) {
             constexpr int I = decltype(ic)::value;
-            copy_in(c0 + (uint32_t)(C::OFF_F + I) * STEP, Fd.f_in + pull_offset<LF, I>(N, g));
+            cp_async_val(c0 + (uint32_t)(C::OFF_F + I) * STEP, Fd.f_in + pull_offset<LF, I>(N, g));
         });
         if constexpr (C::STAGE_G) {
             static_for<LG::Q>([&](auto ic) {
                 constexpr int I = decltype(ic)::value;
-                copy_in(c0 + (uint32_t)(C::OFF_G + I) * STEP, Fd.g_in + pull_offset<LG, I>(N, g));
+                cp_async_val(c0 + (uint32_t)(C::OFF_G + I) * STEP, Fd.g_in + pull_offset<LG, I>(N, g));
             });
         }
         cp_async_commit();   // group 2: f (and g), first needed by the moments
@@ -89,22 +79,17 @@ template <class LF, class LG, class LS, class real, class C, class Fields> struc
     template <int I, bool AGAIN = false> __device__ __forceinline__ real s() const { return real(col[(C::OFF_S + I) * C::NT]); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ real gg() const {
         if constexpr (C::STAGE_G) return real(col[(C::OFF_G + I) * C::NT]);
-        else if constexpr (C::HINT) return real(ld_hint(Fd.g_in + pull_offset<LG, I>((unsigned)P.N, g), pol_g));
         else return real(__ldg(Fd.g_in + pull_offset<LG, I>((unsigned)P.N, g)));
-    }
-    template <class wreal> __device__ __forceinline__ void st(sreal *p, wreal v) const {
-        if constexpr (C::HINT) st_hint(p, sreal(v), pol_out);
-        else st_pop(p, v);
     }
 };
 
 // one tile of BX x BY x BZ nodes with origin (x0, y0, z0); smem_raw: SmemCfg::BYTES bytes of dynamic shared memory
-template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, bool STAGE_G = false, bool HINT = false, class Fields>
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, bool STAGE_G = false, class Fields>
 __device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const Fields &Fd, const CUtensorMap *phi_map,
                                                unsigned char *smem_raw, int x0, int y0, int z0) {
     using sreal = typename Fields::sreal;
     using preal = typename Fields::preal;
-    using C = SmemCfg<LF, LG, LS, sreal, preal, BX, BY, BZ, STAGE_G, HINT>;
+    using C = SmemCfg<LF, LG, LS, sreal, preal, BX, BY, BZ, STAGE_G>;
     using TC = typename C::TC;
     preal *tile = reinterpret_cast<preal *>(smem_raw);
     preal *phiold = reinterpret_cast<preal *>(smem_raw + C::TILE_BYTES);
@@ -118,8 +103,6 @@ __device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const F
         fence_mbar_init();
         fence_proxy_async();
     }
-    // chunked schedule: the K_phi of the chunk after next may fill the SMs as this grid drains (it reads nothing this grid writes)
-    if constexpr (HINT) pdl_launch_dependents();
     const int x = x0 + tx, y = y0 + ty, z = z0 + tz;
     const bool active = node_active<LF::D>(P, x, y, z);
     const bool bc = tile_touches_bc(P, x0, y0, z0, BX, BY, BZ);
@@ -149,13 +132,13 @@ __device__ __forceinline__ void main_tile_smem(const DevParams<real> &P, const F
     }
 }
 
-template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB, class Fields, bool HINT = false>
+template <class LF, class LG, class LS, class real, int MODE, int BX, int BY, int BZ, int MINB, class Fields>
 __global__ void __launch_bounds__(BX *BY *BZ, MINB)
 k_main_smem(const DevParams<real> P, const Fields Fd, const __grid_constant__ CUtensorMap phi_map) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     int y0, z0;
     tile_origin<LF::D>(P, BY, BZ, y0, z0);
-    main_tile_smem<LF, LG, LS, real, MODE, BX, BY, BZ, false, HINT>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, y0, z0);
+    main_tile_smem<LF, LG, LS, real, MODE, BX, BY, BZ>(P, Fd, &phi_map, smem_raw, blockIdx.x * BX, y0, z0);
 }
 
 }  // namespace lbm

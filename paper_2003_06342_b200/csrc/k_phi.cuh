@@ -11,12 +11,11 @@ namespace lbm {
 // Store phi of node g into the padded array and into every ghost image of that node (reading S8-iv):
 // periodic axis -> image one period away; zero-flux face -> mirror phi(-1) = phi(0); Dirichlet face with value v ->
 // phi(-1) = 2 v - phi(0).  Transforms compose in axis order x, y, z (what an axis-by-axis ghost fill would give).
-template <bool HINT = false, class real, class preal>
+template <class real, class preal>
 __device__ __forceinline__ void store_phi_with_images(preal *__restrict__ phi_pad, const DevParams<real> &P,
-                                                      const NodeGeom &g, preal v, uint64_t pol = 0) {
+                                                      const NodeGeom &g, preal v) {
     const long long pc = ((long long)(g.z + P.pz) * P.ppy + (g.y + 1)) * P.ppx + (g.x + P.xpad);
-    if constexpr (HINT) st_hint(phi_pad + pc, v, pol);
-    else phi_pad[pc] = v;
+    phi_pad[pc] = v;
     const bool edge = g.lo[0] | g.hi[0] | g.lo[1] | g.hi[1] | (P.pz && (g.lo[2] | g.hi[2]));
     if (!edge) return;
     int cnt[3];
@@ -88,8 +87,7 @@ __device__ __forceinline__ preal phi_sum(const vreal (&gi)[Q]) {
 // issued before the first sum, which is what a latency-bound streaming kernel needs (measured: DESIGN.md "Kernels").
 // The pulled values are held in the arithmetic type `real` when that is the stored type (all-float kernels: no widening
 // before the error-free sum), else in preal.
-// HINT: loads and the phi store carry the L2 eviction priorities of DevParams::hints (chunked schedule, impl.cuh).
-template <class LG, class real, int BX, int BY, int BZ, int NPT, class sreal, class preal, bool HINT = false>
+template <class LG, class real, int BX, int BY, int BZ, int NPT, class sreal, class preal>
 __global__ void __launch_bounds__(BX *BY *BZ)
 k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, preal *__restrict__ phi_new) {
     using vreal = typename std::conditional<std::is_same<real, sreal>::value, real, preal>::type;
@@ -112,24 +110,13 @@ k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, preal *__restrict
         if (ok[j]) {
             g[j] = make_geom(P, x, y, z);
             if (bc) pull<LG, vreal, true>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
-            else if constexpr (HINT) {
-                const uint64_t pol = l2_policy((int)((P.hints >> 6) & 3u));
-                static_for<LG::Q>([&](auto ic) {
-                    constexpr int I = decltype(ic)::value;
-                    gi[j][I] = vreal(ld_hint(g_in + pull_offset<LG, I>((unsigned)P.N, g[j]), pol));
-                });
-            } else pull<LG, vreal, false>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
+            else pull<LG, vreal, false>(g_in, (unsigned)P.N, g[j], P.bc_g, P.bc_phi, gi[j]);
         }
     }
-    uint64_t pol_st = 0;
-    if constexpr (HINT) pol_st = l2_policy((int)((P.hints >> 8) & 3u));
 #pragma unroll
     for (int j = 0; j < NPT; ++j) {
-        if (ok[j]) store_phi_with_images<HINT>(phi_new, P, g[j], phi_sum<preal>(gi[j]), pol_st);
+        if (ok[j]) store_phi_with_images(phi_new, P, g[j], phi_sum<preal>(gi[j]));
     }
-    // a K_phi launched behind a K_main of the SAME step with programmatic serialisation (chunked schedule) depends on nothing
-    // that kernel writes; waiting here, at the very end, only keeps completion transitive along the stream
-    pdl_wait();
 }
 
 // Initialisation helper: copy a plain [z][y][x] phi into both padded buffers with ghost images.

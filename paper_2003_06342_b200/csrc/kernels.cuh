@@ -78,9 +78,6 @@ template <class real> struct DevParams {
     real eps_n2;
     int phase_change, latent_heat, prescribed_u;
     int grad_scheme, div_scheme;   // LBM_GRAD_*, LBM_DIV_* (include/lbm.h)
-    // L2 eviction priorities of the kernels built with HINT (chunked schedule, impl.cuh), two bits each (ptx.cuh l2_policy):
-    // bits 0-1 K_main's streamed reads (f, s, Pdot, phi^n), 2-3 its read of g, 4-5 its stores, 6-7 K_phi's reads of g, 8-9 its phi store
-    unsigned hints;
 };
 
 // Storage types are separate from the arithmetic type `real` of the kernels (include/lbm.h "precision"):

@@ -168,7 +168,6 @@ template <class real> DevParams<real> make_dev_params(const lbm_params *p, const
     d.latent_heat = (p->flags & LBM_FLAG_LATENT_HEAT) ? 1 : 0;
     d.prescribed_u = (p->flags & LBM_FLAG_PRESCRIBED_U) ? 1 : 0;
     d.grad_scheme = p->grad_scheme; d.div_scheme = p->div_scheme;
-    d.hints = 0;
     return d;
 }
 
@@ -267,7 +266,6 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         c->graph2 = nullptr; c->graph_launches = 0;
         for (int &a : c->attr_done) a = 0;
         c->pdl = !(fl & LBM_FLAG_NO_PDL);
-        c->chunk = 0; c->hints = 0;
         // phi halo tile of K_main: one TMA box per CTA into shared memory (default) or plain loads through L1
         c->phi_tma = !(fl & LBM_FLAG_PHI_LDG) && build_phi_tile_maps(c);
         // pulled populations of K_main: staged in shared memory by cp.async (k_main_smem.cuh) where that measured faster --
@@ -318,17 +316,6 @@ int lbm_step_layers(lbm_ctx *c, int phase, int first, int count, int store_macro
 int lbm_set_stream(lbm_ctx *c, void *cuda_stream) {
     if (!c) return LBM_E_INVALID;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
-    return LBM_OK;
-}
-
-int lbm_set_schedule(lbm_ctx *c, int chunk_layers, unsigned hints) {
-    if (!c || chunk_layers < 0) return LBM_E_INVALID;
-    if (chunk_layers > 0 && !(c->P.nz > 1 && c->P.precision == 64 && c->phi_tma)) return LBM_E_UNSUPPORTED;
-    if (chunk_layers > 0 && (c->P.grad_scheme || c->P.div_scheme)) return LBM_E_UNSUPPORTED;
-    if (c->P.halo[0] | c->P.halo[1]) return LBM_E_UNSUPPORTED;   // slabs step by phases
-    c->chunk = chunk_layers; c->hints = hints;
-    c->pd.hints = c->pf.hints = hints;
-    if (c->graph2) { cudaGraphExecDestroy(c->graph2); c->graph2 = nullptr; }   // a captured graph holds the old schedule
     return LBM_OK;
 }
 

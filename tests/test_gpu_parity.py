@@ -269,45 +269,6 @@ def test_cuda_graph_replay_on_side_stream(gpu, oracle_mod):
     o.close()
 
 
-def test_chunked_schedule(gpu, oracle_mod):
-    """lbm_set_schedule: K_phi / K_main alternating over chunks of z-layers (K_phi one chunk ahead), with and without L2 eviction
-    hints and with K_phi launched programmatically behind K_main.  The schedule changes the order of launches only: every field
-    and population must match the oracle, and the default schedule bit for bit (to 1e-13 where the chunk origins move tiles on or off a physical face).  Periodic z (the ghost layer under layer 0 is
-    the image of the LAST layer) and z walls; chunk sizes that divide nz, that do not, 1 and >= nz."""
-    Pp = wl.base_params(256, 6, 13, grav=[1e-4, 0.0, -2e-4], force=[0.0, 1e-5, 0.0])
-    Pw = wl.base_params(40, 10, 12, grav=[0.0, 0.0, -1e-4])
-    Pw["bc_f"][2] = ["wall", "wall"]; Pw["bc_g"][2] = ["zeroflux", "zeroflux"]; Pw["bc_s"][2] = ["dirichlet", "dirichlet"]
-    Pw["bc_T"][2] = [1.0, 0.0]
-    for P, seed in ((Pp, 71), (Pw, 72)):
-        init = _random_state(P, seed)
-        o = oracle_mod.Oracle(P); o.init(*init); o.step(9)
-        base = gpu.LBM(P, 64); base.init(*init); base.step(9)
-        want = base.read_macro() + tuple(base.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
-        base.destroy()
-        for chunk, hints in ((1, 0), (4, 0), (5, 0x15), (6, 0x10015), (12, 0x10295), (64, 0x10095)):
-            sim = gpu.LBM(P, 64); sim.init(*init)
-            sim.set_schedule(chunk, hints)
-            n0 = sim.launch_count
-            sim.step(4); sim.step(5)
-            nz = P["nz"]; nch = -(-nz // chunk)
-            periodic = P["bc_f"][2][0] == "periodic"
-            nphi = nch + (1 if periodic else 0) - (1 if periodic and (nch - 1) * chunk >= nz - 1 else 0)
-            assert sim.launch_count - n0 == 9 * (nch + nphi), (chunk, sim.launch_count - n0)
-            _compare_state(gpu, sim, o, oracle_mod, TOL64, True, "chunk %d hints %#x" % (chunk, hints))
-            got = sim.read_macro() + tuple(sim.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
-            for a, b in zip(got, want):   # z walls: other tiles take the separately compiled boundary instantiation
-                assert np.array_equal(a, b) if periodic else _maxabs(a, b) <= 1e-13, (chunk, hints)
-            sim.set_schedule(0, 0); sim.step(1)
-            sim.destroy()
-        o.close()
-    # not built for 2D / fp32 contexts
-    sim = gpu.LBM(wl.base_params(40, 20, 1), 64)
-    with pytest.raises(gpu.LBMError):
-        sim.set_schedule(4, 0)
-    sim.set_schedule(0, 0)
-    sim.destroy()
-
-
 # ---------------------------------------------------------------------------- model variants (SURVEY.md 8(f) #4)
 _VARIANTS = (dict(grad_scheme="biased1"), dict(grad_scheme="biased2"), dict(div_scheme="stencil"),
              dict(grad_scheme="biased2", div_scheme="stencil"))
@@ -370,10 +331,12 @@ def test_model_variants_other_modes(gpu, oracle_mod):
         assert _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30) <= REL32, name
     sim.destroy(); o.close()
     Q = dict(P); Q["halo"] = (1, 1)
-    with pytest.raises(gpu.LBMError, match="not built"):
-        gpu.LBM(Q, 64)
     with pytest.raises(gpu.LBMError):
-        gpu.LBM(dict(P, kernels=()), 64).set_schedule(4, 0)
+        gpu.LBM(Q, 64)
+    sim = gpu.LBM(P, 64); sim.init(*init)
+    with pytest.raises(gpu.LBMError, match="not built"):     # LBM_E_UNSUPPORTED: partial launches
+        sim.step_layers(0, 0, 4, False, False)
+    sim.destroy()
 
 
 # ---------------------------------------------------------------------------- D3Q15 Navier-Stokes lattice
