@@ -74,6 +74,7 @@ enum { LBM_DIV_PRODUCT = 0, LBM_DIV_STENCIL = 1 };
 #define LBM_FLAG_POPS_STAGED 32u  /* K_main stages the populations in shared memory with cp.async (default elsewhere)      */
 #define LBM_FLAG_PHI_LDG 64u      /* K_main reads the phi stencil through L1 instead of a TMA box                         */
 #define LBM_FLAG_NO_PDL 256u      /* K_main not launched with programmatic dependent launch behind K_phi                  */
+#define LBM_FLAG_ONE_NODE 512u    /* fp32 3D: K_main with one node per thread instead of a pair of x-adjacent nodes           */
 #define LBM_FLAG_NO_GRAPH 128u    /* no CUDA-graph replay of the steps of small grids                                      */
 
 /* error codes */

@@ -24,9 +24,9 @@ FLAG_PHASE_CHANGE = 1
 FLAG_LATENT_HEAT = 2
 FLAG_PRESCRIBED_U = 4
 # kernel selection (include/lbm.h): speed only, never the method
-FLAG_POPS_GATHER, FLAG_POPS_STAGED, FLAG_PHI_LDG, FLAG_NO_GRAPH, FLAG_NO_PDL = 16, 32, 64, 128, 256
+FLAG_POPS_GATHER, FLAG_POPS_STAGED, FLAG_PHI_LDG, FLAG_NO_GRAPH, FLAG_NO_PDL, FLAG_ONE_NODE = 16, 32, 64, 128, 256, 512
 KERNEL_FLAGS = {"pops_gather": FLAG_POPS_GATHER, "pops_staged": FLAG_POPS_STAGED,
-                "phi_ldg": FLAG_PHI_LDG, "no_graph": FLAG_NO_GRAPH, "no_pdl": FLAG_NO_PDL}
+                "phi_ldg": FLAG_PHI_LDG, "no_graph": FLAG_NO_GRAPH, "no_pdl": FLAG_NO_PDL, "one_node": FLAG_ONE_NODE}
 POPS_F, POPS_G, POPS_S = 0, 1, 2
 STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1

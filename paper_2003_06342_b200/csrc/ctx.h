@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "pairs.cuh"
 
 namespace lbm {
 
@@ -70,13 +71,16 @@ struct lbm_ctx {
     long long nsteps, launches;
     lbm::DevParams<double> pd;
     lbm::DevParams<float> pf;
+    lbm::DevParams<lbm::f2> pf2;   // pf with every value doubled into a pair (k_main_pair.cuh)
     int num_sms;
     // K_main variants: phi halo tile staged by TMA, one box per CTA (k_main_phitma.cuh) ...
     bool phi_tma;
     // ... and the pulled populations, phi^n, Pdot staged by per-thread cp.async (k_main_smem.cuh)
     bool pops_smem;
     bool pdl;   // K_main launched with programmatic stream serialisation behind K_phi
-    int attr_done[8];   // kernel attributes set on this context's device: [MODE] K_main
+    bool pair;  // fp32 3D: K_main carries two x-adjacent nodes per thread (k_main_pair.cuh) ...
+    bool pair_smem;   // ... with the pair's populations staged in shared memory (k_main_pair_smem) or gathered into registers
+    int attr_done[12];   // kernel attributes set on this context's device: [MODE] K_main, [8 + MODE] the pair kernel
     // CUDA graph of two consecutive plain steps, for launch-bound (small) grids
     bool graph_ok;
     cudaGraphExec_t graph2;

@@ -3,6 +3,7 @@
 
 #include "ctx.h"
 #include "k_main.cuh"
+#include "k_main_pair.cuh"
 #include "k_main_phitma.cuh"
 #include "k_main_smem.cuh"
 #include "k_phi.cuh"
@@ -107,8 +108,37 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         return cudaLaunchKernelEx(&cfg, kern, P, F, map);
     }
 
+    // two nodes per thread (k_main_pair.cuh): float populations with a double phi, 3D, 128-wide tiles, even rows
+    static constexpr bool PAIRABLE = D == 3 && std::is_same<real, float>::value && std::is_same<sreal, float>::value &&
+                                     std::is_same<preal, double>::value && T::BX == 128;
+    static constexpr int PAIR_THREADS = 512;   // per SM: 128 registers per thread, as the double-precision kernel
+
     template <int MODE> static int launch_main(lbm_ctx *c, const Fields &F, int pnew = 0) {
         if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU && MODE != MODE_STEP_VAR && MODE != MODE_U) {
+            if constexpr (PAIRABLE) {
+                if (c->pair) {
+                    constexpr int PMINB = PAIR_THREADS / (NT / 2);
+                    using PC = PairSmemCfg<LF, LG, LS, T::BX, T::BY, T::BZ>;
+                    auto kern = c->pair_smem ? k_main_pair_smem<LF, LG, LS, MODE, T::BX, T::BY, T::BZ, PMINB, Fields>
+                                             : k_main_pair<LF, LG, LS, MODE, T::BX, T::BY, T::BZ, PMINB, Fields>;
+                    if (c->pair_smem && !c->attr_done[8 + MODE]) {   // per device: this context's first launch sets them
+                        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PC::BYTES));
+                        const int pct = (int)((PMINB * (PC::BYTES + 1024) * 100 + 233471) / 233472);   // as set_smem_attrs
+                        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, pct > 100 ? 100 : pct));
+                        c->attr_done[8 + MODE] = 1;
+                    }
+                    cudaLaunchConfig_t cfg = {};
+                    cfg.gridDim = grid_layers<T>(c); cfg.blockDim = dim3(NT / 2); cfg.stream = c->stream;
+                    cfg.dynamicSmemBytes = c->pair_smem ? PC::BYTES : 0;
+                    cudaLaunchAttribute at[1];
+                    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+                    at[0].val.programmaticStreamSerializationAllowed = 1;
+                    cfg.attrs = at; cfg.numAttrs = c->pdl ? 1 : 0;
+                    CK(cudaLaunchKernelEx(&cfg, kern, c->pf, c->pf2, F, c->map_phi_tile[pnew]));
+                    c->launches++;
+                    return LBM_OK;
+                }
+            }
             if (c->phi_tma && c->pops_smem) {
                 using C = SmemCfg<LF, LG, LS, sreal, preal, T::BX, T::BY, T::BZ>;
                 auto kern = k_main_smem<LF, LG, LS, real, MODE, T::BX, T::BY, T::BZ, MINB, Fields>;

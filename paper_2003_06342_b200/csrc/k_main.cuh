@@ -6,6 +6,7 @@
 #pragma once
 
 #include "kernels.cuh"
+#include "pairs.cuh"
 
 namespace lbm {
 
@@ -13,9 +14,21 @@ namespace lbm {
 template <class sreal, class real> __device__ __forceinline__ void st_pop(sreal *p, real v) {
     *p = sreal(v);
 }
+// a pair of x-adjacent nodes (pairs.cuh): one 8-byte store; the first node's index is even
+__device__ __forceinline__ void st_pop(float *p, f2 v) { *reinterpret_cast<float2 *>(p) = make_float2(v.x, v.y); }
+__device__ __forceinline__ void st_pop(float *p, d2 v) { *reinterpret_cast<float2 *>(p) = make_float2((float)v.x, (float)v.y); }
 
 __device__ __forceinline__ double rsqrt_(double a) { return rsqrt(a); }
 __device__ __forceinline__ float rsqrt_(float a) { return rsqrtf(a); }
+__device__ __forceinline__ f2 rsqrt_(f2 a) { return f2(rsqrtf(a.x), rsqrtf(a.y)); }
+
+// value types of one work item: those of the field arrays, or pairs of them when a thread carries two nodes (real = f2)
+template <class real, class Fields> struct NodeTypes { using sreal = typename Fields::sreal; using preal = typename Fields::preal; };
+template <class Fields> struct NodeTypes<f2, Fields> { using sreal = float; using preal = d2; };
+
+// a value as the storage type will hold it
+template <class sreal, class real> __device__ __forceinline__ real as_stored(real v) { return real(sreal(v)); }
+template <class sreal> __device__ __forceinline__ f2 as_stored(f2 v) { return v; }   // float storage of float pairs
 
 // Source of one node's inputs, direct variant: gathers straight from global memory (pull with wrap / boundary
 // rules); the phi^{n+1} neighbourhood comes from the padded array through L1/L2.
@@ -66,11 +79,12 @@ template <class LF, class LG, class LS, class real, bool BC, class Fields = DevF
     }
 };
 
-template <class LF, class LG, class LS, class real, int MODE, class Src, class Fields>
-__device__ __forceinline__ void node_update(const DevParams<real> &P, const Fields &Fd, const NodeGeom &g,
+// Geom: NodeGeom, or NodeGeom2 for a pair of nodes (k_main_pair.cuh) -- only the linear index n of the (first) node is used here.
+template <class LF, class LG, class LS, class real, int MODE, class Src, class Fields, class Geom>
+__device__ __forceinline__ void node_update(const DevParams<real> &P, const Fields &Fd, const Geom &g,
                                             const Src &src) {
-    using sreal = typename Fields::sreal;
-    using preal = typename Fields::preal;   // phi arrays; differences of phi are taken in this type, then narrowed
+    using sreal = typename NodeTypes<real, Fields>::sreal;
+    using preal = typename NodeTypes<real, Fields>::preal;   // phi arrays; differences of phi are taken in this type, then narrowed
     const unsigned n = g.n;
     const unsigned N = (unsigned)P.N;
 
@@ -182,8 +196,8 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
             ux = real(Fd.u[n]); uy = real(Fd.u[N + n]); uz = (LF::D == 3) ? real(Fd.u[2 * N + n]) : real(0);
         }
         if constexpr (MODE == MODE_U) {         // velocity pass: u^{n+1} of this node for its neighbours' stencil divergence
-            Fd.u[n] = sreal(ux); Fd.u[N + n] = sreal(uy);
-            if constexpr (LF::D == 3) Fd.u[2 * N + n] = sreal(uz);
+            st_pop(Fd.u + n, ux); st_pop(Fd.u + (N + n), uy);
+            if constexpr (LF::D == 3) st_pop(Fd.u + (2 * N + n), uz);
             return;
         }
         if constexpr (MODE == MODE_STEP_VAR) {  // prescribed, or already in the array (the value the neighbours saw)
@@ -207,17 +221,17 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     if (P.phase_change) {
         const real theta = P.CpL * (T - P.T_sat);
         // this level's collision and the next level's moment corrections use the SAME value (reading S3): the stored one
-        pdot = real(sreal(P.pc_coef * alpha * (theta - P.theta_I) * phi * (real(1) - phi)));
+        pdot = as_stored<sreal>(real(P.pc_coef * alpha * (theta - P.theta_I) * phi * (real(1) - phi)));
     }
-    Fd.pdot[n] = sreal(pdot);
+    st_pop(Fd.pdot + n, pdot);
     if constexpr (MODE == MODE_STEP_MACRO) {
-        Fd.u[n] = sreal(ux); Fd.u[N + n] = sreal(uy); Fd.u[2 * N + n] = sreal(uz);
-        Fd.p[n] = sreal(p); Fd.T[n] = sreal(T);
+        st_pop(Fd.u + n, ux); st_pop(Fd.u + (N + n), uy); st_pop(Fd.u + (2 * N + n), uz);
+        st_pop(Fd.p + n, p); st_pop(Fd.T + n, T);
     }
-    if constexpr (MODE == MODE_STEP_PU) { Fd.p[n] = sreal(p); Fd.T[n] = sreal(T); }
+    if constexpr (MODE == MODE_STEP_PU) { st_pop(Fd.p + n, p); st_pop(Fd.T + n, T); }
     if constexpr (MODE == MODE_STEP_VAR) {
-        Fd.p[n] = sreal(p); Fd.T[n] = sreal(T);
-        if (!(P.prescribed_u || P.div_scheme)) { Fd.u[n] = sreal(ux); Fd.u[N + n] = sreal(uy); Fd.u[2 * N + n] = sreal(uz); }
+        st_pop(Fd.p + n, p); st_pop(Fd.T + n, T);
+        if (!(P.prescribed_u || P.div_scheme)) { st_pop(Fd.u + n, ux); st_pop(Fd.u + (N + n), uy); st_pop(Fd.u + (2 * N + n), uz); }
     }
 
     // ---- H7: sources, equilibria, BGK (Eq.25)

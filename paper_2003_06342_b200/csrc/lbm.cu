@@ -258,6 +258,7 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
     c->cur = 0; c->curphi = 0; c->phase = 0; c->partial = false; c->inited = false; c->nsteps = 0; c->launches = 0; c->timing = false;
     c->pd = make_dev_params<double>(p, L);
     c->pf = make_dev_params<float>(p, L);
+    c->pf2 = make_dev_params<f2>(p, L);
     c->num_sms = prop.multiProcessorCount;
     {   // Kernel variants, chosen by measurement; lbm_params.flags can force the plainer ones.
         const unsigned fl = p->flags;
@@ -272,6 +273,10 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         // fp64 (+3..9% on every large grid) and fp32 in 2D (+8%); fp32 3D stays on the register gather (-1..5%)
         const bool smem_default = p->precision == 64 || p->nz == 1;
         c->pops_smem = c->phi_tma && ((fl & LBM_FLAG_POPS_STAGED) ? true : (fl & LBM_FLAG_POPS_GATHER) ? false : smem_default);
+        // fp32 3D on 128-wide tiles with even rows: two x-adjacent nodes per thread, packed f32x2 arithmetic (k_main_pair.cuh)
+        c->pair = c->phi_tma && p->precision == 32 && p->nz > 1 && c->ops->bx == 128 && p->nx % 2 == 0 && !(fl & LBM_FLAG_ONE_NODE);
+        c->pair_smem = c->pair && !(fl & LBM_FLAG_POPS_GATHER);
+        if (c->pair) c->pops_smem = false;
     }
     *out = c;
     return LBM_OK;
@@ -376,6 +381,7 @@ long long lbm_launch_count(const lbm_ctx *c) { return c ? c->launches : -1; }
 const char *lbm_variant(const lbm_ctx *c) {
     if (!c) return "";
     if (c->P.grad_scheme || c->P.div_scheme) return "direct (model variant)";
+    if (c->pair) return c->pair_smem ? "pair+smem" : "pair+phi-tma";
     return c->phi_tma ? (c->pops_smem ? "gather+smem" : "gather+phi-tma") : "direct";
 }
 int lbm_last_cuda_error(void) { return g_last_cuda_error; }

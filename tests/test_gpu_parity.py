@@ -229,25 +229,39 @@ def test_kernel_variants(gpu, oracle_mod):
     P3z["bc_T"][2] = [1.0, 0.0]
     cases = ((P3, 34), (P3w, 44), (P2, 35), (P2w, 45), (P3z, 46))
     # (flags, variant of the wide 3D case in fp64, in fp32)
-    for names, want64, want32 in (((), "gather+smem", "gather+phi-tma"),
-                                  (("pops_gather",), "gather+phi-tma", "gather+phi-tma"),
-                                  (("pops_staged",), "gather+smem", "gather+smem"),
-                                  (("no_pdl",), "gather+smem", "gather+phi-tma"),
+    for names, want64, want32 in (((), "gather+smem", "pair+smem"),
+                                  (("pops_gather",), "gather+phi-tma", "pair+phi-tma"),
+                                  (("pops_staged",), "gather+smem", "pair+smem"),
+                                  (("no_pdl",), "gather+smem", "pair+smem"),
+                                  (("one_node",), "gather+smem", "gather+phi-tma"),
+                                  (("one_node", "pops_staged"), "gather+smem", "gather+smem"),
                                   (("phi_ldg",), "direct", "direct")):
         sim = gpu.LBM(_with_kernels(P3w, *names), 64); assert sim.variant == want64, (names, sim.variant); sim.destroy()
         sim = gpu.LBM(_with_kernels(P3w, *names), 32); assert sim.variant == want32, (names, sim.variant); sim.destroy()
         for P, seed in cases:
             _run_parity(gpu, oracle_mod, _with_kernels(P, *names), _random_state(P, seed), [1, 12],
                         label="%s %dx%dx%d" % (names, P["nx"], P["ny"], P["nz"]))
-    # fp32 with the staged kernel (3D opt-in, 2D default): inside the fp32 bar
-    for P, seed in ((P3w, 44), (P2w, 45)):
+    # fp32: two nodes per thread (k_main_pair.cuh: the 3D default on 128-wide tiles, populations staged or gathered; periodic tiles
+    # run the packed f32x2 code, tiles on the z walls of P3z the one-node code twice per thread) and one node per thread (gathered,
+    # staged; the 2D default): every one inside the fp32 bar on fields and on the float populations
+    P3r = wl.base_params(250, 5, 4, grav=[1e-4, 0.0, -2e-4])                     # ragged last tile (250 = 128 + 122)
+    for P, seed, names, want in ((P3w, 44, ("one_node", "pops_staged"), "gather+smem"), (P2w, 45, ("pops_staged",), "gather+smem"),
+                                 (P3w, 44, (), "pair+smem"), (P3w, 44, ("pops_gather",), "pair+phi-tma"), (P3w, 44, ("one_node",), "gather+phi-tma"),
+                                 (P3z, 46, (), "pair+smem"), (P3z, 46, ("pops_gather",), "pair+phi-tma"), (P3z, 46, ("one_node",), "gather+phi-tma"),
+                                 (P3r, 47, (), "pair+smem"), (P3r, 47, ("pops_gather",), "pair+phi-tma"), (P3r, 47, ("one_node",), "gather+phi-tma")):
         init = _random_state(P, seed)
         o = oracle_mod.Oracle(P); o.init(*init); o.step(12)
-        sim = gpu.LBM(_with_kernels(P, "pops_staged"), 32); sim.init(*[a.astype(np.float32) for a in init]); sim.step(12)
-        assert sim.variant == "gather+smem"
+        sim = gpu.LBM(_with_kernels(P, *names), 32); sim.init(*[a.astype(np.float32) for a in init]); sim.step(6); sim.step(6)
+        assert sim.variant == want, (names, sim.variant)
         for a, b, name in zip(sim.read_macro(), o.read_macro(), ("phi", "u", "p", "T")):
-            assert _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30) <= REL32, name
+            assert _maxabs(a, b) / max(float(np.abs(b).max()), 1e-30) <= REL32, (names, name)
+        for which in range(3):    # the float populations themselves, both stages
+            for stage, ostage in ((gpu.STAGE_POSTCOLLISION, oracle_mod.POPS_POSTCOLLISION), (gpu.STAGE_STREAMED, oracle_mod.POPS_STREAMED)):
+                a, b = sim.read_pops(which, stage), o.read_pops(which, ostage)
+                assert _maxabs(a, b) / float(np.abs(b).max()) <= REL32, (names, which, stage)
         sim.destroy(); o.close()
+    # odd rows cannot pair: the one-node kernel runs
+    sim = gpu.LBM(wl.base_params(255, 4, 4), 32); assert sim.variant == "gather+phi-tma"; sim.destroy()
 
 
 def test_cuda_graph_replay_on_side_stream(gpu, oracle_mod):
