@@ -200,6 +200,15 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         const int in = c->cur, pnew = 1 - c->curphi;
         dim3 gphi = grid_layers<TP>(c);
         if (D == 3) gphi.z = (gphi.z + PHI_NPT - 1) / PHI_NPT; else gphi.y = (gphi.y + PHI_NPT - 1) / PHI_NPT;
+        if constexpr (PAIRABLE) {
+            if (c->pair) {   // two x-adjacent nodes per thread (k_main_pair.cuh)
+                k_phi_pair<LG, TP::BX, TP::BY, TP::BZ, PHI_NPT><<<gphi, NTP / 2, 0, c->stream>>>(
+                    c->pf, (const float *)wsp<float>(c, c->L.off_g[in]), wsp<double>(c, c->L.off_phi[pnew]));
+                c->launches++;
+                CK(cudaGetLastError());
+                return LBM_OK;
+            }
+        }
         k_phi<LG, real, TP::BX, TP::BY, TP::BZ, PHI_NPT><<<gphi, NTP, 0, c->stream>>>(
             P, (const sreal *)wsp<sreal>(c, c->L.off_g[in]), wsp<preal>(c, c->L.off_phi[pnew]));
         c->launches++;

@@ -8,6 +8,7 @@
 #pragma once
 
 #include "k_main_smem.cuh"
+#include "k_phi.cuh"
 #include "pairs.cuh"
 
 namespace lbm {
@@ -264,6 +265,76 @@ k_main_pair(const DevParams<float> P, const DevParams<f2> P2, const Fields Fd, c
         const NodeGeom2 g = make_geom2(P, x, y, z);
         const SrcPair<LF, LG, LS, TC, Fields> src(P, Fd, g, tile, bar_a, x, y, z, tx, ty, tz);
         node_update<LF, LG, LS, f2, MODE>(P2, Fd, g, src);
+    }
+}
+
+}  // namespace lbm
+
+namespace lbm {
+
+// ---- K_phi for pairs (float populations, double phi, 3D): phi^{n+1} of the two nodes by the error-free sum of k_phi.cuh in packed
+// arithmetic (the one-node kernel is issue-bound in float: 69% of the issue slots at 55% of the DRAM peak), 8-byte loads where the
+// link does not move in x, one 16-byte store of the two doubles.  Nodes with ghost images and tiles on non-periodic faces take
+// the one-node code.
+__device__ __forceinline__ void two_sum2(f2 &hi, f2 &lo, f2 v) {   // Knuth: hi + lo + v = hi' + lo' exactly, both nodes at once
+    const f2 s = add2(hi, v);
+    const f2 bb = add2(s, -hi);
+    lo = add2(lo, add2(add2(hi, -add2(s, -bb)), add2(v, -bb)));
+    hi = s;
+}
+
+template <class LG, int BX, int BY, int BZ, int NPT>
+__global__ void __launch_bounds__(BX / 2 * BY *BZ)
+k_phi_pair(const DevParams<float> P, const float *__restrict__ g_in, double *__restrict__ phi_new) {
+    pdl_launch_dependents();   // as k_phi
+    constexpr int HX = BX / 2;
+    const int t = threadIdx.x;
+    const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY, z0 = P.s0 + blockIdx.z * BZ * NPT;   // this launch covers the layers [P.s0, P.s1)
+    const int x = x0 + 2 * (t % HX), y = y0 + (t / HX) % BY, zb = z0 + t / (HX * BY);
+    if (x >= P.nx || y >= P.ny) return;   // nx is even
+    const unsigned N = (unsigned)P.N;
+    if (tile_touches_bc(P, x0, y0, z0, BX, BY, BZ * NPT)) {
+#pragma unroll 1
+        for (int j = 0; j < 2 * NPT; ++j) {
+            const int z = zb + (j >> 1) * BZ;
+            if (z >= P.s1) break;
+            const NodeGeom g = make_geom(P, x + (j & 1), y, z);
+            float gi[LG::Q];
+            pull<LG, float, true>(g_in, N, g, P.bc_g, P.bc_phi, gi);
+            store_phi_with_images(phi_new, P, g, phi_sum<double>(gi));
+        }
+        return;
+    }
+    f2 gi[NPT][LG::Q];
+    bool ok[NPT];
+#pragma unroll
+    for (int j = 0; j < NPT; ++j) {
+        const int z = zb + j * BZ;
+        ok[j] = z < P.s1;
+        if (ok[j]) {
+            const NodeGeom2 g = make_geom2(P, x, y, z);
+            static_for<LG::Q>([&](auto ic) {
+                constexpr int I = decltype(ic)::value;
+                gi[j][I] = pull_pair<LG, I, false>(g_in, N, g);
+            });
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < NPT; ++j) {
+        if (!ok[j]) continue;
+        const int z = zb + j * BZ;
+        f2 hi = gi[j][0], lo = f2(0.0f);
+#pragma unroll
+        for (int i = 1; i < LG::Q; ++i) two_sum2(hi, lo, gi[j][i]);
+        const double v0 = (double)hi.x + (double)lo.x, v1 = (double)hi.y + (double)lo.y;
+        const bool edge = x == 0 || x + 2 == P.nx || y == 0 || y == P.ny - 1 || z == 0 || z == P.nz - 1;
+        if (!edge) {
+            const long long pc = ((long long)(z + P.pz) * P.ppy + (y + 1)) * P.ppx + (x + P.xpad);
+            *reinterpret_cast<double2 *>(phi_new + pc) = make_double2(v0, v1);   // x and xpad are even: 16-byte aligned
+        } else {
+            store_phi_with_images(phi_new, P, make_geom(P, x, y, z), v0);
+            store_phi_with_images(phi_new, P, make_geom(P, x + 1, y, z), v1);
+        }
     }
 }
 
