@@ -284,8 +284,10 @@ def run_ours(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
         "config": {"workload": args.workload, "grid": [nx, ny, nz], "lattices": [P["lat_f"], P["lat_g"], P["lat_s"]],
                    "parallelism": "replicas x%d" % world, "variant": sim.variant,
-                   "l2": "state (%.1f GB) is far larger than L2; no flush needed" % (sim.workspace_bytes / 1e9)
-                   if sim.workspace_bytes > 1e9 else "state fits L2: numbers are L2-resident",
+                   "l2": "state (%.2f GB) is larger than the 126 MB L2; no flush needed" % (sim.workspace_bytes / 1e9)
+                   if sim.workspace_bytes > 4 * 126e6 else
+                   ("state (%.0f MB) is not far above the 126 MB L2: partly L2-resident, no flush" % (sim.workspace_bytes / 1e6)
+                    if sim.workspace_bytes > 126e6 else "state fits L2: numbers are L2-resident"),
                    "finite": finite},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "MLUPS", "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,

@@ -14,8 +14,10 @@
  * tags G* / S* in comments refer to that list.
  *
  * Parity unpinned: nothing outright; two READINGS the paper cannot confirm stay readings.
- * div(u phi) (S5) is pinned as far as the paper's equations reach: u.grad(phi) by Galilean invariance of the latent-heat
- * source, phi div u by the Eq.(11a) mass balance; only "pointwise product, not a stencil divergence" is a choice.
+ * div(u phi): the paper does not say how it discretised it.  Both candidates are here and both are pinned: the product rule of
+ * reading S5 (u.grad(phi) by Galilean invariance of the latent-heat source, phi div u by the Eq.(11a) mass balance) and the
+ * stencil divergence of reading S17 (equal to u.grad(phi) for uniform u, exact on quadratic fluxes, wall / open ghost rule);
+ * which of the two the paper's authors ran is what stays open.
  * The OPEN pressure face (S12, not in the paper) is pinned in the role config 2 gives it -- normal outflow at a fixed
  * pressure: exact hydrostatic column, outflow = integrated mass source; its behaviour under shear is not (a 32 x 16
  * pressure-driven channel carries 6.5 % more flux than Poiseuille's law, entry effect of the plain anti-bounce-back).

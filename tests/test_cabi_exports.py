@@ -50,6 +50,13 @@ def test_sass_has_tma_and_async_copies(lib):
         assert "UTMALDG" in f and "LDGSTS" in f and "SYNCS" in f, f[:200]
     phitma = [f for f in funcs if f.startswith("_ZN3lbm13k_main_phitma")]
     assert phitma and all("UTMALDG" in f for f in phitma)
+    # fp32 3D: two nodes per thread -- the packed f32x2 arithmetic of sm_100 and the staged pair copies (k_main_pair.cuh)
+    pair = [f for f in funcs if f.startswith("_ZN3lbm16k_main_pair_smem")]
+    assert len(pair) >= 4
+    for f in pair:
+        assert f.count("FFMA2") >= 50 and f.count("FADD2") >= 50 and "UTMALDG" in f and "LDGSTS" in f, f[:200]
+    kphi_pair = [f for f in funcs if f.startswith("_ZN3lbm10k_phi_pair")]
+    assert kphi_pair and all(f.count("FADD2") >= 30 for f in kphi_pair)
 
 
 def test_workspace_bytes_accounting(lib):
