@@ -114,7 +114,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     static constexpr int PAIR_THREADS = 512;   // per SM: 128 registers per thread, as the double-precision kernel
 
     template <int MODE> static int launch_main(lbm_ctx *c, const Fields &F, int pnew = 0) {
-        if constexpr (MODE != MODE_INIT && MODE != MODE_STEP_PU && MODE != MODE_STEP_VAR && MODE != MODE_U) {
+        if constexpr (MODE == MODE_STEP || MODE == MODE_STEP_MACRO) {
             if constexpr (PAIRABLE) {
                 if (c->pair) {
                     constexpr int PMINB = PAIR_THREADS / (NT / 2);
@@ -186,7 +186,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         CK(cudaGetLastError());
         c->cur = 0; c->curphi = 0;
         Fields F = fields(c, 1, 0, 0, 0);   // INIT reads no populations; writes buffer 0
-        int rc = launch_main<MODE_INIT>(c, F);
+        int rc = (P.grad_scheme || P.div_scheme) ? launch_main<MODE_INIT_VAR>(c, F) : launch_main<MODE_INIT>(c, F);
         if (rc) return rc;
         CK(cudaStreamSynchronize(c->stream));
         c->nsteps = 0;

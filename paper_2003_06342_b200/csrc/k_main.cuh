@@ -91,7 +91,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     // ---- H5 (first half): zeroth moment of s.  Loaded first so that these loads are in flight during the stencil.
     src.pops_ready();   // staged variants: the node's asynchronous copies have landed
     real sum_s = real(0);
-    if constexpr (MODE != MODE_INIT) {
+    if constexpr (!mode_is_init<MODE>::value) {
         static_for<LS::Q>([&](auto ic) { sum_s += src.template s<decltype(ic)::value>(); });
     }
 
@@ -153,7 +153,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     // (this level's u of every node: the input at initialisation, written by the MODE_U pass before a step) -- reading S17
     real D_st = real(0);
     bool use_st = false;
-    if constexpr (MODE == MODE_INIT || MODE == MODE_STEP_VAR) {
+    if constexpr (MODE == MODE_INIT_VAR || MODE == MODE_STEP_VAR) {
         if (P.div_scheme) {
             use_st = true;
             static_for<LF::Q>([&](auto ic) {
@@ -173,7 +173,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
 
     real ux, uy, uz, p, T, dtphi;
     real pd_old = real(0);   // production rate of the previous level: in the moment corrections and folded into the stored g_0
-    if constexpr (MODE == MODE_INIT) {
+    if constexpr (mode_is_init<MODE>::value) {
         ux = real(Fd.u[n]); uy = real(Fd.u[N + n]); uz = (LF::D == 3) ? real(Fd.u[2 * N + n]) : real(0);
         p = real(Fd.p[n]); T = real(Fd.T[n]); dtphi = real(0);
     } else {
@@ -250,9 +250,9 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     //    so out_i = a bar_i + (Gamma_i - w_i)(K1 + b c_i.H) + w_i (K2 + b c_i.F),
     //    K1 = om rho cs2 - b u.H,  K2 = om p + b (rho cs2 mdot Drho - u.F).
     {
-        const real om = MODE == MODE_INIT ? real(1) : om_f;
-        const real a = MODE == MODE_INIT ? real(0) : real(1) - om_f;
-        const real b = MODE == MODE_INIT ? P.hdt : P.dt * (real(1) - real(0.5) * om_f);
+        const real om = mode_is_init<MODE>::value ? real(1) : om_f;
+        const real a = mode_is_init<MODE>::value ? real(0) : real(1) - om_f;
+        const real b = mode_is_init<MODE>::value ? P.hdt : P.dt * (real(1) - real(0.5) * om_f);
         const real ic = P.c_cs2f;
         const real tx = ux * ic, ty = uy * ic, tz = uz * ic;          // c u / cs2
         const real U = real(-0.5) * uu * P.inv_cs2f;
@@ -266,7 +266,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
         {   // rest direction: t = 0
             constexpr real w = real(LF::w(0));
             real bar = real(0);
-            if constexpr (MODE != MODE_INIT) bar = src.template f<0, true>();
+            if constexpr (!mode_is_init<MODE>::value) bar = src.template f<0, true>();
             st_pop(Fd.f_out + (n), a * bar + w * (U * K1 + K2));
         }
         static_for<LF::Q>([&](auto icn) {
@@ -275,7 +275,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
                 constexpr int J = LF::opp(I);
                 constexpr real w = real(LF::w(I));
                 real bi = real(0), bj = real(0);
-                if constexpr (MODE != MODE_INIT) { bi = src.template f<I, true>(); bj = src.template f<J, true>(); }
+                if constexpr (!mode_is_init<MODE>::value) { bi = src.template f<I, true>(); bj = src.template f<J, true>(); }
                 const real t = dot_e<LF, I, real>(tx, ty, tz);
                 const real q = real(0.5) * t * t + U;
                 const real h = dot_e<LF, I, real>(Hbx, Hby, Hbz);
@@ -287,9 +287,9 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     }
     // -- temperature (Eq.33a-d, sign of reading G2): eq_i = T Gamma_i, S_i = -w_i (L/Cp)(dphi/dt + D)
     {
-        const real om = MODE == MODE_INIT ? real(1) : om_s;
-        const real a = MODE == MODE_INIT ? real(0) : real(1) - om_s;
-        const real b = MODE == MODE_INIT ? P.hdt : P.dt * (real(1) - real(0.5) * om_s);
+        const real om = mode_is_init<MODE>::value ? real(1) : om_s;
+        const real a = mode_is_init<MODE>::value ? real(0) : real(1) - om_s;
+        const real b = mode_is_init<MODE>::value ? P.hdt : P.dt * (real(1) - real(0.5) * om_s);
         const real ic = P.c_cs2s;
         const real tx = ux * ic, ty = uy * ic, tz = uz * ic;
         const real U1 = real(1) - real(0.5) * uu * P.inv_cs2s;
@@ -298,7 +298,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
         {
             constexpr real w = real(LS::w(0));
             real bar = real(0);
-            if constexpr (MODE != MODE_INIT) bar = src.template s<0, true>();
+            if constexpr (!mode_is_init<MODE>::value) bar = src.template s<0, true>();
             st_pop(Fd.s_out + (n), a * bar + w * (TO * U1 + bQ));
         }
         static_for<LS::Q>([&](auto icn) {
@@ -307,7 +307,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
                 constexpr int J = LS::opp(I);
                 constexpr real w = real(LS::w(I));
                 real bi = real(0), bj = real(0);
-                if constexpr (MODE != MODE_INIT) { bi = src.template s<I, true>(); bj = src.template s<J, true>(); }
+                if constexpr (!mode_is_init<MODE>::value) { bi = src.template s<I, true>(); bj = src.template s<J, true>(); }
                 const real t = dot_e<LS, I, real>(tx, ty, tz);
                 const real q = real(0.5) * t * t + U1;
                 st_pop(Fd.s_out + ((unsigned)I * N + n), a * bi + w * (TO * (q + t) + bQ));
@@ -322,9 +322,9 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
     {
         using greal = preal;
         const greal om_g = greal(P.g_om), dtg = greal(P.g_dt);   // constants carried in double: no widening per node
-        const greal om = MODE == MODE_INIT ? greal(1) : om_g;
-        const greal a = MODE == MODE_INIT ? greal(0) : greal(1) - om_g;
-        const greal b = MODE == MODE_INIT ? greal(0.5) * dtg : dtg * (greal(1) - greal(0.5) * om_g);
+        const greal om = mode_is_init<MODE>::value ? greal(1) : om_g;
+        const greal a = mode_is_init<MODE>::value ? greal(0) : greal(1) - om_g;
+        const greal b = mode_is_init<MODE>::value ? greal(0.5) * dtg : dtg * (greal(1) - greal(0.5) * om_g);
         const greal ic = greal(P.g_c_cs2);
         const greal tx = greal(ux) * ic, ty = greal(uy) * ic, tz = greal(uz) * ic;
         const greal U1 = greal(1) - greal(0.5) * greal(uu) * greal(P.g_inv_cs2);
@@ -341,7 +341,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
             constexpr greal w = greal(LG::w(0));
             const greal hdtg = greal(0.5) * dtg;
             greal bar = greal(0);
-            if constexpr (MODE != MODE_INIT) bar = greal(src.template gg<0>()) - hdtg * greal(pd_old);
+            if constexpr (!mode_is_init<MODE>::value) bar = greal(src.template gg<0>()) - hdtg * greal(pd_old);
             st_pop(Fd.g_out + (n), a * bar + w * (PO * U1 + bP) + hdtg * greal(pdot));
         }
         static_for<LG::Q>([&](auto icn) {
@@ -350,7 +350,7 @@ __device__ __forceinline__ void node_update(const DevParams<real> &P, const Fiel
                 constexpr int J = LG::opp(I);
                 constexpr greal w = greal(LG::w(I));
                 greal bi = greal(0), bj = greal(0);
-                if constexpr (MODE != MODE_INIT) { bi = greal(src.template gg<I>()); bj = greal(src.template gg<J>()); }
+                if constexpr (!mode_is_init<MODE>::value) { bi = greal(src.template gg<I>()); bj = greal(src.template gg<J>()); }
                 const greal t = dot_e<LG, I, greal>(tx, ty, tz);
                 const greal q = greal(0.5) * t * t + U1;
                 const greal cn = dot_e<LG, I, greal>(bx, by, bz);

@@ -26,9 +26,11 @@ enum { BC_PERIODIC = 0, BC_BOUNCE = 1 /* wall / zero-flux */, BC_ANTI = 2 /* ope
 // MODE_STEP_VAR: step with one of the model variants of lbm_params.grad_scheme / div_scheme (biased directional derivatives,
 // PAPER.md:318; stencil divergence of u phi, reading S17); stores u, p, T every step.  MODE_U: the velocity pass
 // that precedes it when the divergence is a stencil (u^{n+1} of every node, Eq.28a, and nothing else).
-enum { MODE_STEP = 0, MODE_STEP_MACRO = 1, MODE_INIT = 2, MODE_STEP_PU = 3, MODE_STEP_VAR = 4, MODE_U = 5 };
-// modes that know the variants (all run the direct kernel; the production kernels carry no trace of them)
-template <int MODE> struct mode_has_variants { static constexpr bool value = MODE == MODE_INIT || MODE == MODE_STEP_VAR || MODE == MODE_U; };
+// MODE_INIT_VAR: initialisation with a variant.
+enum { MODE_STEP = 0, MODE_STEP_MACRO = 1, MODE_INIT = 2, MODE_STEP_PU = 3, MODE_STEP_VAR = 4, MODE_U = 5, MODE_INIT_VAR = 6 };
+// modes that know the variants (all run the direct kernel; the production kernels and the plain initialisation carry no trace of them)
+template <int MODE> struct mode_has_variants { static constexpr bool value = MODE == MODE_INIT_VAR || MODE == MODE_STEP_VAR || MODE == MODE_U; };
+template <int MODE> struct mode_is_init { static constexpr bool value = MODE == MODE_INIT || MODE == MODE_INIT_VAR; };
 
 // ---- compile-time loop over directions ---------------------------------------------------------------
 template <class F, int... I>
