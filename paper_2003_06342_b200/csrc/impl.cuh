@@ -108,9 +108,9 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
         return cudaLaunchKernelEx(&cfg, kern, P, F, map);
     }
 
-    // two nodes per thread (k_main_pair.cuh): float populations with a double phi, 3D, 128-wide tiles, even rows
+    // two nodes per thread (k_main_pair.cuh): float populations with a double phi, 3D, 128- or 64-wide tiles, even rows
     static constexpr bool PAIRABLE = D == 3 && std::is_same<real, float>::value && std::is_same<sreal, float>::value &&
-                                     std::is_same<preal, double>::value && T::BX == 128;
+                                     std::is_same<preal, double>::value && (T::BX == 128 || T::BX == 64);
     static constexpr int PAIR_THREADS = 512;   // per SM: 128 registers per thread, as the double-precision kernel
 
     template <int MODE> static int launch_main(lbm_ctx *c, const Fields &F, int pnew = 0) {

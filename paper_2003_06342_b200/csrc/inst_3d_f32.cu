@@ -5,7 +5,7 @@
 namespace lbm {
 const ImplOps *ops_3d_f32(int nx) {
     if (wide_tile_pays(nx)) return Impl<D3Q19, D3Q7, D3Q7, float, TileWide3Phi, float, double>::ops();
-    if (nx >= 64 && nx % 64 == 0) return Impl<D3Q19, D3Q7, D3Q7, float, TileMid3, float, double>::ops();
+    if (nx >= 64 && nx % 64 == 0) return Impl<D3Q19, D3Q7, D3Q7, float, TileMid3Phi, float, double>::ops();   // 64 x 4: 128 threads of pairs
     return Impl<D3Q19, D3Q7, D3Q7, float, TileNarrow3, float, double>::ops();
 }
 }  // namespace lbm

@@ -273,8 +273,8 @@ int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_
         // fp64 (+3..9% on every large grid) and fp32 in 2D (+8%); fp32 3D stays on the register gather (-1..5%)
         const bool smem_default = p->precision == 64 || p->nz == 1;
         c->pops_smem = c->phi_tma && ((fl & LBM_FLAG_POPS_STAGED) ? true : (fl & LBM_FLAG_POPS_GATHER) ? false : smem_default);
-        // fp32 3D on 128-wide tiles with even rows: two x-adjacent nodes per thread, packed f32x2 arithmetic (k_main_pair.cuh)
-        c->pair = c->phi_tma && p->precision == 32 && p->nz > 1 && c->ops->bx == 128 && p->nx % 2 == 0 && !(fl & LBM_FLAG_ONE_NODE);
+        // fp32 3D on 128- or 64-wide tiles with even rows: two x-adjacent nodes per thread, packed f32x2 arithmetic (k_main_pair.cuh)
+        c->pair = c->phi_tma && p->precision == 32 && p->nz > 1 && c->ops->bx >= 64 && p->nx % 2 == 0 && !(fl & LBM_FLAG_ONE_NODE);
         c->pair_smem = c->pair && !(fl & LBM_FLAG_POPS_GATHER);
         if (c->pair) c->pops_smem = false;
     }
