@@ -38,6 +38,19 @@ template <class T> dim3 grid_layers(const lbm_ctx *c) {
     return dim3((P.nx + T::BX - 1) / T::BX, (n + T::BY - 1) / T::BY, 1);
 }
 
+// Shared-memory carve-out (percent of the 228 KB maximum) for `ctas` resident CTAs of `bytes` dynamic shared memory each (+1 KB
+// that the driver reserves per CTA): the smallest configuration of sm_100 that holds them, requested from below so that the
+// rounding of the percentage cannot tip it into the next larger one.  The rest of the 256 KB stays L1 -- the shifted pulls of
+// neighbouring warps share sectors there (measured on config 4, fp64 K_main ms: 60 KB of L1: 2.89, 92 KB: 2.82, and 3.75 with
+// the maximum carve-out).
+inline int carveout_pct(int ctas, size_t bytes) {
+    const size_t need = (size_t)ctas * (bytes + 1024);
+    const size_t sizes[] = {0, 8, 16, 32, 64, 100, 132, 164, 196, 228};
+    size_t pick = 228;
+    for (size_t s : sizes) if (s * 1024 >= need) { pick = s; break; }
+    return (int)(pick * 1024 * 100 / 233472);
+}
+
 template <class real> const DevParams<real> &dev_params(const lbm_ctx *c);
 template <> inline const DevParams<double> &dev_params<double>(const lbm_ctx *c) { return c->pd; }
 template <> inline const DevParams<float> &dev_params<float>(const lbm_ctx *c) { return c->pf; }
@@ -86,11 +99,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
     template <class K> static int set_smem_attrs(lbm_ctx *c, K kern, size_t bytes, int &done_flag) {
         if (done_flag) return LBM_OK;
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-        // shared-memory carve-out: just enough for MINB resident CTAs (+1 KB each that the driver reserves), the rest
-        // stays L1 -- the shifted pulls of neighbouring warps share sectors there (measured on config 4, K_main ms:
-        // 60 KB of L1: 2.89, 92 KB: 2.82, and 3.75 with the maximum carve-out)
-        const int pct = (int)((MINB * (bytes + 1024) * 100 + 233471) / 233472);
-        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, pct > 100 ? 100 : pct));
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, carveout_pct(MINB, bytes)));
         done_flag = 1;
         return LBM_OK;
     }
@@ -123,8 +132,7 @@ template <class LF, class LG, class LS, class real, class T, class sreal = real,
                                              : k_main_pair<LF, LG, LS, MODE, T::BX, T::BY, T::BZ, PMINB, Fields>;
                     if (c->pair_smem && !c->attr_done[8 + MODE]) {   // per device: this context's first launch sets them
                         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PC::BYTES));
-                        const int pct = (int)((PMINB * (PC::BYTES + 1024) * 100 + 233471) / 233472);   // as set_smem_attrs
-                        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, pct > 100 ? 100 : pct));
+                        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, carveout_pct(PMINB, PC::BYTES)));
                         c->attr_done[8 + MODE] = 1;
                     }
                     cudaLaunchConfig_t cfg = {};

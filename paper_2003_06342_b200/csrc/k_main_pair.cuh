@@ -103,16 +103,14 @@ template <class LF, class LG, class LS, int BX, int BY, int BZ> struct PairSmemC
     static constexpr int QT = LF::Q + LS::Q;
     static constexpr int OFF_F = 0, OFF_S = LF::Q, OFF_PDOT = QT;   // float2 slots
     static constexpr size_t TILE_BYTES = ((size_t)TC::BYTES + 127) / 128 * 128;
-    static constexpr size_t PHIOLD_BYTES = (size_t)NT * 2 * sizeof(double);
+    // phi^n is NOT staged (it rides in registers from before the CTA barrier): with it four CTAs would need the 196 KB shared-memory
+    // configuration; without it they fit the 164 KB one and L1 keeps 92 KB for the sectors that x-shifted pulls share (k_main_smem.cuh)
     static constexpr size_t POPS_BYTES = (size_t)(QT + 1) * NT * sizeof(float2);
-    static constexpr size_t BYTES = TILE_BYTES + PHIOLD_BYTES + POPS_BYTES + 16;   // + the mbarrier
+    static constexpr size_t BYTES = TILE_BYTES + POPS_BYTES + 16;   // + the mbarrier
 };
 
 __device__ __forceinline__ void cp_async_8(uint32_t dst, const void *src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_16(uint32_t dst, const void *src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
 
 template <class LF, class LG, class LS, class C, class Fields> struct SrcPairSmem {
@@ -121,18 +119,14 @@ template <class LF, class LG, class LS, class C, class Fields> struct SrcPairSme
     const Fields &Fd;
     const NodeGeom2 &g;
     const double *tile;      // the first node's own element in the phi tile
-    const double2 *phiold;   // this thread's slot
     const float2 *col;       // this thread's column: value k at col[k * NT]
     uint32_t bar;
-    unsigned pcoff;
+    double2 po;              // phi^n of the pair
     __device__ __forceinline__ SrcPairSmem(const DevParams<float> &P_, const Fields &Fd_, const NodeGeom2 &g_, const double *tile_base,
-                                           const double2 *phiold_base, const float2 *pops_base, uint32_t bar_, int t, int x, int y, int z,
-                                           int tx, int ty, int tz)
-        : P(P_), Fd(Fd_), g(g_), bar(bar_) {
+                                           const float2 *pops_base, uint32_t bar_, int t, int tx, int ty, int tz, double2 po_)
+        : P(P_), Fd(Fd_), g(g_), bar(bar_), po(po_) {
         tile = tile_base + ((tz + 1) * TC::BOXY + ty + 1) * TC::BOXX + tx + TC::EPB;
-        phiold = phiold_base + t;
         col = pops_base + t;
-        pcoff = ((unsigned)(z + P.pz) * (unsigned)P.ppy + (unsigned)(y + 1)) * (unsigned)P.ppx + (unsigned)(x + P.xpad);
     }
     // the two values of direction I into one float2 slot: one 8-byte copy, or two 4-byte copies when the link moves in x
     template <class L, int I> __device__ __forceinline__ void copy_pair(uint32_t dst, const float *__restrict__ src, unsigned N) const {
@@ -150,8 +144,7 @@ template <class LF, class LG, class LS, class C, class Fields> struct SrcPairSme
             copy_pair<LS, I>(c0 + (uint32_t)(C::OFF_S + I) * STEP, Fd.s_in, N);
         });
         cp_async_8(c0 + (uint32_t)C::OFF_PDOT * STEP, Fd.pdot_in + g.n);
-        cp_async_16(smem_u32(phiold), Fd.phi_old + pcoff);
-        cp_async_commit();   // group 1: what the stencil and closure phase needs (s, Pdot, phi^n)
+        cp_async_commit();   // group 1: what the stencil and closure phase needs (s, Pdot)
         static_for<LF::Q>([&](auto ic) {
             constexpr int I = decltype(ic)::value;
             copy_pair<LF, I>(c0 + (uint32_t)(C::OFF_F + I) * STEP, Fd.f_in, N);
@@ -169,7 +162,7 @@ template <class LF, class LG, class LS, class C, class Fields> struct SrcPairSme
         }
         return d2(p[0], p[1]);
     }
-    __device__ __forceinline__ d2 phi_old() const { const double2 v = *phiold; return d2(v.x, v.y); }
+    __device__ __forceinline__ d2 phi_old() const { return d2(po.x, po.y); }
     __device__ __forceinline__ f2 pdot_old() const { const float2 v = col[C::OFF_PDOT * C::NT]; return f2(v.x, v.y); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ f2 f() const { const float2 v = col[(C::OFF_F + I) * C::NT]; return f2(v.x, v.y); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ f2 s() const { const float2 v = col[(C::OFF_S + I) * C::NT]; return f2(v.x, v.y); }
@@ -183,9 +176,8 @@ k_main_pair_smem(const DevParams<float> P, const DevParams<f2> P2, const Fields 
     using TC = typename C::TC;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *tile = reinterpret_cast<double *>(smem_raw);
-    double2 *phiold = reinterpret_cast<double2 *>(smem_raw + C::TILE_BYTES);
-    float2 *pops = reinterpret_cast<float2 *>(smem_raw + C::TILE_BYTES + C::PHIOLD_BYTES);
-    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + C::TILE_BYTES + C::PHIOLD_BYTES + C::POPS_BYTES);
+    float2 *pops = reinterpret_cast<float2 *>(smem_raw + C::TILE_BYTES);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + C::TILE_BYTES + C::POPS_BYTES);
     constexpr int HX = BX / 2;
     const int t = threadIdx.x;
     const int tx = 2 * (t % HX), ty = (t / HX) % BY, tz = t / (HX * BY);
@@ -202,10 +194,13 @@ k_main_pair_smem(const DevParams<float> P, const DevParams<f2> P2, const Fields 
     const bool active = node_active<3>(P, x, y, z);   // nx is even: the second node of an active pair is active
     const bool bc = tile_touches_bc(P, x0, y0, z0, BX, BY, BZ);
     NodeGeom2 g;
+    double2 po = make_double2(0.0, 0.0);
     if (active && !bc) {
         g = make_geom2(P, x, y, z);
-        const SrcPairSmem<LF, LG, LS, C, Fields> src(P, Fd, g, tile, phiold, pops, bar_a, t, x, y, z, tx, ty, tz);
+        const SrcPairSmem<LF, LG, LS, C, Fields> src(P, Fd, g, tile, pops, bar_a, t, tx, ty, tz, po);
         src.prefetch();   // before the barrier below: the copies fly while the CTA assembles
+        po = __ldg(reinterpret_cast<const double2 *>(
+            Fd.phi_old + (((unsigned)(z + P.pz) * (unsigned)P.ppy + (unsigned)(y + 1)) * (unsigned)P.ppx + (unsigned)(x + P.xpad))));
     }
     if (t == 0) {
         pdl_wait();   // phi^{n+1} is K_phi's output, the only input the preceding launch writes
@@ -222,7 +217,7 @@ k_main_pair_smem(const DevParams<float> P, const DevParams<f2> P2, const Fields 
             node_update<LF, LG, LS, float, MODE>(P, Fd, g1, src);
         }
     } else {
-        const SrcPairSmem<LF, LG, LS, C, Fields> src(P, Fd, g, tile, phiold, pops, bar_a, t, x, y, z, tx, ty, tz);
+        const SrcPairSmem<LF, LG, LS, C, Fields> src(P, Fd, g, tile, pops, bar_a, t, tx, ty, tz, po);
         node_update<LF, LG, LS, f2, MODE>(P2, Fd, g, src);
     }
 }
