@@ -20,7 +20,7 @@ from test_oracle_bruteforce import _random_state  # noqa: E402
 
 
 def cases():
-    P = wl.base_params(136, 6, 5, grav=[1e-4, 0.0, -2e-4])                    # 3D wide tiles, ragged x
+    P = wl.base_params(250, 6, 5, grav=[1e-4, 0.0, -2e-4])                    # 3D wide tiles (128 + 122), ragged x
     yield "3d wide periodic", P, 11
     P = wl.base_params(64, 5, 6, grav=[0.0, 0.0, -1e-4])                      # 3D 64 x 2 tiles, z walls
     P["bc_f"][2] = ["wall", "wall"]; P["bc_g"][2] = ["zeroflux", "zeroflux"]; P["bc_s"][2] = ["dirichlet", "dirichlet"]
@@ -44,7 +44,8 @@ def main():
     for name, P, seed in cases():
         init = _random_state(P, seed)
         for prec in (64, 32):
-            for kernels in ((), ("pops_gather",), ("pops_staged",), ("phi_ldg",), ("no_graph", "no_pdl")):
+            for kernels in ((), ("pops_gather",), ("pops_staged",), ("phi_ldg",), ("no_graph", "no_pdl"), ("one_node",),
+                            ("one_node", "pops_staged")):
                 Q = dict(P); Q["kernels"] = kernels
                 sim = binding.LBM(Q, prec)
                 sim.init(*[a.astype(sim.dtype) for a in init])

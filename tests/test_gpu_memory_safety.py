@@ -51,7 +51,8 @@ def test_guard_bands_poison_and_determinism(gpu, oracle_mod, prec):
         if prec == 64:
             o = oracle_mod.Oracle(P); o.init(*init); o.step(7)
             ref = o.read_macro(); o.close()
-        for kernels in ((), ("pops_gather",), ("pops_staged",), ("phi_ldg",), ("no_graph", "no_pdl")):
+        for kernels in ((), ("pops_gather",), ("pops_staged",), ("phi_ldg",), ("no_graph", "no_pdl"), ("one_node",),
+                        ("one_node", "pops_staged")):   # fp32 3D: the first three run pairs of nodes, the last two one node per thread
             Q = dict(P); Q["kernels"] = kernels
             runs = []
             for rep in range(2):
