@@ -236,6 +236,11 @@ int lbm_read_pops_noalloc(lbm_ctx *c, int which, int stage, void *h_pops);
 /* Block until everything enqueued on the context's stream has finished; returns LBM_E_CUDA on a fault. */
 int lbm_sync(lbm_ctx *c);
 
+/* Number of values of the current state (post-collision populations, production field, phi) that are not finite -> *n_bad.
+ * The explicit scheme can leave its stable range (low mobility) and lbm_step never looks; this call does, off the
+ * hot path (one pass over the state, no allocation: it uses the context's scratch field; synchronises). */
+int lbm_check_finite(lbm_ctx *c, long long *n_bad);
+
 /* Per-kernel device timing for measurement (off by default).  While enabled, lbm_step brackets K_phi and K_main of
  * every step (at most 4096 steps between two lbm_kernel_times calls) with CUDA events on the context's stream.
  * lbm_kernel_times synchronises, returns the summed durations in milliseconds and the number of timed steps,

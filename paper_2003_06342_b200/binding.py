@@ -33,7 +33,7 @@ HALO_PHI, HALO_POPS = 0, 1
 NOALLOC_SCRATCH_BYTES = 8 << 20
 
 EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
-           "lbm_sync", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
+           "lbm_sync", "lbm_check_finite", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
 
@@ -88,6 +88,7 @@ def load_library():
         L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_read_pops_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_sync.argtypes = [C.c_void_p]
+        L.lbm_check_finite.argtypes = [C.c_void_p, C.POINTER(C.c_longlong)]
         L.lbm_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.lbm_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.lbm_step_count.restype = C.c_longlong
@@ -278,6 +279,12 @@ class LBM:
         out = np.empty((self.Q[which],) + self.shape, self.dtype)
         _check(self._L.lbm_read_pops_noalloc(self._h, int(which), int(stage), C.c_void_p(out.ctypes.data)), "lbm_read_pops_noalloc")
         return out
+
+    def check_finite(self) -> int:
+        """lbm_check_finite: number of non-finite values in the current state (0 = the run is still in its stable range)."""
+        n = C.c_longlong(-1)
+        _check(self._L.lbm_check_finite(self._h, C.byref(n)), "lbm_check_finite")
+        return int(n.value)
 
     def sync(self):
         _check(self._L.lbm_sync(self._h), "lbm_sync")

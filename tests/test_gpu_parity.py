@@ -594,6 +594,24 @@ def test_api_states_and_degenerate_calls(gpu, oracle_mod):
     sim.destroy(); sim.destroy(); o.close()                  # destroy is idempotent
 
 
+def test_check_finite(gpu):
+    """lbm_check_finite counts the non-finite values of the current state (populations, production field, phi): 0 on a healthy
+    run in both precisions and dimensions; every population of a node whose initial T is NaN, and what spreads from it, otherwise."""
+    for dims, prec in (((40, 10, 7), 64), ((136, 6, 5), 32), ((40, 20, 1), 64), ((40, 20, 1), 32)):
+        P = wl.base_params(*dims, grav=[1e-4, 0.0, 0.0])
+        init = [a.astype(np.float64 if prec == 64 else np.float32) for a in _random_state(P, 93)]
+        sim = gpu.LBM(P, prec); sim.init(*init); sim.step(5)
+        assert sim.check_finite() == 0
+        init[1][0, 3, 5] = np.nan
+        sim.init(*init)
+        n0 = sim.check_finite()
+        q_s = 7 if dims[2] > 1 else 5
+        assert n0 >= q_s + 1                 # the s populations of that node and its production rate, at least
+        sim.step(3)
+        assert sim.check_finite() > n0       # ... and it spreads
+        sim.destroy()
+
+
 def test_device_resident_fields(gpu, oracle_mod):
     """lbm_init / lbm_set_velocity / lbm_read_macro take DEVICE pointers as well (unified addressing)."""
     import torch
