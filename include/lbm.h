@@ -70,8 +70,9 @@ enum { LBM_DIV_PRODUCT = 0, LBM_DIV_STENCIL = 1 };
                                  /* f is still stepped (its p is reported) but its first moment is ignored             */
 /* Kernel selection.  The defaults are chosen by measurement per precision and grid; these flags force
  * the plainer kernels (all are parity-tested; results agree to rounding).  They change speed, never the method. */
-#define LBM_FLAG_POPS_GATHER 16u  /* K_main gathers the populations into registers (default of fp32 3D)                    */
-#define LBM_FLAG_POPS_STAGED 32u  /* K_main stages the populations in shared memory with cp.async (default elsewhere)      */
+#define LBM_FLAG_POPS_GATHER 16u  /* K_main gathers the populations into registers                                         */
+#define LBM_FLAG_POPS_STAGED 32u  /* K_main stages the populations in shared memory with cp.async (the default, except for    */
+                                  /* fp32 3D grids that cannot pair: odd or narrow rows, LBM_FLAG_ONE_NODE)                */
 #define LBM_FLAG_PHI_LDG 64u      /* K_main reads the phi stencil through L1 instead of a TMA box                         */
 #define LBM_FLAG_NO_PDL 256u      /* K_main not launched with programmatic dependent launch behind K_phi                  */
 #define LBM_FLAG_ONE_NODE 512u    /* fp32 3D: K_main with one node per thread instead of a pair of x-adjacent nodes           */
@@ -252,7 +253,9 @@ int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *ste
 long long lbm_step_count(const lbm_ctx *c);
 long long lbm_launch_count(const lbm_ctx *c);
 
-/* Name of the kernel variant the context steps with, for logs: "gather+smem", "gather+phi-tma" or "direct". */
+/* Name of the kernel variant the context steps with, for logs: "gather+smem", "gather+phi-tma", "direct" (one node per thread:
+ * populations staged in shared memory / gathered into registers with the phi tile by TMA / everything through L1), "pair+smem",
+ * "pair+phi-tma" (fp32 3D: two nodes per thread, staged / gathered), "direct (model variant)" (grad_scheme / div_scheme). */
 const char *lbm_variant(const lbm_ctx *c);
 
 /* Last CUDA runtime error code seen by this library (cudaError_t as int), 0 if none. */
