@@ -322,10 +322,12 @@ k_phi_pair(const DevParams<float> P, const float *__restrict__ g_in, double *__r
 #pragma unroll
         for (int i = 1; i < LG::Q; ++i) two_sum2(hi, lo, gi[j][i]);
         const double v0 = (double)hi.x + (double)lo.x, v1 = (double)hi.y + (double)lo.y;
-        const bool edge = x == 0 || x + 2 == P.nx || y == 0 || y == P.ny - 1 || z == 0 || z == P.nz - 1;
-        if (!edge) {
+        const bool edge = y == 0 || y == P.ny - 1 || z == 0 || z == P.nz - 1;
+        if (!edge) {   // at most the periodic images in x (store_phi_periodic_tile, k_phi.cuh)
             const long long pc = ((long long)(z + P.pz) * P.ppy + (y + 1)) * P.ppx + (x + P.xpad);
             *reinterpret_cast<double2 *>(phi_new + pc) = make_double2(v0, v1);   // x and xpad are even: 16-byte aligned
+            if (x == 0) phi_new[pc + P.nx] = v0;
+            if (x + 2 == P.nx) phi_new[pc + 1 - P.nx] = v1;
         } else {
             store_phi_with_images(phi_new, P, make_geom(P, x, y, z), v0);
             store_phi_with_images(phi_new, P, make_geom(P, x + 1, y, z), v1);

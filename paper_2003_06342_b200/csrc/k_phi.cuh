@@ -54,6 +54,19 @@ __device__ __forceinline__ void store_phi_with_images(preal *__restrict__ phi_pa
             }
 }
 
+// Store phi of a node of a tile that touches NO non-periodic face.  Such a node can only have periodic images; the common one --
+// the node sits on the first or last column of a periodic row and nowhere else on the edge of the grid -- is ONE extra store, one
+// period away in x.  (Every row has two such nodes, so a quarter of the warps of a 256-wide grid would otherwise walk through
+// the general image tables of store_phi_with_images for the sake of one lane.)  Rows and planes on the edge take the general path.
+template <class real, class preal>
+__device__ __forceinline__ void store_phi_periodic_tile(preal *__restrict__ phi_pad, const DevParams<real> &P, const NodeGeom &g, preal v) {
+    if (g.lo[1] | g.hi[1] | (P.pz && (g.lo[2] | g.hi[2]))) { store_phi_with_images(phi_pad, P, g, v); return; }
+    const long long pc = ((long long)(g.z + P.pz) * P.ppy + (g.y + 1)) * P.ppx + (g.x + P.xpad);
+    phi_pad[pc] = v;
+    if (g.lo[0]) phi_pad[pc + P.nx] = v;
+    if (g.hi[0]) phi_pad[pc - P.nx] = v;
+}
+
 // Each thread handles NPT nodes, NPT tiles apart along the slowest tiled axis (z in 3D, y in 2D); all 8 NPT loads are
 // issued before the first sum, which is what a latency-bound streaming kernel needs (measured: DESIGN.md "Kernels").
 // phi^{n+1} = sum_i g_i + dt/2 Pdot (Eq.32); the last term is already inside the stored rest population (k_main.cuh), so
@@ -115,7 +128,9 @@ k_phi(const DevParams<real> P, const sreal *__restrict__ g_in, preal *__restrict
     }
 #pragma unroll
     for (int j = 0; j < NPT; ++j) {
-        if (ok[j]) store_phi_with_images(phi_new, P, g[j], phi_sum<preal>(gi[j]));
+        if (!ok[j]) continue;
+        if (bc) store_phi_with_images(phi_new, P, g[j], phi_sum<preal>(gi[j]));
+        else store_phi_periodic_tile(phi_new, P, g[j], phi_sum<preal>(gi[j]));
     }
 }
 
