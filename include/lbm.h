@@ -237,6 +237,14 @@ int lbm_read_pops_noalloc(lbm_ctx *c, int which, int stage, void *h_pops);
 /* Block until everything enqueued on the context's stream has finished; returns LBM_E_CUDA on a fault. */
 int lbm_sync(lbm_ctx *c);
 
+/* Checkpoint / resume.  lbm_save_state copies the whole state of the context (a 64-byte header and the workspace image:
+ * lbm_state_bytes bytes) to the HOST buffer h_state; lbm_load_state puts such an image back into a context created for the same
+ * grid, lattice set and precision (else LBM_E_INVALID; the physical parameters are the caller's business) -- also one that was never
+ * initialised.  The restored context continues bit for bit.  Between steps only (LBM_E_STATE inside a phased step); both synchronise. */
+size_t lbm_state_bytes(const lbm_ctx *c);
+int lbm_save_state(lbm_ctx *c, void *h_state);
+int lbm_load_state(lbm_ctx *c, const void *h_state);
+
 /* Number of values of the current state (post-collision populations, production field, phi) that are not finite -> *n_bad.
  * The explicit scheme can leave its stable range (low mobility) and lbm_step never looks; this call does, off the
  * hot path (one pass over the state, no allocation: it uses the context's scratch field; synchronises). */

@@ -33,7 +33,7 @@ HALO_PHI, HALO_POPS = 0, 1
 NOALLOC_SCRATCH_BYTES = 8 << 20
 
 EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
-           "lbm_sync", "lbm_check_finite", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
+           "lbm_sync", "lbm_check_finite", "lbm_state_bytes", "lbm_save_state", "lbm_load_state", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
 
@@ -89,6 +89,10 @@ def load_library():
         L.lbm_read_pops_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_sync.argtypes = [C.c_void_p]
         L.lbm_check_finite.argtypes = [C.c_void_p, C.POINTER(C.c_longlong)]
+        L.lbm_state_bytes.restype = C.c_size_t
+        L.lbm_state_bytes.argtypes = [C.c_void_p]
+        L.lbm_save_state.argtypes = [C.c_void_p, C.c_void_p]
+        L.lbm_load_state.argtypes = [C.c_void_p, C.c_void_p]
         L.lbm_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.lbm_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.lbm_step_count.restype = C.c_longlong
@@ -279,6 +283,19 @@ class LBM:
         out = np.empty((self.Q[which],) + self.shape, self.dtype)
         _check(self._L.lbm_read_pops_noalloc(self._h, int(which), int(stage), C.c_void_p(out.ctypes.data)), "lbm_read_pops_noalloc")
         return out
+
+    def save_state(self) -> np.ndarray:
+        """lbm_save_state: the whole state as a byte array (header + workspace image) for lbm_load_state."""
+        buf = np.empty(int(self._L.lbm_state_bytes(self._h)), dtype=np.uint8)
+        _check(self._L.lbm_save_state(self._h, C.c_void_p(buf.ctypes.data)), "lbm_save_state")
+        return buf
+
+    def load_state(self, buf: np.ndarray):
+        """lbm_load_state: continue from an image saved by a context of the same grid, lattice set and precision."""
+        buf = np.ascontiguousarray(buf, dtype=np.uint8)
+        if buf.size != int(self._L.lbm_state_bytes(self._h)):
+            raise ValueError("state image of %d bytes, this context needs %d" % (buf.size, int(self._L.lbm_state_bytes(self._h))))
+        _check(self._L.lbm_load_state(self._h, C.c_void_p(buf.ctypes.data)), "lbm_load_state")
 
     def check_finite(self) -> int:
         """lbm_check_finite: number of non-finite values in the current state (0 = the run is still in its stable range)."""

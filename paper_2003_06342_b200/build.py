@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC_DIR = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblbm_b200.so")
-SOURCES = ["lbm.cu", "halo.cu", "noalloc.cu", "finite.cu", "inst_2d995_f64.cu", "inst_2d995_f32.cu", "inst_2d999_f64.cu", "inst_2d999_f32.cu",
+SOURCES = ["lbm.cu", "halo.cu", "noalloc.cu", "finite.cu", "state.cu", "inst_2d995_f64.cu", "inst_2d995_f32.cu", "inst_2d999_f64.cu", "inst_2d999_f32.cu",
            "inst_3d_f64.cu", "inst_3d_f32.cu", "inst_3d15_f64.cu", "inst_3d15_f32.cu"]
 
 

@@ -594,6 +594,34 @@ def test_api_states_and_degenerate_calls(gpu, oracle_mod):
     sim.destroy(); sim.destroy(); o.close()                  # destroy is idempotent
 
 
+def test_save_and_load_state(gpu):
+    """Checkpoint / resume: a context restored from lbm_save_state continues bit for bit -- also a fresh context that never saw
+    lbm_init, also from an odd step count (the other half of the double buffers is current), in both precisions; an image of another
+    grid or precision is refused."""
+    for dims, prec in (((40, 10, 7), 64), ((136, 6, 5), 32), ((40, 20, 1), 64)):
+        P = wl.base_params(*dims, grav=[1e-4, 0.0, 0.0])
+        dt = np.float64 if prec == 64 else np.float32
+        init = [a.astype(dt) for a in _random_state(P, 94)]
+        a = gpu.LBM(P, prec); a.init(*init); a.step(5)
+        image = a.save_state()
+        a.step(6)
+        want = a.read_macro() + tuple(a.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
+        b = gpu.LBM(P, prec)
+        b.load_state(image)
+        assert b.step_count == 5
+        b.step(6)
+        got = b.read_macro() + tuple(b.read_pops(w, gpu.STAGE_POSTCOLLISION) for w in range(3))
+        for x, y in zip(got, want):
+            assert np.array_equal(x, y)
+        a.load_state(image); a.step(6)      # and back into the context it came from
+        assert np.array_equal(a.read_macro()[3], want[3])
+        other = gpu.LBM(P, 96 - prec)
+        with pytest.raises((gpu.LBMError, ValueError)):
+            other.load_state(image)
+        for s in (a, b, other):
+            s.destroy()
+
+
 def test_check_finite(gpu):
     """lbm_check_finite counts the non-finite values of the current state (populations, production field, phi): 0 on a healthy
     run in both precisions and dimensions; every population of a node whose initial T is NaN, and what spreads from it, otherwise."""
