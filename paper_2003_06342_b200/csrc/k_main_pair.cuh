@@ -94,17 +94,19 @@ template <class LF, class LG, class LS, class TC, class Fields> struct SrcPair {
     template <int I, bool AGAIN = false> __device__ __forceinline__ f2 gg() const { return pull_pair<LG, I, AGAIN>(Fd.g_in, (unsigned)P.N, g); }
 };
 
-// ---- the same with the pair's f and s values, phi^n and Pdot staged in shared memory by per-thread cp.async (as k_main_smem.cuh):
+// ---- the same with the pair's f, s and g values and Pdot staged in shared memory by per-thread cp.async (as k_main_smem.cuh):
 // 16 warps per SM holding their loads in registers leave the memory system idle (measured: 63% of the DRAM peak, issue slots 30%
-// busy, 8 long-scoreboard stalls per issue); staged, all 47 copies of a pair are in flight at once.
+// busy, 8 long-scoreboard stalls per issue); staged, all 56 copies of a pair are in flight at once.  Unlike in double precision,
+// staging g pays here (K_main 1.549 -> 1.522 ms on config 4): read as plain loads at their collision, the last thing a thread
+// does, their latency is exposed with nothing left to overlap it.
 template <class LF, class LG, class LS, int BX, int BY, int BZ> struct PairSmemCfg {
     using TC = PhiTileCfg<double, 3, BX, BY, BZ>;
     static constexpr int NT = BX / 2 * BY * BZ;
-    static constexpr int QT = LF::Q + LS::Q;
-    static constexpr int OFF_F = 0, OFF_S = LF::Q, OFF_PDOT = QT;   // float2 slots
+    static constexpr int QT = LF::Q + LS::Q + LG::Q;
+    static constexpr int OFF_F = 0, OFF_S = LF::Q, OFF_G = LF::Q + LS::Q, OFF_PDOT = QT;   // float2 slots
     static constexpr size_t TILE_BYTES = ((size_t)TC::BYTES + 127) / 128 * 128;
-    // phi^n is NOT staged (it rides in registers from before the CTA barrier): with it four CTAs would need the 196 KB shared-memory
-    // configuration; without it they fit the 164 KB one and L1 keeps 92 KB for the sectors that x-shifted pulls share (k_main_smem.cuh)
+    // phi^n is NOT staged (it rides in registers from before the CTA barrier): four CTAs fit the 196 KB shared-memory configuration
+    // without it, not with it
     static constexpr size_t POPS_BYTES = (size_t)(QT + 1) * NT * sizeof(float2);
     static constexpr size_t BYTES = TILE_BYTES + POPS_BYTES + 16;   // + the mbarrier
 };
@@ -149,7 +151,11 @@ template <class LF, class LG, class LS, class C, class Fields> struct SrcPairSme
             constexpr int I = decltype(ic)::value;
             copy_pair<LF, I>(c0 + (uint32_t)(C::OFF_F + I) * STEP, Fd.f_in, N);
         });
-        cp_async_commit();   // group 2: f, first needed by the moments
+        static_for<LG::Q>([&](auto ic) {
+            constexpr int I = decltype(ic)::value;
+            copy_pair<LG, I>(c0 + (uint32_t)(C::OFF_G + I) * STEP, Fd.g_in, N);
+        });
+        cp_async_commit();   // group 2: f and g, first needed by the moments
     }
     __device__ __forceinline__ void pops_ready() const { cp_async_wait_1(); }
     __device__ __forceinline__ void f_ready() const { cp_async_wait_all(); }
@@ -166,7 +172,7 @@ template <class LF, class LG, class LS, class C, class Fields> struct SrcPairSme
     __device__ __forceinline__ f2 pdot_old() const { const float2 v = col[C::OFF_PDOT * C::NT]; return f2(v.x, v.y); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ f2 f() const { const float2 v = col[(C::OFF_F + I) * C::NT]; return f2(v.x, v.y); }
     template <int I, bool AGAIN = false> __device__ __forceinline__ f2 s() const { const float2 v = col[(C::OFF_S + I) * C::NT]; return f2(v.x, v.y); }
-    template <int I, bool AGAIN = false> __device__ __forceinline__ f2 gg() const { return pull_pair<LG, I, AGAIN>(Fd.g_in, (unsigned)P.N, g); }
+    template <int I, bool AGAIN = false> __device__ __forceinline__ f2 gg() const { const float2 v = col[(C::OFF_G + I) * C::NT]; return f2(v.x, v.y); }
 };
 
 template <class LF, class LG, class LS, int MODE, int BX, int BY, int BZ, int MINB, class Fields>
