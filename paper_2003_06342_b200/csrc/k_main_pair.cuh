@@ -96,7 +96,7 @@ template <class LF, class LG, class LS, class TC, class Fields> struct SrcPair {
 
 // ---- the same with the pair's f, s and g values and Pdot staged in shared memory by per-thread cp.async (as k_main_smem.cuh):
 // 16 warps per SM holding their loads in registers leave the memory system idle (measured: 63% of the DRAM peak, issue slots 30%
-// busy, 8 long-scoreboard stalls per issue); staged, all 56 copies of a pair are in flight at once.  Unlike in double precision,
+// busy, 8 long-scoreboard stalls per issue); staged, all 48 copies of a pair are in flight at once.  Unlike in double precision,
 // staging g pays here (K_main 1.549 -> 1.522 ms on config 4): read as plain loads at their collision, the last thing a thread
 // does, their latency is exposed with nothing left to overlap it.
 template <class LF, class LG, class LS, int BX, int BY, int BZ> struct PairSmemCfg {
