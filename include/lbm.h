@@ -258,6 +258,10 @@ int lbm_set_timing(lbm_ctx *c, int enable);
 int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *steps);
 
 /* Counters: steps taken since init; kernels launched by this context since creation. */
+/* For callers that capture lbm_step_layers / lbm_halo_* calls in a CUDA graph of their own (slabs.py does for small slabs): the
+ * calls made during capture only record, and a replay runs them without the library seeing it -- add `steps` and `launches`
+ * (either may be negative) to the context's counters.  The buffer parity is the caller's to keep: capture an even number of steps. */
+int lbm_note_replay(lbm_ctx *c, long long steps, long long launches);
 long long lbm_step_count(const lbm_ctx *c);
 long long lbm_launch_count(const lbm_ctx *c);
 

@@ -33,7 +33,7 @@ HALO_PHI, HALO_POPS = 0, 1
 NOALLOC_SCRATCH_BYTES = 8 << 20
 
 EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
-           "lbm_sync", "lbm_check_finite", "lbm_state_bytes", "lbm_save_state", "lbm_load_state", "lbm_set_timing", "lbm_kernel_times", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
+           "lbm_sync", "lbm_check_finite", "lbm_state_bytes", "lbm_save_state", "lbm_load_state", "lbm_set_timing", "lbm_kernel_times", "lbm_note_replay", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
 
@@ -95,6 +95,7 @@ def load_library():
         L.lbm_load_state.argtypes = [C.c_void_p, C.c_void_p]
         L.lbm_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.lbm_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.lbm_note_replay.argtypes = [C.c_void_p, C.c_longlong, C.c_longlong]
         L.lbm_step_count.restype = C.c_longlong
         L.lbm_step_count.argtypes = [C.c_void_p]
         L.lbm_launch_count.restype = C.c_longlong
@@ -296,6 +297,10 @@ class LBM:
         if buf.size != int(self._L.lbm_state_bytes(self._h)):
             raise ValueError("state image of %d bytes, this context needs %d" % (buf.size, int(self._L.lbm_state_bytes(self._h))))
         _check(self._L.lbm_load_state(self._h, C.c_void_p(buf.ctypes.data)), "lbm_load_state")
+
+    def note_replay(self, steps: int, launches: int):
+        """lbm_note_replay: account for steps run (or only recorded) by a CUDA graph of the caller's."""
+        _check(self._L.lbm_note_replay(self._h, int(steps), int(launches)), "lbm_note_replay")
 
     def check_finite(self) -> int:
         """lbm_check_finite: number of non-finite values in the current state (0 = the run is still in its stable range)."""

@@ -376,6 +376,13 @@ int lbm_kernel_times(lbm_ctx *c, double *ms_phi, double *ms_main, long long *ste
     return LBM_OK;
 }
 
+int lbm_note_replay(lbm_ctx *c, long long steps, long long launches) {
+    if (!c) return LBM_E_INVALID;
+    if (c->nsteps + steps < 0 || c->launches + launches < 0) return LBM_E_INVALID;
+    c->nsteps += steps; c->launches += launches;
+    return LBM_OK;
+}
+
 long long lbm_step_count(const lbm_ctx *c) { return c ? c->nsteps : -1; }
 long long lbm_launch_count(const lbm_ctx *c) { return c ? c->launches : -1; }
 const char *lbm_variant(const lbm_ctx *c) {

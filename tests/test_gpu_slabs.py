@@ -170,3 +170,25 @@ def test_slab_api_states(gpu):
     Pm["halo"] = (0, 0)                                                # mixed kinds without the ghost layer
     with pytest.raises(gpu.LBMError):
         gpu.LBM(Pm, 64)
+
+
+def test_graph_replay_of_the_overlapped_step(gpu):
+    """Small slabs replay their overlapped step from a CUDA graph of two consecutive steps captured across the compute and the
+    exchange stream, one graph per buffer parity (slabs.SlabGroup, lbm_note_replay): same bits as the launches themselves, from
+    even and from odd step counts, and the contexts' step counters follow the replays."""
+    for P, seed in ((wl.base_params(136, 6, 12, grav=[1e-4, -2e-4, 5e-5]), 65), (wl.base_params(40, 36, 1, grav=[1e-4, -1e-4, 0.0]), 66)):
+        init = _random_state(P, seed)
+        a = slabs.SlabGroup(P, 3, 64, overlap=True, graph=True)
+        b = slabs.SlabGroup(P, 3, 64, overlap=True, graph=False)
+        for g in (a, b):
+            g.init(*init)
+        total = 0
+        for n in (1, 12, 11, 9):          # parities 1, 1, 0 at the start of the graph-eligible calls
+            a.step(n); b.step(n); total += n
+            assert len(a._graphs) >= (1 if total > 1 else 0) and not b._graphs
+            assert all(s.sim.step_count == total for s in a.slabs), [s.sim.step_count for s in a.slabs]
+            assert [s.sim.launch_count for s in a.slabs] == [s.sim.launch_count for s in b.slabs]
+            for x, y in zip(_state(a, gpu).values(), _state(b, gpu).values()):
+                assert np.array_equal(x, y), (n, total)
+        assert len(a._graphs) == 2
+        a.destroy(); b.destroy()
