@@ -210,6 +210,12 @@ int lbm_set_stream(lbm_ctx *c, void *cuda_stream);
 int lbm_halo_bytes(const lbm_ctx *c, int what, size_t *bytes);
 int lbm_halo_pack(lbm_ctx *c, int what, int side, void *d_buf);
 int lbm_halo_unpack(lbm_ctx *c, int what, int side, const void *d_buf);
+/* Pack and unpack in one launch where the neighbour's workspace can be addressed from this device (the same GPU, or a peer-mapped
+ * workspace over NVLink): the boundary layer next to the ghost side `side` of c goes straight into the ghost layer of the OPPOSITE
+ * side of `peer`, with no buffer in between.  Both contexts must stand at the same point of the same step (LBM_E_STATE otherwise)
+ * and describe slabs of one domain (same lattice set, precision, nx, ny).  Enqueued on c's stream; the caller orders it against the
+ * kernels of `peer` that read the ghost layer. */
+int lbm_halo_push(lbm_ctx *c, int what, int side, lbm_ctx *peer);
 
 /* Copy the macroscopic fields of the current time level to HOST arrays; any pointer may be NULL.
  * h_u is [3][z][y][x].  Synchronises. */

@@ -32,7 +32,7 @@ STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1
 NOALLOC_SCRATCH_BYTES = 8 << 20
 
-EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_halo_push", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
            "lbm_sync", "lbm_check_finite", "lbm_state_bytes", "lbm_save_state", "lbm_load_state", "lbm_set_timing", "lbm_kernel_times", "lbm_note_replay", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
@@ -84,6 +84,7 @@ def load_library():
         L.lbm_halo_bytes.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_size_t)]
         L.lbm_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.lbm_halo_push.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_read_macro.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_read_pops_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
@@ -256,6 +257,10 @@ class LBM:
 
     def halo_unpack(self, what: int, side: int, buf):
         _check(self._L.lbm_halo_unpack(self._h, int(what), int(side), self._dev_buf(what, buf)), "lbm_halo_unpack")
+
+    def halo_push(self, what: int, side: int, peer: "LBM"):
+        """lbm_halo_push: this slab's boundary layer of ``side`` straight into the opposite ghost layer of ``peer`` (one launch)."""
+        _check(self._L.lbm_halo_push(self._h, int(what), int(side), peer._h), "lbm_halo_push")
 
     def set_velocity(self, u):
         ptr, keep = _host_ptr(u, self.dtype, (3,) + self.shape, "u")

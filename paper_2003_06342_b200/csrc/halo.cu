@@ -27,6 +27,17 @@ __global__ void __launch_bounds__(256) k_halo_copy(const HaloPlan plan, T *__res
     }
 }
 
+// region r of `src` into region r of `dst` (same number and size of regions): a boundary layer straight into a ghost layer
+template <class T>
+__global__ void __launch_bounds__(256) k_halo_push(const HaloPlan src, const HaloPlan dst) {
+    const int r = blockIdx.y;
+    const T *a = reinterpret_cast<const T *>(src.ptr[r]);
+    T *b = reinterpret_cast<T *>(dst.ptr[r]);
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < src.elems;
+         i += (unsigned long long)gridDim.x * blockDim.x)
+        b[i] = a[i];
+}
+
 namespace {
 
 template <class L> void add_pops(HaloPlan &pl, const lbm_ctx *c, size_t off, int axis, int dir, long long layer, size_t es) {
@@ -122,6 +133,28 @@ int lbm_halo_bytes(const lbm_ctx *c, int what, size_t *bytes) {
     const int side = c->P.halo[0] ? 0 : 1;   // the size depends neither on the side nor on the phase
     if (!lbm::make_plan(c, what, side, false, pl)) return LBM_E_INVALID;
     *bytes = (size_t)pl.count * (size_t)pl.elems * (size_t)(what == LBM_HALO_PHI ? c->L.es_phi : c->L.es);
+    return LBM_OK;
+}
+
+int lbm_halo_push(lbm_ctx *c, int what, int side, lbm_ctx *peer) {
+    using namespace lbm;
+    if (!c || !peer || (what != LBM_HALO_PHI && what != LBM_HALO_POPS) || (side != 0 && side != 1)) return LBM_E_INVALID;
+    if (!c->P.halo[side] || !peer->P.halo[1 - side]) return LBM_E_INVALID;
+    if (!c->inited || !peer->inited) return LBM_E_STATE;
+    // both contexts at the same point of the same step (see halo_copy for when phi and when the populations travel)
+    if (c->phase != peer->phase || c->partial != peer->partial || c->cur != peer->cur || c->curphi != peer->curphi) return LBM_E_STATE;
+    const bool phi_time = (c->phase == 1 && !c->partial) || (c->phase == 0 && c->partial);
+    if ((what == LBM_HALO_PHI) != phi_time) return LBM_E_STATE;
+    if (c->set != peer->set || c->L.es != peer->L.es) return LBM_E_INVALID;
+    HaloPlan src, dst;
+    if (!make_plan(c, what, side, /*ghost=*/false, src) || !make_plan(peer, what, 1 - side, /*ghost=*/true, dst)) return LBM_E_INVALID;
+    if (src.count != dst.count || src.elems != dst.elems) return LBM_E_INVALID;   // the two slabs differ in the slab axis only
+    const unsigned gx = (unsigned)((src.elems + 1023) / 1024 > 0 ? (src.elems + 1023) / 1024 : 1);
+    const dim3 grid(gx > 1184u ? 1184u : gx, (unsigned)src.count);
+    if ((what == LBM_HALO_PHI ? c->L.es_phi : c->L.es) == 8) k_halo_push<double><<<grid, 256, 0, c->stream>>>(src, dst);
+    else k_halo_push<float><<<grid, 256, 0, c->stream>>>(src, dst);
+    c->launches++;
+    CK(cudaGetLastError());
     return LBM_OK;
 }
 

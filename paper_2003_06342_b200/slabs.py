@@ -123,6 +123,17 @@ def exchange_local(slabs, what: int, periodic: bool):
                 sl.halo_unpack(what, side, slabs[nb[side]].buffers(what)[1 - side])
 
 
+def exchange_push(slabs, what: int, periodic: bool):
+    """All slabs in one process on one GPU (or with peer-mapped workspaces): every cut side is ONE launch that copies the
+    boundary layer straight into the neighbour's ghost layer (lbm_halo_push) -- no buffers, no unpack."""
+    world = len(slabs)
+    for r, sl in enumerate(slabs):
+        nb = neighbours(r, world, periodic)
+        for side in range(2):
+            if sl.halo[side]:
+                sl.halo_push(what, side, slabs[nb[side]])
+
+
 def exchange_dist(slab, what: int, rank: int, world: int, periodic: bool, group=None):
     """One slab per rank: pack, post all sends and receives as one batch, wait, unpack.
 
@@ -280,6 +291,9 @@ class Slab:
     def halo_unpack(self, what, side, buf):
         self.sim.halo_unpack(what, side, buf)
 
+    def halo_push(self, what, side, peer):
+        self.sim.halo_push(what, side, peer.sim)
+
     def set_stream(self, stream):
         self.sim.set_stream(stream)
 
@@ -321,9 +335,12 @@ class Slab:
 class SlabGroup:
     """``nslabs`` slabs of one domain in one process, on the current device and stream."""
 
-    def __init__(self, P: dict, nslabs: int, precision: int = 64, overlap: bool = True, graph: bool = True):
+    def __init__(self, P: dict, nslabs: int, precision: int = 64, overlap: bool = True, graph: bool = True, push: bool = True):
         import torch
         self.P = P
+        # the slabs share a GPU: a boundary layer goes straight into the neighbour's ghost layer (one launch per cut side and
+        # phase) instead of pack -> buffer -> unpack (two); push=False keeps the buffered exchange a multi-process run uses
+        self._exchange = exchange_push if push else exchange_local
         # the overlapped step of small slabs is launch-bound (fourteen short launches per slab and step): replay it from a CUDA
         # graph of two consecutive steps (the buffers alternate with period 2), captured across both streams, one per parity
         self.graph = graph
@@ -339,14 +356,14 @@ class SlabGroup:
         for s in self.slabs:
             s.init(phi, T, u, p)
         if self.any_halo:
-            exchange_local(self.slabs, HALO_POPS, self.periodic)   # ghost populations of level 0
+            self._exchange(self.slabs, HALO_POPS, self.periodic)   # ghost populations of level 0
 
     def step(self, n: int = 1):
         if not self.any_halo:
             self.slabs[0].sim.step(n)
             return
         if self.overlap:
-            exch = lambda what: exchange_local(self.slabs, what, self.periodic)   # noqa: E731
+            exch = lambda what: self._exchange(self.slabs, what, self.periodic)   # noqa: E731
             plain = n - 1
             small = max(s.sim.N for s in self.slabs) <= (1 << 21)
             if self.graph and small and plain >= 6:
@@ -361,10 +378,10 @@ class SlabGroup:
         for k in range(n):
             for s in self.slabs:
                 s.sim.step_phase(0)
-            exchange_local(self.slabs, HALO_PHI, self.periodic)
+            self._exchange(self.slabs, HALO_PHI, self.periodic)
             for s in self.slabs:
                 s.sim.step_phase(1, store_macros=(k == n - 1))
-            exchange_local(self.slabs, HALO_POPS, self.periodic)
+            self._exchange(self.slabs, HALO_POPS, self.periodic)
 
     def _replay(self, pairs: int, exch) -> int:
         """``pairs`` times two plain steps from the CUDA graph of the current buffer parity; returns the steps done."""

@@ -39,8 +39,10 @@ def _state(group_or_sim, gpu):
 def _check(gpu, oracle_mod, P, init, nslabs_list, horizons, precision=64, oracle=True, exact=True):
     single = gpu.LBM(P, precision)
     single.init(*init)
-    nslabs_list = [n for n in nslabs_list for _ in range(2)]
-    groups = [slabs.SlabGroup(P, n, precision, overlap=(i % 2 == 0)) for i, n in enumerate(nslabs_list)]
+    # per slab count: overlapped schedule with the ghost layers pushed straight into the neighbour (lbm_halo_push), the plain
+    # schedule with pushes, and the overlapped schedule with the buffered pack / unpack exchange a multi-process run uses
+    nslabs_list = [n for n in nslabs_list for _ in range(3)]
+    groups = [slabs.SlabGroup(P, n, precision, overlap=(i % 3 != 1), push=(i % 3 != 2)) for i, n in enumerate(nslabs_list)]
     for g in groups:
         g.init(*init)
     o = None
