@@ -216,6 +216,11 @@ int lbm_halo_unpack(lbm_ctx *c, int what, int side, const void *d_buf);
  * and describe slabs of one domain (same lattice set, precision, nx, ny).  Enqueued on c's stream; the caller orders it against the
  * kernels of `peer` that read the ghost layer. */
 int lbm_halo_push(lbm_ctx *c, int what, int side, lbm_ctx *peer);
+/* The same for a neighbour that lives in ANOTHER process or on another GPU: *peer_params are the parameters its context was created
+ * with and d_peer_workspace is its workspace as mapped into this process (CUDA IPC / peer access: a device pointer valid on the
+ * current device).  The neighbour is taken to stand where c stands -- the slabs of a domain step in lockstep; ordering across the
+ * processes (inter-process events) is the caller's. */
+int lbm_halo_push_mapped(lbm_ctx *c, int what, int side, const lbm_params *peer_params, void *d_peer_workspace);
 
 /* Copy the macroscopic fields of the current time level to HOST arrays; any pointer may be NULL.
  * h_u is [3][z][y][x].  Synchronises. */

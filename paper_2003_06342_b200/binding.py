@@ -32,7 +32,7 @@ STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1
 NOALLOC_SCRATCH_BYTES = 8 << 20
 
-EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_halo_push", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_halo_push", "lbm_halo_push_mapped", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
            "lbm_sync", "lbm_check_finite", "lbm_state_bytes", "lbm_save_state", "lbm_load_state", "lbm_set_timing", "lbm_kernel_times", "lbm_note_replay", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
@@ -85,6 +85,7 @@ def load_library():
         L.lbm_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_halo_push.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.lbm_halo_push_mapped.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(lbm_params), C.c_void_p]
         L.lbm_read_macro.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_read_pops_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
@@ -262,6 +263,12 @@ class LBM:
         """lbm_halo_push: this slab's boundary layer of ``side`` straight into the opposite ghost layer of ``peer`` (one launch)."""
         _check(self._L.lbm_halo_push(self._h, int(what), int(side), peer._h), "lbm_halo_push")
 
+    def halo_push_mapped(self, what: int, side: int, peer_params: dict, peer_workspace_ptr: int):
+        """lbm_halo_push_mapped: as halo_push, for a neighbour known by its parameters and its (peer-mapped) workspace pointer."""
+        s = make_params(peer_params, self.precision)
+        _check(self._L.lbm_halo_push_mapped(self._h, int(what), int(side), C.byref(s), C.c_void_p(int(peer_workspace_ptr))),
+               "lbm_halo_push_mapped")
+
     def set_velocity(self, u):
         ptr, keep = _host_ptr(u, self.dtype, (3,) + self.shape, "u")
         _check(self._L.lbm_set_velocity(self._h, C.c_void_p(ptr)), "lbm_set_velocity")
@@ -315,6 +322,11 @@ class LBM:
 
     def sync(self):
         _check(self._L.lbm_sync(self._h), "lbm_sync")
+
+    @property
+    def workspace_ptr(self) -> int:
+        """Device address of the workspace lent to the library (what a neighbour maps for lbm_halo_push_mapped)."""
+        return int(self._ws.data_ptr())
 
     @property
     def stream(self):

@@ -44,6 +44,9 @@ struct ImplOps {
     int bx, by, bz;   // tile of nodes per CTA
 };
 
+// lbm.cu: validation, lattice set and workspace layout of a parameter block (also of a PEER's, lbm_halo_push_mapped)
+int describe_params(const lbm_params *p, LatSet *set, Layout *L);
+
 // defined in inst_*.cu (compiled in parallel); nx selects the tile shape
 const ImplOps *ops_2d995_f64(int nx);
 const ImplOps *ops_3d15_f64(int nx);

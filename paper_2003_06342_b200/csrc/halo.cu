@@ -136,16 +136,43 @@ int lbm_halo_bytes(const lbm_ctx *c, int what, size_t *bytes) {
     return LBM_OK;
 }
 
+namespace lbm {
+namespace {
+// boundary layer of `side` of c -> ghost layer of the opposite side of `peer` (a context, or a description of a mapped workspace)
+int halo_push(lbm_ctx *c, int what, int side, const lbm_ctx *peer);
+}  // namespace
+}  // namespace lbm
+
 int lbm_halo_push(lbm_ctx *c, int what, int side, lbm_ctx *peer) {
-    using namespace lbm;
-    if (!c || !peer || (what != LBM_HALO_PHI && what != LBM_HALO_POPS) || (side != 0 && side != 1)) return LBM_E_INVALID;
-    if (!c->P.halo[side] || !peer->P.halo[1 - side]) return LBM_E_INVALID;
-    if (!c->inited || !peer->inited) return LBM_E_STATE;
+    if (!c || !peer) return LBM_E_INVALID;
+    if (!peer->inited) return LBM_E_STATE;
     // both contexts at the same point of the same step (see halo_copy for when phi and when the populations travel)
     if (c->phase != peer->phase || c->partial != peer->partial || c->cur != peer->cur || c->curphi != peer->curphi) return LBM_E_STATE;
+    return lbm::halo_push(c, what, side, peer);
+}
+
+int lbm_halo_push_mapped(lbm_ctx *c, int what, int side, const lbm_params *peer_params, void *d_peer_workspace) {
+    using namespace lbm;
+    if (!c || !peer_params || !d_peer_workspace) return LBM_E_INVALID;
+    // a description of the neighbour's context, standing where this one stands: the two step in lockstep
+    lbm_ctx peer{};
+    const int rc = describe_params(peer_params, &peer.set, &peer.L);
+    if (rc) return rc;
+    peer.P = *peer_params;
+    peer.ws = static_cast<char *>(d_peer_workspace);
+    peer.inited = true; peer.phase = c->phase; peer.partial = c->partial; peer.cur = c->cur; peer.curphi = c->curphi;
+    return halo_push(c, what, side, &peer);
+}
+
+namespace lbm {
+namespace {
+int halo_push(lbm_ctx *c, int what, int side, const lbm_ctx *peer) {
+    if ((what != LBM_HALO_PHI && what != LBM_HALO_POPS) || (side != 0 && side != 1)) return LBM_E_INVALID;
+    if (!c->P.halo[side] || !peer->P.halo[1 - side]) return LBM_E_INVALID;
+    if (!c->inited) return LBM_E_STATE;
     const bool phi_time = (c->phase == 1 && !c->partial) || (c->phase == 0 && c->partial);
     if ((what == LBM_HALO_PHI) != phi_time) return LBM_E_STATE;
-    if (c->set != peer->set || c->L.es != peer->L.es) return LBM_E_INVALID;
+    if (c->set != peer->set || c->L.es != peer->L.es || c->P.nx != peer->P.nx || (c->P.nz > 1 && c->P.ny != peer->P.ny)) return LBM_E_INVALID;
     HaloPlan src, dst;
     if (!make_plan(c, what, side, /*ghost=*/false, src) || !make_plan(peer, what, 1 - side, /*ghost=*/true, dst)) return LBM_E_INVALID;
     if (src.count != dst.count || src.elems != dst.elems) return LBM_E_INVALID;   // the two slabs differ in the slab axis only
@@ -157,6 +184,8 @@ int lbm_halo_push(lbm_ctx *c, int what, int side, lbm_ctx *peer) {
     CK(cudaGetLastError());
     return LBM_OK;
 }
+}  // namespace
+}  // namespace lbm
 
 int lbm_halo_pack(lbm_ctx *c, int what, int side, void *d_buf) { return lbm::halo_copy(c, what, side, d_buf, true); }
 

@@ -215,6 +215,16 @@ bool build_phi_tile_maps(lbm_ctx *c) {
 // layer pairs; 0 / negative = the defaults chosen by measurement.
 }  // namespace
 
+namespace lbm {
+int describe_params(const lbm_params *p, LatSet *set, Layout *L) {
+    const int rc = validate(p);
+    if (rc) return rc;
+    *set = lattice_set(p);
+    *L = make_layout(p);
+    return LBM_OK;
+}
+}  // namespace lbm
+
 // ------------------------------------------------------------------------------------------------ C ABI
 extern "C" {
 

@@ -134,6 +134,19 @@ def exchange_push(slabs, what: int, periodic: bool):
                 sl.halo_push(what, side, slabs[nb[side]])
 
 
+def exchange_push_mapped(slabs, what: int, periodic: bool):
+    """As :func:`exchange_push`, with the neighbour known only by its parameters and the device address of its workspace
+    (lbm_halo_push_mapped) -- the form a multi-process run takes once the workspaces are peer-mapped (CUDA IPC); here the
+    "mapped" address is simply the neighbour's own, which is how the call is tested on one GPU."""
+    world = len(slabs)
+    for r, sl in enumerate(slabs):
+        nb = neighbours(r, world, periodic)
+        for side in range(2):
+            if sl.halo[side]:
+                peer = slabs[nb[side]]
+                sl.sim.halo_push_mapped(what, side, peer.P, peer.sim.workspace_ptr)
+
+
 def exchange_dist(slab, what: int, rank: int, world: int, periodic: bool, group=None):
     """One slab per rank: pack, post all sends and receives as one batch, wait, unpack.
 
@@ -340,7 +353,7 @@ class SlabGroup:
         self.P = P
         # the slabs share a GPU: a boundary layer goes straight into the neighbour's ghost layer (one launch per cut side and
         # phase) instead of pack -> buffer -> unpack (two); push=False keeps the buffered exchange a multi-process run uses
-        self._exchange = exchange_push if push else exchange_local
+        self._exchange = exchange_push_mapped if push == "mapped" else (exchange_push if push else exchange_local)
         # the overlapped step of small slabs is launch-bound (fourteen short launches per slab and step): replay it from a CUDA
         # graph of two consecutive steps (the buffers alternate with period 2), captured across both streams, one per parity
         self.graph = graph

@@ -174,6 +174,33 @@ def test_slab_api_states(gpu):
         gpu.LBM(Pm, 64)
 
 
+def test_push_to_a_mapped_workspace(gpu, oracle_mod):
+    """lbm_halo_push_mapped: the neighbour given by its parameters and the address of its workspace only (the form a peer-mapped
+    multi-process run uses) -- same bits as the undecomposed run on a periodic box, walls within a few ulp, oracle within 1e-10."""
+    P = wl.base_params(136, 6, 11, grav=[1e-4, -2e-4, 5e-5])
+    init = _random_state(P, 67)
+    single = gpu.LBM(P, 64); single.init(*init); single.step(7)
+    o = oracle_mod.Oracle(P); o.init(*init); o.step(7)
+    for n in (2, 3):
+        g = slabs.SlabGroup(P, n, 64, overlap=True, push="mapped"); g.init(*init); g.step(7)
+        for k, v in _state(single, gpu).items():
+            assert np.array_equal(_state(g, gpu)[k], v), (n, k)
+        for a, b in zip(g.read_macro(), o.read_macro()):
+            assert np.abs(a - b).max() <= TOL64
+        g.destroy()
+    single.destroy(); o.close()
+    P, st = wl.config4_film3d(40, 24, 14, h0=5.0, amp=1.5)
+    single = gpu.LBM(P, 32); single.init(st["phi"].astype(np.float32), st["T"].astype(np.float32)); single.step(6)
+    g = slabs.SlabGroup(P, 3, 32, overlap=False, push="mapped"); g.init(st["phi"].astype(np.float32), st["T"].astype(np.float32)); g.step(6)
+    for a, b in zip(g.read_macro(), single.read_macro()):
+        assert np.abs(a.astype(np.float64) - b).max() <= ULP32
+    # a neighbour that does not fit: other row length
+    bad = dict(g.slabs[1].P, nx=P["nx"] + 2)
+    with pytest.raises(gpu.LBMError):
+        g.slabs[0].sim.halo_push_mapped(slabs.HALO_POPS, 1, bad, g.slabs[1].sim.workspace_ptr)
+    g.destroy(); single.destroy()
+
+
 def test_graph_replay_of_the_overlapped_step(gpu):
     """Small slabs replay their overlapped step from a CUDA graph of two consecutive steps captured across the compute and the
     exchange stream, one graph per buffer parity (slabs.SlabGroup, lbm_note_replay): same bits as the launches themselves, from
