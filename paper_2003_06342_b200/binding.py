@@ -324,6 +324,11 @@ class LBM:
         _check(self._L.lbm_sync(self._h), "lbm_sync")
 
     @property
+    def workspace_tensor(self):
+        """The torch tensor that holds the workspace (what a neighbouring process maps through CUDA IPC)."""
+        return self._ws
+
+    @property
     def workspace_ptr(self) -> int:
         """Device address of the workspace lent to the library (what a neighbour maps for lbm_halo_push_mapped)."""
         return int(self._ws.data_ptr())

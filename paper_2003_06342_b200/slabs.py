@@ -176,6 +176,58 @@ def exchange_dist(slab, what: int, rank: int, world: int, periodic: bool, group=
             slab.halo_unpack(what, side, src)
 
 
+class PeerTransport:
+    """Ghost-layer exchange of one slab per process WITHOUT a communication library: every process maps its neighbours'
+    workspaces through CUDA IPC (the handles travel once, over ``torch.distributed`` object collectives) and pushes its boundary
+    layers straight into their ghost layers (lbm_halo_push_mapped: one copy kernel per cut side and phase, stores over
+    NVLink / peer memory).  Ordering: after its pushes a rank records an inter-process event; a host barrier makes sure every rank
+    has recorded before anybody enqueues the wait for its neighbours' events (a wait captures the latest record at the time of the
+    call).  No kernel waits on another one; the double-buffered populations and phi arrays keep a push of step n + 1 off the
+    layers step n still reads."""
+
+    def __init__(self, slab, rank: int, world: int, periodic: bool, group=None):
+        import torch
+        import torch.distributed as dist
+        from torch.multiprocessing.reductions import reduce_tensor
+        self.slab, self.rank, self.world, self.group = slab, rank, world, group
+        self.nb = neighbours(rank, world, periodic)
+        dev = torch.cuda.current_device()
+        self.done = {what: torch.cuda.Event(enable_timing=False, interprocess=True) for what in (HALO_PHI, HALO_POPS)}
+        for ev in self.done.values():
+            ev.record(slab.sim.stream)                  # the CUDA event exists from its first record on
+        mine = {"ws": reduce_tensor(slab.sim.workspace_tensor), "P": slab.P,
+                "ev": {what: ev.ipc_handle() for what, ev in self.done.items()}}
+        infos = [None] * world
+        dist.all_gather_object(infos, mine, group=group)
+        self.peer_ws, self.peer_P, self.peer_ev = {}, {}, {}
+        for side in range(2):
+            if slab.halo[side] and self.nb[side] != rank:
+                info = infos[self.nb[side]]
+                rebuild, args = info["ws"]
+                self.peer_ws[side] = rebuild(*args)      # the neighbour's workspace, mapped into this process
+                self.peer_P[side] = info["P"]
+                self.peer_ev[side] = {what: torch.cuda.Event.from_ipc_handle(dev, h) for what, h in info["ev"].items()}
+
+    def exchange(self, what: int):
+        """On torch's CURRENT stream (the slab's calls are enqueued there too): push, record, barrier, wait."""
+        import torch
+        import torch.distributed as dist
+        s = self.slab
+        st = torch.cuda.current_stream()
+        for side in range(2):
+            if not s.halo[side]:
+                continue
+            if self.nb[side] == self.rank:
+                s.sim.halo_push(what, side, s.sim)       # a single periodic slab is its own neighbour
+            else:
+                s.sim.halo_push_mapped(what, side, self.peer_P[side], self.peer_ws[side].data_ptr())
+        self.done[what].record(st)
+        dist.barrier(group=self.group)                   # host: everybody has enqueued its pushes and recorded
+        for side in range(2):
+            if s.halo[side] and self.nb[side] != self.rank:
+                st.wait_event(self.peer_ev[side][what])  # my ghost layer of `side` was written by that neighbour
+
+
 # ------------------------------------------------------------------------------------------- overlapped schedule (host logic)
 def layer_parts(n_local: int, halo):
     """Owned layers of a slab with ``n_local`` layers (ghosts included) by role: ``boundary`` = [(first, count)] of the owned
@@ -437,10 +489,14 @@ class SlabGroup:
 class DistSlab:
     """The slab of this rank in a ``torch.distributed`` job (one process per GPU)."""
 
-    def __init__(self, P: dict, rank: int, world: int, precision: int = 64, group=None, overlap: bool = True):
+    def __init__(self, P: dict, rank: int, world: int, precision: int = 64, group=None, overlap: bool = True,
+                 transport: str = "p2p"):
+        """``transport``: "p2p" -- pack, ``torch.distributed`` point-to-point calls (NCCL over NVLink), unpack; "peer" -- the
+        neighbours' workspaces mapped through CUDA IPC and written directly (:class:`PeerTransport`; same node only)."""
         self.periodic = axis_is_periodic(P)
         import torch
         self.rank, self.world, self.group = rank, world, group
+        self.transport = transport
         self.overlap = overlap and not P.get("prescribed_u", False)
         if self.overlap:
             # kernels on a compute stream of the slab's own; packs, transfers and unpacks on the exchange stream
@@ -452,29 +508,44 @@ class DistSlab:
             self.stream = torch.cuda.current_stream()
             self.slab = Slab(P, rank, world, precision, stream=self.stream)
             self.sched = None
+        if transport == "peer" and not self.overlap:
+            # the plain schedule lets K_main run over the ghost layers and relies on the unpack that follows it in the SAME stream
+            # to overwrite the result; a neighbour's push from another process is not ordered against that kernel
+            raise ValueError("the peer transport needs the overlapped schedule (ghost layers are never computed there)")
+        self.peer = PeerTransport(self.slab, rank, world, self.periodic, group) if transport == "peer" and self.slab.has_halo else None
+
+    def _exchange(self, what):
+        if self.peer is not None:
+            self.peer.exchange(what)
+        else:
+            exchange_dist(self.slab, what, self.rank, self.world, self.periodic, self.group)
 
     def init(self, phi, T=None, u=None, p=None, local=False):
         """GLOBAL fields, or with ``local=True`` this rank's layers including the ghost copies (Slab.layer_range)."""
         import torch
         (self.slab.init_local if local else self.slab.init)(phi, T, u, p)
+        if self.peer is not None:
+            import torch.distributed as dist
+            dist.barrier(group=self.group)           # lbm_init has finished everywhere (it writes the ghost layers too) before anybody pushes
         if self.slab.has_halo:
             with torch.cuda.stream(self.stream):     # packs, transfers and unpacks of level 0 on the compute stream
-                exchange_dist(self.slab, HALO_POPS, self.rank, self.world, self.periodic, self.group)
+                self._exchange(HALO_POPS)
 
     def step(self, n: int = 1):
+        import torch
         s = self.slab
         if not s.has_halo:
             s.sim.step(n)
             return
         if self.overlap:
-            step_overlapped([s], lambda what: exchange_dist(s, what, self.rank, self.world, self.periodic, self.group),
-                            self.sched, n)
+            step_overlapped([s], self._exchange, self.sched, n)
             return
-        for k in range(n):
-            s.sim.step_phase(0)
-            exchange_dist(s, HALO_PHI, self.rank, self.world, self.periodic, self.group)
-            s.sim.step_phase(1, store_macros=(k == n - 1))
-            exchange_dist(s, HALO_POPS, self.rank, self.world, self.periodic, self.group)
+        with torch.cuda.stream(self.stream):
+            for k in range(n):
+                s.sim.step_phase(0)
+                self._exchange(HALO_PHI)
+                s.sim.step_phase(1, store_macros=(k == n - 1))
+                self._exchange(HALO_POPS)
 
     def read_macro(self):
         """Owned layers of this rank (no gather: results stay sharded)."""
