@@ -324,20 +324,20 @@ def run_slabs(args):
             raise SystemExit("bench.py: --parallelism slabs is defined for config4 (stacked along z)")
         P, _ = wl.config4_film3d(16, 16, 16)                      # parameters only
         P.update(nx=256, ny=256, nz=512 * world)
-        sim = slabs.DistSlab(P, rank, world, prec, overlap=not args.no_overlap)
+        sim = slabs.DistSlab(P, rank, world, prec, overlap=not args.no_overlap, transport=args.transport)
         z0, z1 = sim.slab.layer_range()
         _, I = wl.config4_film3d(256, 256, 512 * world, zrange=(z0, z1))
         sim.init(I["phi"], I["T"], local=True)
-        n_slabs, mode = world, "slabs x%d (one per rank, NCCL p2p ghost exchange)" % world
+        n_slabs, mode = world, "slabs x%d (one per rank, %s ghost exchange)" % (world, "NCCL p2p" if args.transport == "p2p" else "peer-memory push")
         owned = sim.slab.P["slab"]["count"] * 256 * 256
         scaling = "weak"
     elif args.parallelism == "slabs-strong":
         # the paper's decomposed runs: ONE domain cut into one slab per rank along its slowest axis,
         # e.g. --workload config3_1024x1024_q9 on 4 ranks (4 x 1024x256), config3_4096x3072_q9_mm on 8
         P, I = make_workload(args.workload)
-        sim = slabs.DistSlab(P, rank, world, prec, overlap=not args.no_overlap)
+        sim = slabs.DistSlab(P, rank, world, prec, overlap=not args.no_overlap, transport=args.transport)
         sim.init(I["phi"], I["T"])
-        n_slabs, mode = world, "one domain cut into %d slabs (one per rank, NCCL p2p ghost exchange)" % world
+        n_slabs, mode = world, "one domain cut into %d slabs (one per rank, %s ghost exchange)" % (world, "NCCL p2p" if args.transport == "p2p" else "peer-memory push")
         owned = sim.slab.P["slab"]["count"] * (P["nx"] * P["ny"] if P["nz"] > 1 else P["nx"])
         scaling = "strong"
     else:
@@ -386,6 +386,9 @@ def main():
     ap.add_argument("--parallelism", default="replicas", choices=("replicas", "slabs", "slabs-strong"),
                     help="N > 1: independent replicas (default, the bench contract), one slab of a stacked domain per rank (weak), "
                          "or ONE domain cut into one slab per rank (strong; the paper's decomposed runs)")
+    ap.add_argument("--transport", default="p2p", choices=("p2p", "peer"),
+                    help="slabs under torchrun: ghost layers by torch.distributed point-to-point calls (NCCL) or pushed into the "
+                         "neighbours' CUDA-IPC-mapped workspaces (same node)")
     ap.add_argument("--no-overlap", action="store_true", help="slabs: the plain one-stream schedule instead of boundary layers first")
     ap.add_argument("--slabs", type=int, default=0, help="cut the workload into this many slabs on ONE GPU (overhead measurement)")
     args = ap.parse_args()

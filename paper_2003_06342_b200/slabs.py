@@ -189,7 +189,10 @@ class PeerTransport:
         import torch
         import torch.distributed as dist
         from torch.multiprocessing.reductions import reduce_tensor
-        self.slab, self.rank, self.world, self.group = slab, rank, world, group
+        self.slab, self.rank, self.world = slab, rank, world
+        # the handles and the barriers are host business: a gloo group beside an NCCL job (an NCCL barrier would stall the stream)
+        self.group = group if dist.get_backend(group) == "gloo" else dist.new_group(backend="gloo")
+        group = self.group
         self.nb = neighbours(rank, world, periodic)
         dev = torch.cuda.current_device()
         self.done = {what: torch.cuda.Event(enable_timing=False, interprocess=True) for what in (HALO_PHI, HALO_POPS)}
