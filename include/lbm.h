@@ -221,6 +221,13 @@ int lbm_halo_push(lbm_ctx *c, int what, int side, lbm_ctx *peer);
  * current device).  The neighbour is taken to stand where c stands -- the slabs of a domain step in lockstep; ordering across the
  * processes (inter-process events) is the caller's. */
 int lbm_halo_push_mapped(lbm_ctx *c, int what, int side, const lbm_params *peer_params, void *d_peer_workspace);
+/* Ordering between processes without the host: lbm_stream_signal enqueues, on the context's stream, the write of `value` to the
+ * 32-bit word d_flag (typically in the neighbour's peer-mapped memory) once everything enqueued before it -- the pushes -- is
+ * visible; lbm_stream_wait holds the context's stream until the word d_flag (in this process's memory) is >= value (as a wrapping
+ * signed difference).  Both are stream memory operations of the driver: no kernel spins and no host call blocks.
+ * LBM_E_UNSUPPORTED where the driver does not offer them. */
+int lbm_stream_signal(lbm_ctx *c, void *d_flag, unsigned value);
+int lbm_stream_wait(lbm_ctx *c, void *d_flag, unsigned value);
 
 /* Copy the macroscopic fields of the current time level to HOST arrays; any pointer may be NULL.
  * h_u is [3][z][y][x].  Synchronises. */

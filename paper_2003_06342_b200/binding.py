@@ -32,7 +32,7 @@ STAGE_POSTCOLLISION, STAGE_STREAMED = 0, 1
 HALO_PHI, HALO_POPS = 0, 1
 NOALLOC_SCRATCH_BYTES = 8 << 20
 
-EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_halo_push", "lbm_halo_push_mapped", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
+EXPORTS = ["lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_set_velocity", "lbm_step_phase", "lbm_step_layers", "lbm_set_stream", "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_halo_push", "lbm_halo_push_mapped", "lbm_stream_signal", "lbm_stream_wait", "lbm_read_macro", "lbm_read_pops", "lbm_read_pops_noalloc",
            "lbm_sync", "lbm_check_finite", "lbm_state_bytes", "lbm_save_state", "lbm_load_state", "lbm_set_timing", "lbm_kernel_times", "lbm_note_replay", "lbm_step_count", "lbm_launch_count", "lbm_variant", "lbm_last_cuda_error", "lbm_strerror",
            "lbm_destroy"]
 
@@ -86,6 +86,8 @@ def load_library():
         L.lbm_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_halo_push.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_halo_push_mapped.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(lbm_params), C.c_void_p]
+        L.lbm_stream_signal.argtypes = [C.c_void_p, C.c_void_p, C.c_uint]
+        L.lbm_stream_wait.argtypes = [C.c_void_p, C.c_void_p, C.c_uint]
         L.lbm_read_macro.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.lbm_read_pops.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.lbm_read_pops_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
@@ -268,6 +270,14 @@ class LBM:
         s = make_params(peer_params, self.precision)
         _check(self._L.lbm_halo_push_mapped(self._h, int(what), int(side), C.byref(s), C.c_void_p(int(peer_workspace_ptr))),
                "lbm_halo_push_mapped")
+
+    def stream_signal(self, flag_ptr: int, value: int):
+        """lbm_stream_signal: write ``value`` to the 32-bit device word at ``flag_ptr`` after what this context has enqueued so far."""
+        _check(self._L.lbm_stream_signal(self._h, C.c_void_p(int(flag_ptr)), int(value) & 0xFFFFFFFF), "lbm_stream_signal")
+
+    def stream_wait(self, flag_ptr: int, value: int):
+        """lbm_stream_wait: hold this context's stream until the 32-bit device word at ``flag_ptr`` is >= ``value``."""
+        _check(self._L.lbm_stream_wait(self._h, C.c_void_p(int(flag_ptr)), int(value) & 0xFFFFFFFF), "lbm_stream_wait")
 
     def set_velocity(self, u):
         ptr, keep = _host_ptr(u, self.dtype, (3,) + self.shape, "u")

@@ -194,3 +194,34 @@ int lbm_halo_unpack(lbm_ctx *c, int what, int side, const void *d_buf) {
 }
 
 }  // extern "C"
+
+// ---- stream-ordered flags for the peer transport (include/lbm.h): cuStreamWriteValue32 / cuStreamWaitValue32 are executed by the
+// GPU's front end in stream order -- no kernel spins, no host call waits -- and the write is a memory barrier for everything the
+// stream did before it, so a counter written into the neighbour's (peer-mapped) memory after a push says "the ghost layer is there".
+#include <cudaTypedefs.h>
+
+namespace {
+typedef CUresult(CUDAAPI *stream_value_fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+stream_value_fn stream_value_entry(const char *name) {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint(name, &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) return nullptr;
+    return reinterpret_cast<stream_value_fn>(p);
+}
+}  // namespace
+
+extern "C" int lbm_stream_signal(lbm_ctx *c, void *d_flag, unsigned value) {
+    if (!c || !d_flag) return LBM_E_INVALID;
+    static stream_value_fn fn = stream_value_entry("cuStreamWriteValue32");
+    if (!fn) return LBM_E_UNSUPPORTED;
+    if (fn(c->stream, reinterpret_cast<CUdeviceptr>(d_flag), value, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS) return LBM_E_CUDA;
+    return LBM_OK;
+}
+
+extern "C" int lbm_stream_wait(lbm_ctx *c, void *d_flag, unsigned value) {
+    if (!c || !d_flag) return LBM_E_INVALID;
+    static stream_value_fn fn = stream_value_entry("cuStreamWaitValue32");
+    if (!fn) return LBM_E_UNSUPPORTED;
+    if (fn(c->stream, reinterpret_cast<CUdeviceptr>(d_flag), value, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS) return LBM_E_CUDA;
+    return LBM_OK;
+}

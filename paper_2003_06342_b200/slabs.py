@@ -180,43 +180,57 @@ class PeerTransport:
     """Ghost-layer exchange of one slab per process WITHOUT a communication library: every process maps its neighbours'
     workspaces through CUDA IPC (the handles travel once, over ``torch.distributed`` object collectives) and pushes its boundary
     layers straight into their ghost layers (lbm_halo_push_mapped: one copy kernel per cut side and phase, stores over
-    NVLink / peer memory).  Ordering: after its pushes a rank records an inter-process event; a host barrier makes sure every rank
-    has recorded before anybody enqueues the wait for its neighbours' events (a wait captures the latest record at the time of the
-    call).  No kernel waits on another one; the double-buffered populations and phi arrays keep a push of step n + 1 off the
-    layers step n still reads."""
+    NVLink / peer memory).  Ordering, ``sync="flags"`` (the default): after its pushes a rank enqueues the write of the exchange's
+    sequence number into a word of the neighbour's (mapped) memory, and enqueues a wait on its own word for the neighbour's --
+    stream memory operations of the driver (lbm_stream_signal / lbm_stream_wait): nothing on the host waits and no kernel spins.
+    ``sync="events"``: an inter-process event per exchange kind and a host barrier that makes sure every rank has recorded before
+    anybody enqueues the wait (a wait captures the latest record at the time of the call).  In both, the double-buffered
+    populations and phi arrays keep a push of step n + 1 off the layers step n still reads."""
 
-    def __init__(self, slab, rank: int, world: int, periodic: bool, group=None):
+    def __init__(self, slab, rank: int, world: int, periodic: bool, group=None, sync: str = "flags"):
         import torch
         import torch.distributed as dist
         from torch.multiprocessing.reductions import reduce_tensor
-        self.slab, self.rank, self.world = slab, rank, world
+        self.slab, self.rank, self.world, self.sync = slab, rank, world, sync
         # the handles and the barriers are host business: a gloo group beside an NCCL job (an NCCL barrier would stall the stream)
         self.group = group if dist.get_backend(group) == "gloo" else dist.new_group(backend="gloo")
         group = self.group
         self.nb = neighbours(rank, world, periodic)
         dev = torch.cuda.current_device()
+        self.flags = torch.zeros(4, dtype=torch.int32, device="cuda")     # word [2 * what + side]: last exchange received there
+        self.seq = {HALO_PHI: 0, HALO_POPS: 0}
         self.done = {what: torch.cuda.Event(enable_timing=False, interprocess=True) for what in (HALO_PHI, HALO_POPS)}
         for ev in self.done.values():
             ev.record(slab.sim.stream)                  # the CUDA event exists from its first record on
-        mine = {"ws": reduce_tensor(slab.sim.workspace_tensor), "P": slab.P,
+        torch.cuda.synchronize()
+        mine = {"ws": reduce_tensor(slab.sim.workspace_tensor), "flags": reduce_tensor(self.flags), "P": slab.P,
                 "ev": {what: ev.ipc_handle() for what, ev in self.done.items()}}
         infos = [None] * world
         dist.all_gather_object(infos, mine, group=group)
-        self.peer_ws, self.peer_P, self.peer_ev = {}, {}, {}
+        self.peer_ws, self.peer_flags, self.peer_P, self.peer_ev = {}, {}, {}, {}
         for side in range(2):
             if slab.halo[side] and self.nb[side] != rank:
                 info = infos[self.nb[side]]
                 rebuild, args = info["ws"]
                 self.peer_ws[side] = rebuild(*args)      # the neighbour's workspace, mapped into this process
+                rebuild, args = info["flags"]
+                self.peer_flags[side] = rebuild(*args)
                 self.peer_P[side] = info["P"]
                 self.peer_ev[side] = {what: torch.cuda.Event.from_ipc_handle(dev, h) for what, h in info["ev"].items()}
 
+    def ready(self):
+        """Host barrier (once, after lbm_init, which writes the ghost layers too): nobody pushes into a workspace still being set up."""
+        import torch.distributed as dist
+        dist.barrier(group=self.group)
+
     def exchange(self, what: int):
-        """On torch's CURRENT stream (the slab's calls are enqueued there too): push, record, barrier, wait."""
+        """On torch's CURRENT stream (the slab's calls are enqueued there too): push, signal, wait."""
         import torch
         import torch.distributed as dist
         s = self.slab
         st = torch.cuda.current_stream()
+        self.seq[what] += 1
+        seq = self.seq[what]
         for side in range(2):
             if not s.halo[side]:
                 continue
@@ -224,6 +238,13 @@ class PeerTransport:
                 s.sim.halo_push(what, side, s.sim)       # a single periodic slab is its own neighbour
             else:
                 s.sim.halo_push_mapped(what, side, self.peer_P[side], self.peer_ws[side].data_ptr())
+                if self.sync == "flags":                 # my push lands in the neighbour's ghost layer of the OPPOSITE side
+                    s.sim.stream_signal(self.peer_flags[side].data_ptr() + 4 * (2 * what + (1 - side)), seq)
+        if self.sync == "flags":
+            for side in range(2):
+                if s.halo[side] and self.nb[side] != self.rank:
+                    s.sim.stream_wait(self.flags.data_ptr() + 4 * (2 * what + side), seq)
+            return
         self.done[what].record(st)
         dist.barrier(group=self.group)                   # host: everybody has enqueued its pushes and recorded
         for side in range(2):
@@ -493,7 +514,7 @@ class DistSlab:
     """The slab of this rank in a ``torch.distributed`` job (one process per GPU)."""
 
     def __init__(self, P: dict, rank: int, world: int, precision: int = 64, group=None, overlap: bool = True,
-                 transport: str = "p2p"):
+                 transport: str = "p2p", peer_sync: str = "flags"):
         """``transport``: "p2p" -- pack, ``torch.distributed`` point-to-point calls (NCCL over NVLink), unpack; "peer" -- the
         neighbours' workspaces mapped through CUDA IPC and written directly (:class:`PeerTransport`; same node only)."""
         self.periodic = axis_is_periodic(P)
@@ -515,7 +536,8 @@ class DistSlab:
             # the plain schedule lets K_main run over the ghost layers and relies on the unpack that follows it in the SAME stream
             # to overwrite the result; a neighbour's push from another process is not ordered against that kernel
             raise ValueError("the peer transport needs the overlapped schedule (ghost layers are never computed there)")
-        self.peer = PeerTransport(self.slab, rank, world, self.periodic, group) if transport == "peer" and self.slab.has_halo else None
+        self.peer = (PeerTransport(self.slab, rank, world, self.periodic, group, sync=peer_sync)
+                     if transport == "peer" and self.slab.has_halo else None)
 
     def _exchange(self, what):
         if self.peer is not None:
@@ -528,8 +550,7 @@ class DistSlab:
         import torch
         (self.slab.init_local if local else self.slab.init)(phi, T, u, p)
         if self.peer is not None:
-            import torch.distributed as dist
-            dist.barrier(group=self.group)           # lbm_init has finished everywhere (it writes the ghost layers too) before anybody pushes
+            self.peer.ready()                        # lbm_init has finished everywhere (it writes the ghost layers too) before anybody pushes
         if self.slab.has_halo:
             with torch.cuda.stream(self.stream):     # packs, transfers and unpacks of level 0 on the compute stream
                 self._exchange(HALO_POPS)

@@ -1,5 +1,6 @@
 """DistSlab with the "peer" transport: one slab per PROCESS, the neighbours' workspaces mapped through CUDA IPC and written
-directly by lbm_halo_push_mapped, inter-process events for the ordering -- no communication library on the data path.  CUDA IPC
+directly by lbm_halo_push_mapped; ordering by stream memory operations on flags in mapped memory (lbm_stream_signal / lbm_stream_wait:
+no host synchronisation at all) or by inter-process events and a host barrier -- no communication library on the data path.  CUDA IPC
 works between two processes on ONE device as well, so this is the multi-process slab path running on the one GPU available:
 two processes, both on cuda:0, against the whole-domain oracle.  (What it cannot show is NVLink: on one GPU the "peer" memory is
 local.  No kernel waits on another one -- the ordering is stream waits on events -- so the two processes merely time-slice.)"""
@@ -15,7 +16,7 @@ from test_oracle_bruteforce import _random_state
 pytestmark = pytest.mark.gpu
 
 
-def _worker(rank, world, port, P, init, overlap, precision, nsteps, out):
+def _worker(rank, world, port, P, init, sync, precision, nsteps, out):
     import torch
     import torch.distributed as dist
     from paper_2003_06342_b200 import slabs
@@ -23,7 +24,7 @@ def _worker(rank, world, port, P, init, overlap, precision, nsteps, out):
     torch.cuda.set_device(0)                       # every rank on the same device
     dist.init_process_group("gloo", rank=rank, world_size=world)     # host collectives only: handles, barriers
     dt = np.float64 if precision == 64 else np.float32
-    sim = slabs.DistSlab(P, rank, world, precision, overlap=overlap, transport="peer")
+    sim = slabs.DistSlab(P, rank, world, precision, overlap=True, transport="peer", peer_sync=sync)
     sim.init(*[None if a is None else a.astype(dt) for a in init])
     sim.step(3)
     sim.step(nsteps - 3)
@@ -33,7 +34,7 @@ def _worker(rank, world, port, P, init, overlap, precision, nsteps, out):
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("case", ["periodic", "walls", "walls-fp32", "periodic-3ranks"])
+@pytest.mark.parametrize("case", ["periodic", "walls", "walls-fp32", "periodic-3ranks", "periodic-events", "walls-events"])
 def test_peer_transport_two_processes_one_gpu(oracle_mod, case):
     import torch.multiprocessing as mp
     world = 3 if "3ranks" in case else 2
@@ -49,7 +50,7 @@ def test_peer_transport_two_processes_one_gpu(oracle_mod, case):
     s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
-    procs = [ctx.Process(target=_worker, args=(r, world, port, P, init, True, precision, nsteps, out))
+    procs = [ctx.Process(target=_worker, args=(r, world, port, P, init, "events" if "events" in case else "flags", precision, nsteps, out))
              for r in range(world)]
     for p in procs:
         p.start()
